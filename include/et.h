@@ -1,0 +1,162 @@
+/*
+ * et.h -- C ABI of libet.so: the energy-test hot path of arXiv:1612.04705 on
+ * one NVIDIA B200 (sm_100a).  Citations are /root/reference/PAPER.md:<line>.
+ *
+ * What the library computes
+ *   psi_ij = exp(-d_ij^2 / (2 sigma^2)), d_ij the Euclidean distance of events
+ *   i and j in the caller's phase-space coordinates;
+ *   T = sum_{i<j in X} psi/(n(n-1)) + sum_{i<j in Xbar} psi/(nbar(nbar-1))
+ *       - sum_{i in X, j in Xbar} psi/(n nbar)                    (Eq. 2);
+ *   its per-event-weighted form (Sect. 3; reading R7);
+ *   the permutation p-value: fraction of permutation T values greater than the
+ *   observed T; the Sect. 5 sample split by the sign of a triple
+ *   product and the P-odd test (I+IV) vs (II+III).
+ *
+ * Conventions (all entry points)
+ *   - Coordinates are row-major [n][dim], dtype per `et_dtype`; weights and
+ *     momenta are always double.  `mem` says where EVERY array argument of the
+ *     call lives except those documented as host: ET_HOST (plain host memory;
+ *     the library stages it to the device itself) or ET_DEVICE (device pointers
+ *     on the context's device, e.g. from PyTorch).  Inputs are never modified
+ *     and never freed by the library.
+ *   - Result structs and T_perm are HOST memory owned by the caller.
+ *   - Pooled event index: X events are 0..n-1, Xbar events n..n+nbar-1.
+ *   - The context owns a stream (or borrows the caller's), all scratch and the
+ *     label buffers; it is not thread-safe (one context per host thread).
+ *   - Every call is complete (stream-synchronised) on return.
+ *   - On any status != ET_OK the outputs are untouched and et_last_error()
+ *     explains.  There is no CPU fallback: without a CUDA device et_create
+ *     fails with ET_ERR_CUDA.
+ *   - Limits: 1 <= dim <= ET_MAX_DIM, n >= 2, nbar >= 2, n + nbar < 2^31,
+ *     1 <= nperm <= ET_MAX_NPERM.
+ */
+#ifndef ET_H_
+#define ET_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ET_MAX_DIM 8
+#define ET_MAX_NPERM 65536
+
+typedef struct et_ctx et_ctx; /* opaque */
+
+typedef enum {
+    ET_OK = 0,
+    ET_ERR_INVALID = -1,    /* null pointer, n < 2, nbar < 2, dim out of range, nperm out of range */
+    ET_ERR_SIGMA = -2,      /* sigma <= 0 or not finite                                            */
+    ET_ERR_NONFINITE = -3,  /* NaN/Inf in coordinates or weights (checked on the device in prep)   */
+    ET_ERR_DEGENERATE = -4, /* weighted: W <= 1 or Wbar <= 1 for the observed split                */
+    ET_ERR_NOMEM = -5,
+    ET_ERR_CUDA = -6
+} et_status;
+
+typedef enum { ET_F32 = 0, ET_F64 = 1 } et_dtype;
+typedef enum { ET_HOST = 0, ET_DEVICE = 1 } et_memspace;
+
+/* T and its parts, in the order of Eq. 2: T = T_xx + T_bb - T_xb. */
+typedef struct {
+    double T, T_xx, T_bb, T_xb; /* normalised terms                                              */
+    double S_xx, S_bb, S_xb;    /* raw psi sums (i<j within, all pairs across), weighted if any  */
+    double W, Wbar;             /* n, nbar, or the weight sums                                   */
+    int64_t n_pairs;            /* unordered pairs that enter T                                  */
+} et_result;
+
+typedef struct {
+    et_result observed;
+    double p_value;   /* count_gt / nperm  (strict >; reading R3)                   */
+    int64_t count_gt; /* #{p : T_p > T_obs}                                                       */
+    int64_t n_near;   /* #{p : |T_p - T_obs| <= 1e-9 (|T_xx|+|T_bb|+|T_xb|)} or T_p NaN (R5, R10) */
+    int64_t nperm;
+} et_perm_result;
+
+typedef struct {
+    int64_t count[4];    /* N(I), N(II), N(III), N(IV) of Eq. 4               */
+    et_result p_even;    /* (I+II) vs (III+IV): the default X vs Xbar test        */
+    et_perm_result p_odd;/* (I+IV) vs (II+III) with its permutation p-value       */
+} et_podd_result;
+
+/* Device-side timings of the last call, CUDA events on the context's stream. */
+typedef struct {
+    double ms_total;   /* whole call on the device, staging copies included                      */
+    double ms_pairs;   /* the O(N^2) kernels only (all-pairs, row sums, permutation sums)         */
+    double ms_labels;  /* permutation label generation                                            */
+    int64_t launches;  /* kernels launched by the call                                            */
+    int64_t pair_evals;/* psi evaluations the kernels performed (padding and diagonals included)  */
+} et_stats;
+
+/* Options for et_set_option. */
+typedef enum {
+    ET_OPT_PERM_KERNEL = 0 /* 0: CUDA-core 32-permutations-per-psi kernel (default)             */
+} et_option;
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t to
+ * borrow, or NULL for a library-owned stream. */
+et_status et_create(et_ctx **ctx, int device, void *cuda_stream);
+void et_destroy(et_ctx *ctx);
+/* Context-owned explanation of the last non-OK status; never freed by the caller. */
+const char *et_last_error(const et_ctx *ctx);
+et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value);
+et_status et_get_stats(const et_ctx *ctx, et_stats *out);
+const char *et_version(void);
+
+/* Eq. 2 for samples x[n][dim], xbar[nbar][dim]. */
+et_status et_T(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar,
+               int dim, et_dtype dtype, et_memspace mem, double sigma, et_result *out);
+
+/* Per-event-weighted Eq. 2 (reading R7): psi_ij -> w_i w_j psi_ij,
+ * n -> W = sum of weights.  wx[n], wxbar[nbar] double, same memory space. */
+et_status et_T_weighted(et_ctx *ctx, const void *x, const double *wx, int64_t n,
+                        const void *xbar, const double *wxbar, int64_t nbar,
+                        int dim, et_dtype dtype, et_memspace mem, double sigma, et_result *out);
+
+/* Permutation test.  Permutation p reassigns the pooled events
+ * to samples of the original sizes by the rule of reading R4 (Philox4x32-10
+ * keys, the n smallest composites go to X); weights (both NULL or both given)
+ * travel with their events.  T_perm[nperm] (host) receives the
+ * permutation T values; a degenerate weighted split gives NaN and is not
+ * counted.  The observed T goes through the same kernels as the T_p. */
+et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int64_t n,
+                              const void *xbar, const double *wxbar, int64_t nbar,
+                              int dim, et_dtype dtype, et_memspace mem, double sigma,
+                              int64_t nperm, uint64_t seed, double *T_perm, et_perm_result *out);
+
+/* Sect. 5 split (Eq. 4): C = pB . (pC x pD), momenta [n][3]
+ * double in the mother rest frame.  positive[i] = 1 iff C > 0 (is_conjugate = 0)
+ * or -C > 0 (is_conjugate = 1, momenta of the C-conjugate particles); C == 0 is
+ * negative (reading R11).  `positive` lives in `mem`; *n_positive is host. */
+et_status et_podd_split(et_ctx *ctx, const double *pB, const double *pC, const double *pD,
+                        int64_t n, int is_conjugate, et_memspace mem,
+                        uint8_t *positive, int64_t *n_positive);
+
+/* P-odd test: split X by C_T and Xbar by -Cbar_T (momenta
+ * mom_x[n][3][3], mom_xbar[nbar][3][3] = (pB, pC, pD) per event), form
+ * A = I + IV and B = II + III in that order (each part in input order), run the
+ * permutation test on (A, B) in the same coordinates, and return the P-even T
+ * of (I+II) vs (III+IV) from the same pass. */
+et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t n,
+                       const void *xbar, const double *mom_xbar, int64_t nbar,
+                       int dim, et_dtype dtype, et_memspace mem, double sigma,
+                       int64_t nperm, uint64_t seed, double *T_perm, et_podd_result *out);
+
+/* Test hook: the permutation labels of reading R4, bit-packed,
+ * mask[i * ceil(nperm/32) + (p >> 5)] bit (p & 31) = 1 iff pooled event i is in
+ * sample X of permutation p.  `mask` lives in `mem`. */
+et_status et_perm_labels(et_ctx *ctx, int64_t N, int64_t n, int64_t nperm, uint64_t seed,
+                         et_memspace mem, uint32_t *mask);
+
+/* Test hook: per-row class sums for the listed pooled rows (host int64),
+ *   r_x[k] = sum_{j in X, j != i} w_j psi_ij,  r_xbar[k] = sum_{j in Xbar, j != i} w_j psi_ij
+ * (w = 1 when wx == wxbar == NULL).  r_x, r_xbar are host arrays [nrows]. */
+et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n,
+                      const void *xbar, const double *wxbar, int64_t nbar,
+                      int dim, et_dtype dtype, et_memspace mem, double sigma,
+                      const int64_t *rows, int64_t nrows, double *r_x, double *r_xbar);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ET_H_ */

@@ -1,0 +1,293 @@
+"""Thin ctypes front of libet.so (include/et.h): argument marshalling only.
+
+Every step of the path runs inside the CUDA library; this module turns numpy
+arrays (host memory) or torch CUDA tensors (device memory) into the plain
+pointers and sizes of the C ABI and copies the result structs into dataclasses.
+There is no CPU fallback: if libet.so is missing, cannot be loaded, or no CUDA
+device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libet.so")
+
+ET_OK = 0
+ET_F32, ET_F64 = 0, 1
+ET_HOST, ET_DEVICE = 0, 1
+ET_OPT_PERM_KERNEL = 0
+STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ERR_NONFINITE", -4: "ET_ERR_DEGENERATE",
+                -5: "ET_ERR_NOMEM", -6: "ET_ERR_CUDA"}
+
+# every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
+SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
+           "et_T_weighted", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+
+
+class EtError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+class _Result(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("T", "T_xx", "T_bb", "T_xb", "S_xx", "S_bb", "S_xb", "W", "Wbar")] + [
+        ("n_pairs", C.c_int64)]
+
+
+class _PermResult(C.Structure):
+    _fields_ = [("observed", _Result), ("p_value", C.c_double), ("count_gt", C.c_int64), ("n_near", C.c_int64),
+                ("nperm", C.c_int64)]
+
+
+class _PoddResult(C.Structure):
+    _fields_ = [("count", C.c_int64 * 4), ("p_even", _Result), ("p_odd", _PermResult)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("ms_total", C.c_double), ("ms_pairs", C.c_double), ("ms_labels", C.c_double), ("launches", C.c_int64),
+                ("pair_evals", C.c_int64)]
+
+
+@dataclass
+class Result:
+    T: float
+    T_xx: float
+    T_bb: float
+    T_xb: float
+    S_xx: float
+    S_bb: float
+    S_xb: float
+    W: float
+    Wbar: float
+    n_pairs: int
+
+    @property
+    def term_scale(self) -> float:
+        return abs(self.T_xx) + abs(self.T_bb) + abs(self.T_xb)
+
+
+@dataclass
+class PermResult:
+    observed: Result
+    p_value: float
+    count_gt: int
+    n_near: int
+    nperm: int
+    T_perm: np.ndarray
+
+
+@dataclass
+class PoddResult:
+    count: tuple
+    p_even: Result
+    p_odd: PermResult
+
+
+@dataclass
+class Stats:
+    ms_total: float
+    ms_pairs: float
+    ms_labels: float
+    launches: int
+    pair_evals: int
+
+
+_lib = None
+
+
+def lib():
+    """Loads libet.so; raises if the CUDA extension has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1612_04705_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.et_last_error.restype = C.c_char_p
+        L.et_last_error.argtypes = [C.c_void_p]
+        L.et_version.restype = C.c_char_p
+        L.et_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
+        L.et_destroy.argtypes = [C.c_void_p]
+        L.et_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def _res(r: _Result) -> Result:
+    return Result(*(getattr(r, k) for k, _ in _Result._fields_))
+
+
+class _Arr:
+    """A pointer plus what the ABI needs to know about it."""
+
+    def __init__(self, ptr, dtype, mem, shape, keep):
+        self.ptr, self.dtype, self.mem, self.shape, self.keep = ptr, dtype, mem, shape, keep
+
+
+def _is_torch(a) -> bool:
+    return type(a).__module__.startswith("torch")
+
+
+def _marshal(a, want=None) -> _Arr:
+    """numpy array -> host pointer; torch CUDA tensor -> device pointer.  `want` forces a dtype ("f64")."""
+    if a is None:
+        return _Arr(None, None, None, None, None)
+    if _is_torch(a):
+        import torch
+
+        if want == "f64" and a.dtype != torch.float64:
+            a = a.double()
+        if a.dtype not in (torch.float32, torch.float64, torch.uint8, torch.int32, torch.uint32):
+            a = a.double()
+        a = a.contiguous()
+        mem = ET_DEVICE if a.is_cuda else ET_HOST
+        dt = ET_F32 if a.dtype == torch.float32 else ET_F64
+        return _Arr(C.c_void_p(a.data_ptr()), dt, mem, tuple(a.shape), a)
+    a = np.asarray(a)
+    if want == "f64" or a.dtype not in (np.float32, np.float64):
+        a = a.astype(np.float64)
+    a = np.ascontiguousarray(a)
+    dt = ET_F32 if a.dtype == np.float32 else ET_F64
+    return _Arr(C.c_void_p(a.ctypes.data), dt, ET_HOST, a.shape, a)
+
+
+def _coords(x, xbar):
+    ax, ab = _marshal(x), _marshal(xbar)
+    if ax.mem != ab.mem or ax.dtype != ab.dtype:
+        raise ValueError("x and xbar must share memory space and dtype")
+    if len(ax.shape) == 1:
+        ax.shape, ab.shape = (ax.shape[0], 1), (ab.shape[0], 1)
+    if len(ax.shape) != 2 or len(ab.shape) != 2 or ax.shape[1] != ab.shape[1]:
+        raise ValueError("x and xbar must be [n, dim] and [nbar, dim]")
+    return ax, ab
+
+
+class Context:
+    """One et_ctx: a device, a stream and the scratch of the library.  Not thread-safe."""
+
+    def __init__(self, device: int = 0, stream=None):
+        self._h = C.c_void_p()
+        L = lib()
+        sp = None
+        if stream is not None:
+            sp = C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+        st = L.et_create(C.byref(self._h), device, sp)
+        if st != ET_OK:
+            self._h = C.c_void_p()
+            raise EtError(st, "et_create failed (no CUDA device? there is no CPU fallback)")
+
+    def close(self):
+        if self._h:
+            lib().et_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check(self, st):
+        if st != ET_OK:
+            raise EtError(st, lib().et_last_error(self._h).decode())
+
+    def set_option(self, opt: int, value: int):
+        self._check(lib().et_set_option(self._h, C.c_int(opt), C.c_int64(value)))
+
+    def stats(self) -> Stats:
+        s = _Stats()
+        self._check(lib().et_get_stats(self._h, C.byref(s)))
+        return Stats(s.ms_total, s.ms_pairs, s.ms_labels, s.launches, s.pair_evals)
+
+    # ---------------------------------------------------------------- Eq. 2
+    def T(self, x, xbar, sigma: float) -> Result:
+        ax, ab = _coords(x, xbar)
+        out = _Result()
+        self._check(lib().et_T(self._h, ax.ptr, C.c_int64(ax.shape[0]), ab.ptr, C.c_int64(ab.shape[0]), C.c_int(ax.shape[1]),
+                               C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
+        return _res(out)
+
+    def T_weighted(self, x, wx, xbar, wxbar, sigma: float) -> Result:
+        ax, ab = _coords(x, xbar)
+        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
+        if awx.mem != ax.mem or awb.mem != ax.mem:
+            raise ValueError("weights must live where the coordinates live")
+        out = _Result()
+        self._check(lib().et_T_weighted(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
+                                        C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
+        return _res(out)
+
+    # ---------------------------------------------------------------- permutation test
+    def permutation_test(self, x, xbar, sigma: float, nperm: int, seed: int, wx=None, wxbar=None) -> PermResult:
+        ax, ab = _coords(x, xbar)
+        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
+        if wx is not None and (awx.mem != ax.mem or awb.mem != ax.mem):
+            raise ValueError("weights must live where the coordinates live")
+        Tp = np.zeros(max(int(nperm), 1), dtype=np.float64)
+        out = _PermResult()
+        self._check(lib().et_permutation_test(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr,
+                                              C.c_int64(ab.shape[0]), C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem),
+                                              C.c_double(sigma), C.c_int64(nperm), C.c_uint64(seed),
+                                              Tp.ctypes.data_as(C.c_void_p), C.byref(out)))
+        return PermResult(_res(out.observed), out.p_value, out.count_gt, out.n_near, out.nperm, Tp)
+
+    # ---------------------------------------------------------------- Sect. 5
+    def podd_split(self, pB, pC, pD, is_conjugate: bool):
+        aB, aC, aD = _marshal(pB, "f64"), _marshal(pC, "f64"), _marshal(pD, "f64")
+        n = aB.shape[0]
+        cnt = C.c_int64(0)
+        if aB.mem == ET_DEVICE:
+            import torch
+
+            pos = torch.empty(n, dtype=torch.uint8, device=aB.keep.device)
+            pp = C.c_void_p(pos.data_ptr())
+        else:
+            pos = np.zeros(n, dtype=np.uint8)
+            pp = pos.ctypes.data_as(C.c_void_p)
+        self._check(lib().et_podd_split(self._h, aB.ptr, aC.ptr, aD.ptr, C.c_int64(n), C.c_int(int(is_conjugate)),
+                                        C.c_int(aB.mem), pp, C.byref(cnt)))
+        return pos, int(cnt.value)
+
+    def podd_test(self, x, mom_x, xbar, mom_xbar, sigma: float, nperm: int, seed: int) -> PoddResult:
+        ax, ab = _coords(x, xbar)
+        amx, amb = _marshal(mom_x, "f64"), _marshal(mom_xbar, "f64")
+        if amx.mem != ax.mem or amb.mem != ax.mem:
+            raise ValueError("momenta must live where the coordinates live")
+        Tp = np.zeros(max(int(nperm), 1), dtype=np.float64)
+        out = _PoddResult()
+        self._check(lib().et_podd_test(self._h, ax.ptr, amx.ptr, C.c_int64(ax.shape[0]), ab.ptr, amb.ptr, C.c_int64(ab.shape[0]),
+                                       C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma),
+                                       C.c_int64(nperm), C.c_uint64(seed), Tp.ctypes.data_as(C.c_void_p), C.byref(out)))
+        po = out.p_odd
+        return PoddResult(tuple(out.count), _res(out.p_even),
+                          PermResult(_res(po.observed), po.p_value, po.count_gt, po.n_near, po.nperm, Tp))
+
+    # ---------------------------------------------------------------- test hooks
+    def perm_labels(self, N: int, n: int, nperm: int, seed: int) -> np.ndarray:
+        mask = np.zeros((N, (nperm + 31) // 32), dtype=np.uint32)
+        self._check(lib().et_perm_labels(self._h, C.c_int64(N), C.c_int64(n), C.c_int64(nperm), C.c_uint64(seed),
+                                         C.c_int(ET_HOST), mask.ctypes.data_as(C.c_void_p)))
+        return mask
+
+    def row_sums(self, x, xbar, sigma: float, rows, wx=None, wxbar=None):
+        ax, ab = _coords(x, xbar)
+        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
+        rows = np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
+        rx, rb = np.zeros(len(rows)), np.zeros(len(rows))
+        self._check(lib().et_row_sums(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
+                                      C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma),
+                                      rows.ctypes.data_as(C.c_void_p), C.c_int64(len(rows)),
+                                      rx.ctypes.data_as(C.c_void_p), rb.ctypes.data_as(C.c_void_p)))
+        return rx, rb

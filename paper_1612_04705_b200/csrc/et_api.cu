@@ -1,0 +1,928 @@
+// et_api.cu -- host side of libet.so: context, argument checking, staging, kernel orchestration.
+// The C ABI is declared in include/et.h.  Nothing here computes on the CPU beyond O(1) bookkeeping: every step
+// of the path (prep, split, labels, all-pairs sums, permutation sums, the statistic and the p-value) is a kernel.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/et.h"
+#include "et_kernels.cuh"
+
+using namespace et;
+
+namespace {
+
+struct Buf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+struct Layout {
+    int ncls = 2;
+    long long n = 0, nbar = 0, N = 0, npad = 0;
+    long long seg_first[kMaxCls + 1] = {0};  // first pooled (label) index of each class segment
+    long long seg_count[kMaxCls] = {0};
+    long long seg_pos[kMaxCls + 1] = {0};    // first padded row of each class segment
+    long long n_a = 0;                       // size of the first sample of the two-sample test (classes < split)
+    int split = 1;                           // classes [0, split) form sample A, the rest sample B
+};
+
+}  // namespace
+
+struct et_ctx {
+    int device = 0;
+    int num_sms = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    char err[512] = {0};
+    // scratch (grow-only)
+    Buf in_x, in_xbar, in_wx, in_wxbar, in_mx, in_mb, in_aux;
+    Buf rec, tilecls, partials, sums, rowsum, mask, sel, hist, partQ, Q, partRW, RW, mm, flag, counter;
+    Buf src, posx, posb, blkcnt, totals, clsw, clssum, result, tperm, rows, rowsout, count64;
+    void *pinned = nullptr;
+    size_t pinned_cap = 0;
+    // events / stats
+    cudaEvent_t ev[8] = {nullptr};
+    et_stats stats = {};
+    double acc_pairs_ms = 0, acc_labels_ms = 0;
+    int64_t opt_perm_kernel = 0;
+};
+
+namespace {
+
+et_status fail(et_ctx *c, et_status st, const char *fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return st;
+}
+
+#define CUDA_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? ET_ERR_NOMEM : ET_ERR_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                         \
+    } while (0)
+#define ET_TRY(expr)                     \
+    do {                                 \
+        et_status s_ = (expr);           \
+        if (s_ != ET_OK) return s_;      \
+    } while (0)
+
+et_status ensure(et_ctx *ctx, Buf &b, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    if (b.cap >= bytes) return ET_OK;
+    if (b.p) CUDA_TRY(cudaFree(b.p));
+    b.p = nullptr;
+    b.cap = 0;
+    CUDA_TRY(cudaMalloc(&b.p, bytes));
+    b.cap = bytes;
+    return ET_OK;
+}
+
+et_status ensure_pinned(et_ctx *ctx, size_t bytes)
+{
+    if (ctx->pinned_cap >= bytes) return ET_OK;
+    if (ctx->pinned) CUDA_TRY(cudaFreeHost(ctx->pinned));
+    ctx->pinned = nullptr;
+    ctx->pinned_cap = 0;
+    CUDA_TRY(cudaMallocHost(&ctx->pinned, bytes));
+    ctx->pinned_cap = bytes;
+    return ET_OK;
+}
+
+// Returns a device pointer for an input array: the pointer itself (ET_DEVICE) or a staged copy (ET_HOST).
+et_status stage_in(et_ctx *ctx, const void *p, size_t bytes, et_memspace mem, Buf &b, const void **out)
+{
+    if (!p) { *out = nullptr; return ET_OK; }
+    if (mem == ET_DEVICE) { *out = p; return ET_OK; }
+    ET_TRY(ensure(ctx, b, bytes));
+    CUDA_TRY(cudaMemcpyAsync(b.p, p, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    *out = b.p;
+    return ET_OK;
+}
+
+inline size_t elem_size(et_dtype t) { return t == ET_F32 ? 4 : 8; }
+
+et_status check_common(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, int dim, et_dtype dtype,
+                       et_memspace mem, double sigma)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!x || !xbar) return fail(ctx, ET_ERR_INVALID, "null coordinate pointer");
+    if (n < 2 || nbar < 2) return fail(ctx, ET_ERR_INVALID, "n and nbar must be >= 2 (Eq. 2 divides by n(n-1)); got %lld, %lld", (long long)n, (long long)nbar);
+    if (n + nbar >= (1ll << 31)) return fail(ctx, ET_ERR_INVALID, "n + nbar must be < 2^31");
+    if (dim < 1 || dim > ET_MAX_DIM) return fail(ctx, ET_ERR_INVALID, "dim must be in 1..%d; got %d", ET_MAX_DIM, dim);
+    if (dtype != ET_F32 && dtype != ET_F64) return fail(ctx, ET_ERR_INVALID, "bad dtype");
+    if (mem != ET_HOST && mem != ET_DEVICE) return fail(ctx, ET_ERR_INVALID, "bad memspace");
+    if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(ctx, ET_ERR_SIGMA, "sigma must be finite and > 0");
+    return ET_OK;
+}
+
+inline long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
+
+void layout_two(Layout &L, long long n, long long nbar)
+{
+    L.ncls = 2;
+    L.n = n; L.nbar = nbar; L.N = n + nbar;
+    L.seg_count[0] = n; L.seg_count[1] = nbar;
+    L.seg_first[0] = 0; L.seg_first[1] = n; L.seg_first[2] = n + nbar;
+    L.seg_pos[0] = 0; L.seg_pos[1] = round_up(n, kPad); L.seg_pos[2] = L.seg_pos[1] + round_up(nbar, kPad);
+    L.npad = L.seg_pos[2];
+    L.split = 1;
+    L.n_a = n;
+}
+
+void layout_four(Layout &L, long long n, long long nbar, const long long cnt[4])
+{
+    L.ncls = 4;
+    L.n = n; L.nbar = nbar; L.N = n + nbar;
+    long long first = 0, pos = 0;
+    for (int c = 0; c < 4; ++c) {
+        L.seg_count[c] = cnt[c];
+        L.seg_first[c] = first;
+        L.seg_pos[c] = pos;
+        first += cnt[c];
+        pos += round_up(cnt[c], kPad);
+    }
+    L.seg_first[4] = first;
+    L.seg_pos[4] = pos;
+    L.npad = pos;
+    L.split = 2;
+    L.n_a = cnt[0] + cnt[1];
+}
+
+et_status upload_tile_classes(et_ctx *ctx, const Layout &L)
+{
+    const long long nt = L.npad / kPad;
+    std::vector<uint8_t> cls((size_t)nt);
+    for (int c = 0; c < L.ncls; ++c)
+        for (long long t = L.seg_pos[c] / kPad; t < L.seg_pos[c + 1] / kPad; ++t) cls[(size_t)t] = (uint8_t)c;
+    ET_TRY(ensure(ctx, ctx->tilecls, (size_t)nt));
+    CUDA_TRY(cudaMemcpyAsync(ctx->tilecls.p, cls.data(), (size_t)nt, cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // cls goes out of scope
+    return ET_OK;
+}
+
+// ---- call bracketing / stats -----------------------------------------------------------------------------
+et_status begin_call(et_ctx *ctx)
+{
+    ctx->stats = et_stats{};
+    ctx->acc_pairs_ms = ctx->acc_labels_ms = 0;
+    CUDA_TRY(cudaSetDevice(ctx->device));
+    CUDA_TRY(cudaEventRecord(ctx->ev[0], ctx->stream));
+    return ET_OK;
+}
+et_status end_call(et_ctx *ctx)
+{
+    CUDA_TRY(cudaEventRecord(ctx->ev[1], ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    float ms = 0;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+    ctx->stats.ms_total = ms;
+    ctx->stats.ms_pairs = ctx->acc_pairs_ms;
+    ctx->stats.ms_labels = ctx->acc_labels_ms;
+    return ET_OK;
+}
+// Bracket a group of launches with events; the elapsed time is read (after a sync) by span_end.
+et_status span_begin(et_ctx *ctx, int slot) { CUDA_TRY(cudaEventRecord(ctx->ev[slot], ctx->stream)); return ET_OK; }
+et_status span_end(et_ctx *ctx, int slot, double *acc)
+{
+    CUDA_TRY(cudaEventRecord(ctx->ev[slot + 1], ctx->stream));
+    CUDA_TRY(cudaEventSynchronize(ctx->ev[slot + 1]));
+    float ms = 0;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ctx->ev[slot], ctx->ev[slot + 1]));
+    *acc += ms;
+    return ET_OK;
+}
+
+#define LAUNCH_CHECK()                          \
+    do {                                        \
+        ctx->stats.launches += 1;               \
+        CUDA_TRY(cudaGetLastError());           \
+    } while (0)
+
+// ---- prep ------------------------------------------------------------------------------------------------
+template <typename TIn>
+et_status run_prep_t(et_ctx *ctx, const TIn *x, const TIn *xbar, const double *wx, const double *wxbar, const int *src,
+                     const Layout &L, int dim, double sigma)
+{
+    ET_TRY(ensure(ctx, ctx->mm, 16 * sizeof(uint32_t)));
+    ET_TRY(ensure(ctx, ctx->flag, sizeof(int)));
+    ET_TRY(ensure_pinned(ctx, 4096));
+    uint32_t *h = static_cast<uint32_t *>(ctx->pinned);
+    for (int k = 0; k < 8; ++k) { h[2 * k] = 0xffffffffu; h[2 * k + 1] = 0u; }
+    CUDA_TRY(cudaMemcpyAsync(ctx->mm.p, h, 16 * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(cudaMemsetAsync(ctx->flag.p, 0, sizeof(int), ctx->stream));
+    const int grid = ctx->num_sms * 4;
+    k_minmax<TIn><<<grid, 256, 0, ctx->stream>>>(x, L.n, dim, wx, static_cast<uint32_t *>(ctx->mm.p), static_cast<int *>(ctx->flag.p));
+    LAUNCH_CHECK();
+    k_minmax<TIn><<<grid, 256, 0, ctx->stream>>>(xbar, L.nbar, dim, wxbar, static_cast<uint32_t *>(ctx->mm.p), static_cast<int *>(ctx->flag.p));
+    LAUNCH_CHECK();
+    CUDA_TRY(cudaMemcpyAsync(h + 32, ctx->mm.p, 16 * sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(h + 64, ctx->flag.p, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    if (h[64] != 0) return fail(ctx, ET_ERR_NONFINITE, "NaN or Inf in coordinates or weights");
+
+    PrepParams P{};
+    for (int k = 0; k < dim; ++k) P.centre[k] = 0.5 * ((double)key2f(h[32 + 2 * k]) + (double)key2f(h[32 + 2 * k + 1]));
+    P.scale = std::sqrt(1.4426950408889634074 / (2.0 * sigma * sigma));
+    P.n = L.n; P.nbar = L.nbar; P.npad = L.npad; P.dim = dim; P.ncls = L.ncls;
+    for (int c = 0; c <= L.ncls; ++c) P.seg_pos[c] = L.seg_pos[c];
+    for (int c = 0; c < L.ncls; ++c) P.seg_count[c] = L.seg_count[c];
+    ET_TRY(ensure(ctx, ctx->rec, (size_t)L.npad * rec_floats(dim) * sizeof(float)));
+    k_prep<TIn><<<grid, 256, 0, ctx->stream>>>(x, xbar, wx, wxbar, src, P, static_cast<float *>(ctx->rec.p));
+    LAUNCH_CHECK();
+    return ET_OK;
+}
+
+et_status run_prep(et_ctx *ctx, const void *x, const void *xbar, const double *wx, const double *wxbar, const int *src,
+                   const Layout &L, int dim, et_dtype dtype, double sigma)
+{
+    if (dtype == ET_F32)
+        return run_prep_t<float>(ctx, static_cast<const float *>(x), static_cast<const float *>(xbar), wx, wxbar, src, L, dim, sigma);
+    return run_prep_t<double>(ctx, static_cast<const double *>(x), static_cast<const double *>(xbar), wx, wxbar, src, L, dim, sigma);
+}
+
+// ---- kernel dispatch over dim ----------------------------------------------------------------------------
+#define DISPATCH_DIM(dim, ...)                                                   \
+    switch (dim) {                                                               \
+        case 1: { constexpr int D = 1; __VA_ARGS__; } break;                            \
+        case 2: { constexpr int D = 2; __VA_ARGS__; } break;                            \
+        case 3: { constexpr int D = 3; __VA_ARGS__; } break;                            \
+        case 4: { constexpr int D = 4; __VA_ARGS__; } break;                            \
+        case 5: { constexpr int D = 5; __VA_ARGS__; } break;                            \
+        case 6: { constexpr int D = 6; __VA_ARGS__; } break;                            \
+        case 7: { constexpr int D = 7; __VA_ARGS__; } break;                            \
+        default: { constexpr int D = 8; __VA_ARGS__; } break;                           \
+    }
+
+template <typename K>
+int resident_blocks(et_ctx *ctx, K kernel)
+{
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+    return per_sm * ctx->num_sms;
+}
+
+constexpr int kRT = 4;    // rows per thread in K-T (i-tile = 1024 rows = kPad)
+constexpr int kRRow = 2;  // rows per thread in K-ROW (i-tile = 512 rows)
+
+// K-T: class-pair sums into ctx->sums (device, kSumSlots doubles).
+et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim)
+{
+    const int nT = (int)(L.npad / (kThreads * kRT));
+    const long long nunits = (long long)nT * (nT + 1) / 2;
+    ET_TRY(ensure(ctx, ctx->sums, kSumSlots * sizeof(double)));
+    ET_TRY(span_begin(ctx, 2));
+    DISPATCH_DIM(dim, {
+        int grid = resident_blocks(ctx, k_pairs_T<D, kRT>);
+        if ((long long)grid > nunits) grid = (int)nunits;
+        ET_TRY(ensure(ctx, ctx->partials, (size_t)grid * kSumSlots * sizeof(double)));
+        k_pairs_T<D, kRT><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), nT,
+                                                             static_cast<const uint8_t *>(ctx->tilecls.p), nunits,
+                                                             static_cast<double *>(ctx->partials.p));
+        LAUNCH_CHECK();
+        k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partials.p), grid, kSumSlots,
+                                                 static_cast<double *>(ctx->sums.p));
+        LAUNCH_CHECK();
+    });
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ctx->stats.pair_evals += nunits * (long long)(kThreads * kRT) * (kThreads * kRT);
+    return ET_OK;
+}
+
+// K-ROW: rowsum[c][row] for all rows.
+template <int C>
+et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
+{
+    const int nT = (int)(L.npad / (kThreads * kRRow));
+    RowSegs segs{};
+    for (int c = 0; c <= C; ++c) segs.jt_begin[c] = (int)(L.seg_pos[c] / kTileJ);
+    ET_TRY(ensure(ctx, ctx->rowsum, (size_t)C * L.npad * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->counter, sizeof(int)));
+    CUDA_TRY(cudaMemsetAsync(ctx->counter.p, 0, sizeof(int), ctx->stream));
+    ET_TRY(span_begin(ctx, 2));
+    DISPATCH_DIM(dim, {
+        int grid = resident_blocks(ctx, k_pairs_rows<D, kRRow, C>);
+        if (grid > nT) grid = nT;
+        k_pairs_rows<D, kRRow, C><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), nT, L.npad,
+                                                                    static_cast<const uint8_t *>(ctx->tilecls.p), segs,
+                                                                    static_cast<int *>(ctx->counter.p),
+                                                                    static_cast<double *>(ctx->rowsum.p));
+        LAUNCH_CHECK();
+    });
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ctx->stats.pair_evals += L.npad * L.npad;
+    return ET_OK;
+}
+et_status run_pairs_rows(et_ctx *ctx, const Layout &L, int dim)
+{
+    return L.ncls == 2 ? run_pairs_rows_c<2>(ctx, L, dim) : run_pairs_rows_c<4>(ctx, L, dim);
+}
+
+// ---- labels ----------------------------------------------------------------------------------------------
+// Radix select of K*_p for every permutation into ctx->sel.
+et_status run_label_select(et_ctx *ctx, long long N, long long n_x, int nperm, uint64_t seed)
+{
+    ET_TRY(ensure(ctx, ctx->sel, (size_t)nperm * sizeof(SelState)));
+    ET_TRY(ensure(ctx, ctx->hist, (size_t)nperm * 256 * sizeof(unsigned int)));
+    CUDA_TRY(cudaMemsetAsync(ctx->hist.p, 0, (size_t)nperm * 256 * sizeof(unsigned int), ctx->stream));
+    k_sel_init<<<(nperm + 255) / 256, 256, 0, ctx->stream>>>(static_cast<SelState *>(ctx->sel.p), nperm, n_x);
+    LAUNCH_CHECK();
+    const int ev = 8;
+    const dim3 grid((unsigned)((N + (long long)kThreads * ev - 1) / ((long long)kThreads * ev)), (unsigned)((nperm + 3) / 4));
+    for (int pass = 0; pass < 8; ++pass) {
+        k_sel_hist<<<grid, kThreads, 0, ctx->stream>>>(N, nperm, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), pass,
+                                                      static_cast<const SelState *>(ctx->sel.p),
+                                                      static_cast<unsigned int *>(ctx->hist.p), ev);
+        LAUNCH_CHECK();
+        k_sel_pick<<<(nperm + 7) / 8, 256, 0, ctx->stream>>>(static_cast<SelState *>(ctx->sel.p),
+                                                             static_cast<unsigned int *>(ctx->hist.p), nperm);
+        LAUNCH_CHECK();
+    }
+    return ET_OK;
+}
+
+// Internal masks: column 0 = observed labelling (pooled index < n_a), column p + 1 = permutation p;
+// word g of padded row r at mask[g * npad + r]; padding rows are zero.
+et_status run_labels_internal(et_ctx *ctx, const Layout &L, int nperm, uint64_t seed, int *nwords_out)
+{
+    const int nwords = (nperm + 1 + 31) / 32;
+    ET_TRY(span_begin(ctx, 4));
+    ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
+    ET_TRY(ensure(ctx, ctx->mask, (size_t)nwords * L.npad * sizeof(uint32_t)));
+    CUDA_TRY(cudaMemsetAsync(ctx->mask.p, 0, (size_t)nwords * L.npad * sizeof(uint32_t), ctx->stream));
+    LabelOut lo{};
+    lo.stride_g = L.npad;
+    lo.stride_i = 1;
+    lo.nseg = L.ncls;
+    for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
+    for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
+    const dim3 grid((unsigned)((L.N + kThreads - 1) / kThreads), (unsigned)nwords);
+    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, 1, nwords, (uint32_t)(seed & 0xffffffffu),
+                                                     (uint32_t)(seed >> 32), static_cast<const SelState *>(ctx->sel.p), lo,
+                                                     static_cast<uint32_t *>(ctx->mask.p));
+    LAUNCH_CHECK();
+    ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
+    *nwords_out = nwords;
+    return ET_OK;
+}
+
+// ---- statistic kernels (H6) -------------------------------------------------------------------------------
+struct DevT {
+    et_result r;
+    int status;  // 0 ok, ET_ERR_DEGENERATE
+};
+
+__device__ void form_result(double S_xx, double S_bb, double S_xb, double W, double Wbar, long long npairs, DevT *out)
+{
+    et_result r;
+    r.S_xx = S_xx; r.S_bb = S_bb; r.S_xb = S_xb; r.W = W; r.Wbar = Wbar; r.n_pairs = npairs;
+    if (!(W > 1.0) || !(Wbar > 1.0)) {
+        r.T = r.T_xx = r.T_bb = r.T_xb = nan("");
+        out->r = r;
+        out->status = ET_ERR_DEGENERATE;
+        return;
+    }
+    r.T_xx = S_xx / (W * (W - 1.0));
+    r.T_bb = S_bb / (Wbar * (Wbar - 1.0));
+    r.T_xb = S_xb / (W * Wbar);
+    r.T = r.T_xx + r.T_bb - r.T_xb;
+    out->r = r;
+    out->status = 0;
+}
+
+// Eq. 2 from class-pair sums S[c1*4+c2] (c1 <= c2) and class weights; sample A = classes with bit set in mask_a.
+// One thread.  Used for X vs Xbar (2 classes) and for the P-even / P-odd regroupings of the four classes.
+__global__ void k_stat_from_sums(const double *__restrict__ S, const double *__restrict__ clsw, int ncls, unsigned mask_a,
+                                 long long npairs, DevT *out)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    double sxx = 0, sbb = 0, sxb = 0, W = 0, Wb = 0;
+    for (int c1 = 0; c1 < ncls; ++c1) {
+        const bool a1 = mask_a >> c1 & 1u;
+        (a1 ? W : Wb) += clsw[c1];
+        for (int c2 = c1; c2 < ncls; ++c2) {
+            const bool a2 = mask_a >> c2 & 1u;
+            const double s = S[c1 * 4 + c2];
+            if (a1 && a2) sxx += s;
+            else if (!a1 && !a2) sbb += s;
+            else sxb += s;
+        }
+    }
+    form_result(sxx, sbb, sxb, W, Wb, npairs, out);
+}
+
+// class weights: clsw[c] = sum of w over the rows of class c (fixed order: tiles in order, then threads)
+__global__ void __launch_bounds__(kThreads) k_tile_weights(const float *__restrict__ rec, int F, int dim, double *__restrict__ out)
+{
+    __shared__ double s[kThreads / 32];
+    const long long base = (long long)blockIdx.x * kPad;
+    double a = 0.0;
+    for (int k = threadIdx.x; k < kPad; k += kThreads) a += (double)rec[(base + k) * F + dim];
+    a = warp_sum(a);
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < kThreads / 32; ++w) t += s[w];
+        out[blockIdx.x] = t;
+    }
+}
+// out[c] (or out[c1*4+c2] when ncol > 1) = sum over the tiles of class c of in[tile*ncol + k]
+__global__ void k_reduce_by_class(const double *__restrict__ in, const uint8_t *__restrict__ tile_cls, int ntiles, int ncol,
+                                  double *__restrict__ out)
+{
+    const int c = threadIdx.x / ncol, k = threadIdx.x % ncol;
+    if (c >= kMaxCls) return;
+    double s = 0.0;
+    for (int t = 0; t < ntiles; ++t)
+        if (tile_cls[t] == c) s += in[(long long)t * ncol + k];
+    if (ncol == 1) out[c] = s;
+    else out[c * 4 + k] = s;
+}
+// rowsum-derived class-pair matrix M[c1*4+c2] = sum_{i in c1} w_i rowsum[c2][i] -> unordered-pair sums
+// S[c1*4+c2] (c1 <= c2): diagonal halved, off-diagonal the mean of the two orientations.
+__global__ void k_sym_class_sums(const double *__restrict__ M, int ncls, double *__restrict__ S)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    for (int a = 0; a < 16; ++a) S[a] = 0.0;
+    for (int c1 = 0; c1 < ncls; ++c1)
+        for (int c2 = c1; c2 < ncls; ++c2)
+            S[c1 * 4 + c2] = c1 == c2 ? 0.5 * M[c1 * 4 + c1] : 0.5 * (M[c1 * 4 + c2] + M[c2 * 4 + c1]);
+}
+
+// Permutation statistic (H6): columns c = 0 (observed) and c = p + 1.  From Q_c, R_c, W_c, S = RW_all / 2, Wtot:
+//   S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q  (SURVEY 8(a) identity), Eq. 2 with W = W_c, Wbar = Wtot - W_c.
+// Then count = #{T_p > T_obs}, n_near = #{|T_p - T_obs| <= 1e-9 * term scale, or T_p NaN}.
+struct DevPerm {
+    et_perm_result r;
+    int status;
+};
+__global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q, const double *__restrict__ RW, int nwords, int nperm,
+                                                  long long npairs, double *__restrict__ T_perm, DevPerm *out)
+{
+    // RW layout: [g][which][kRWCols]
+    __shared__ DevT obs;
+    __shared__ unsigned long long s_cnt, s_near;
+    const double S = 0.5 * RW[0 * 2 * kRWCols + 0 * kRWCols + 32];
+    const double Wtot = RW[0 * 2 * kRWCols + 1 * kRWCols + 32];
+    if (threadIdx.x == 0) {
+        const double q = Q[0], r = RW[0], w = RW[kRWCols];
+        form_result(q, S - r + q, r - 2.0 * q, w, Wtot - w, npairs, &obs);
+        s_cnt = 0ull;
+        s_near = 0ull;
+    }
+    __syncthreads();
+    const double Tobs = obs.r.T;
+    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb));
+    unsigned long long cnt = 0, near = 0;
+    for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
+        const int c = p + 1, g = c >> 5, b = c & 31;
+        const double q = Q[g * 32 + b], r = RW[(g * 2 + 0) * kRWCols + b], w = RW[(g * 2 + 1) * kRWCols + b];
+        DevT t;
+        form_result(q, S - r + q, r - 2.0 * q, w, Wtot - w, npairs, &t);
+        T_perm[p] = t.r.T;
+        if (t.status != 0) { near += 1; continue; }
+        if (t.r.T > Tobs) cnt += 1;
+        if (fabs(t.r.T - Tobs) <= guard) near += 1;
+    }
+    atomicAdd(&s_cnt, cnt);
+    atomicAdd(&s_near, near);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        out->r.observed = obs.r;
+        out->r.count_gt = (long long)s_cnt;
+        out->r.n_near = (long long)s_near;
+        out->r.nperm = nperm;
+        out->r.p_value = (double)s_cnt / (double)nperm;
+        out->status = obs.status;
+    }
+    (void)nwords;
+}
+
+// class weights into ctx->clsw (kMaxCls doubles)
+et_status run_class_weights(et_ctx *ctx, const Layout &L, int dim)
+{
+    const int nt = (int)(L.npad / kPad);
+    ET_TRY(ensure(ctx, ctx->clssum, (size_t)nt * 4 * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->clsw, kMaxCls * sizeof(double)));
+    k_tile_weights<<<nt, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+                                                    static_cast<double *>(ctx->clssum.p));
+    LAUNCH_CHECK();
+    k_reduce_by_class<<<1, kMaxCls, 0, ctx->stream>>>(static_cast<const double *>(ctx->clssum.p),
+                                                     static_cast<const uint8_t *>(ctx->tilecls.p), nt, 1,
+                                                     static_cast<double *>(ctx->clsw.p));
+    LAUNCH_CHECK();
+    return ET_OK;
+}
+
+long long pairs_two(long long a, long long b) { return a * (a - 1) / 2 + b * (b - 1) / 2 + a * b; }
+
+// Fetch a DevT / DevPerm from the device.
+template <typename T>
+et_status fetch(et_ctx *ctx, const void *dev, T *host)
+{
+    ET_TRY(ensure_pinned(ctx, 4096));
+    CUDA_TRY(cudaMemcpyAsync(ctx->pinned, dev, sizeof(T), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    memcpy(host, ctx->pinned, sizeof(T));
+    return ET_OK;
+}
+
+// ---- the two-sample T from prepared records ---------------------------------------------------------------
+et_status do_T(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar, int64_t nbar,
+               int dim, et_dtype dtype, et_memspace mem, double sigma, et_result *out)
+{
+    ET_TRY(begin_call(ctx));
+    const void *dx, *dxb, *dwx, *dwb;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
+    ET_TRY(stage_in(ctx, wxbar, (size_t)nbar * 8, mem, ctx->in_wxbar, &dwb));
+    Layout L;
+    layout_two(L, n, nbar);
+    ET_TRY(upload_tile_classes(ctx, L));
+    ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigma));
+    ET_TRY(run_class_weights(ctx, L, dim));
+    ET_TRY(run_pairs_T(ctx, L, dim));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
+    k_stat_from_sums<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), static_cast<const double *>(ctx->clsw.p),
+                                                2, 0x1u, pairs_two(n, nbar), static_cast<DevT *>(ctx->result.p));
+    LAUNCH_CHECK();
+    DevT r;
+    ET_TRY(fetch(ctx, ctx->result.p, &r));
+    ET_TRY(end_call(ctx));
+    if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "weighted normalisation degenerate: W = %g, Wbar = %g (need > 1)", r.r.W, r.r.Wbar);
+    *out = r.r;
+    return ET_OK;
+}
+
+// ---- permutation sums from prepared records + masks -------------------------------------------------------
+et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
+{
+    // Q: CUDA-core kernel, one launch per mask word
+    const int nT = (int)(L.npad / (kThreads * 2));
+    const long long nunits = (long long)nT * (nT + 1) / 2;
+    ET_TRY(ensure(ctx, ctx->Q, (size_t)nwords * 32 * sizeof(double)));
+    ET_TRY(span_begin(ctx, 2));
+    DISPATCH_DIM(dim, {
+        int grid = resident_blocks(ctx, k_perm32<D>);
+        if ((long long)grid > nunits) grid = (int)nunits;
+        ET_TRY(ensure(ctx, ctx->partQ, (size_t)grid * 32 * sizeof(double)));
+        for (int g = 0; g < nwords; ++g) {
+            k_perm32<D><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p),
+                                                           static_cast<const uint32_t *>(ctx->mask.p) + (long long)g * L.npad, nT,
+                                                           nunits, static_cast<double *>(ctx->partQ.p));
+            LAUNCH_CHECK();
+            k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partQ.p), grid, 32,
+                                                     static_cast<double *>(ctx->Q.p) + g * 32);
+            LAUNCH_CHECK();
+        }
+    });
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ctx->stats.pair_evals += (long long)nwords * nunits * (kThreads * 2LL) * (kThreads * 2LL);
+
+    // R, W per column
+    const int nchunk = 64;
+    ET_TRY(ensure(ctx, ctx->partRW, (size_t)nwords * nchunk * 2 * kRWCols * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->RW, (size_t)nwords * 2 * kRWCols * sizeof(double)));
+    const dim3 grid_rw((unsigned)nchunk, (unsigned)nwords);
+    if (L.ncls == 2)
+        k_perm_RW<2><<<grid_rw, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+                                                           static_cast<const uint32_t *>(ctx->mask.p),
+                                                           static_cast<const double *>(ctx->rowsum.p), L.npad, nchunk,
+                                                           static_cast<double *>(ctx->partRW.p));
+    else
+        k_perm_RW<4><<<grid_rw, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+                                                           static_cast<const uint32_t *>(ctx->mask.p),
+                                                           static_cast<const double *>(ctx->rowsum.p), L.npad, nchunk,
+                                                           static_cast<double *>(ctx->partRW.p));
+    LAUNCH_CHECK();
+    // partRW[g][chunk][2*kRWCols] -> RW[g][2*kRWCols]: per word a column reduction over the chunks
+    for (int g = 0; g < nwords; ++g) {
+        k_reduce_cols<<<1, 96, 0, ctx->stream>>>(static_cast<const double *>(ctx->partRW.p) + (long long)g * nchunk * 2 * kRWCols,
+                                                 nchunk, 2 * kRWCols, static_cast<double *>(ctx->RW.p) + (long long)g * 2 * kRWCols);
+        LAUNCH_CHECK();
+    }
+    return ET_OK;
+}
+
+et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, double *T_perm, et_perm_result *out)
+{
+    ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
+    k_perm_stat<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->Q.p), static_cast<const double *>(ctx->RW.p), nwords,
+                                            (int)nperm, npairs, static_cast<double *>(ctx->tperm.p),
+                                            static_cast<DevPerm *>(ctx->result.p));
+    LAUNCH_CHECK();
+    DevPerm r;
+    ET_TRY(fetch(ctx, ctx->result.p, &r));
+    if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "weighted normalisation degenerate: W = %g, Wbar = %g (need > 1)", r.r.observed.W, r.r.observed.Wbar);
+    CUDA_TRY(cudaMemcpyAsync(T_perm, ctx->tperm.p, (size_t)nperm * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    *out = r.r;
+    return ET_OK;
+}
+
+}  // namespace
+
+// =============================================================================================== C ABI
+extern "C" {
+
+const char *et_version(void) { return "libet 0.1 (sm_100a)"; }
+
+et_status et_create(et_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return ET_ERR_INVALID;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || device < 0 || device >= ndev) return ET_ERR_CUDA;
+    et_ctx *ctx = new (std::nothrow) et_ctx();
+    if (!ctx) return ET_ERR_NOMEM;
+    ctx->device = device;
+    bool ok = cudaSetDevice(device) == cudaSuccess;
+    cudaDeviceProp prop;
+    ok = ok && cudaGetDeviceProperties(&prop, device) == cudaSuccess;
+    if (ok) ctx->num_sms = prop.multiProcessorCount;
+    if (ok) {
+        if (cuda_stream) { ctx->stream = static_cast<cudaStream_t>(cuda_stream); ctx->own_stream = false; }
+        else { ok = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking) == cudaSuccess; ctx->own_stream = ok; }
+    }
+    for (int i = 0; ok && i < 8; ++i) ok = cudaEventCreate(&ctx->ev[i]) == cudaSuccess;
+    if (!ok) { et_destroy(ctx); return ET_ERR_CUDA; }
+    *out = ctx;
+    return ET_OK;
+}
+
+void et_destroy(et_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    if (ctx->stream) cudaStreamSynchronize(ctx->stream);
+    Buf *bufs[] = {&ctx->in_x, &ctx->in_xbar, &ctx->in_wx, &ctx->in_wxbar, &ctx->in_mx, &ctx->in_mb, &ctx->in_aux, &ctx->rec,
+                   &ctx->tilecls, &ctx->partials, &ctx->sums, &ctx->rowsum, &ctx->mask, &ctx->sel, &ctx->hist, &ctx->partQ,
+                   &ctx->Q, &ctx->partRW, &ctx->RW, &ctx->mm, &ctx->flag, &ctx->counter, &ctx->src, &ctx->posx, &ctx->posb,
+                   &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
+                   &ctx->count64};
+    for (Buf *b : bufs)
+        if (b->p) cudaFree(b->p);
+    if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    for (int i = 0; i < 8; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->own_stream && ctx->stream) cudaStreamDestroy(ctx->stream);
+    delete ctx;
+}
+
+const char *et_last_error(const et_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (opt == ET_OPT_PERM_KERNEL) {
+        if (value != 0) return fail(ctx, ET_ERR_INVALID, "unknown permutation kernel %lld", (long long)value);
+        ctx->opt_perm_kernel = value;
+        return ET_OK;
+    }
+    return fail(ctx, ET_ERR_INVALID, "unknown option %d", (int)opt);
+}
+
+et_status et_get_stats(const et_ctx *ctx, et_stats *out)
+{
+    if (!ctx || !out) return ET_ERR_INVALID;
+    *out = ctx->stats;
+    return ET_OK;
+}
+
+et_status et_T(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, int dim, et_dtype dtype, et_memspace mem,
+               double sigma, et_result *out)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!out) return fail(ctx, ET_ERR_INVALID, "null output");
+    return do_T(ctx, x, nullptr, n, xbar, nullptr, nbar, dim, dtype, mem, sigma, out);
+}
+
+et_status et_T_weighted(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar,
+                        int64_t nbar, int dim, et_dtype dtype, et_memspace mem, double sigma, et_result *out)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!out || !wx || !wxbar) return fail(ctx, ET_ERR_INVALID, "null weights or output");
+    return do_T(ctx, x, wx, n, xbar, wxbar, nbar, dim, dtype, mem, sigma, out);
+}
+
+et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar,
+                              int64_t nbar, int dim, et_dtype dtype, et_memspace mem, double sigma, int64_t nperm, uint64_t seed,
+                              double *T_perm, et_perm_result *out)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!out || !T_perm) return fail(ctx, ET_ERR_INVALID, "null output");
+    if ((wx == nullptr) != (wxbar == nullptr)) return fail(ctx, ET_ERR_INVALID, "give both weight arrays or neither");
+    if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
+    ET_TRY(begin_call(ctx));
+    const void *dx, *dxb, *dwx, *dwb;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
+    ET_TRY(stage_in(ctx, wxbar, (size_t)nbar * 8, mem, ctx->in_wxbar, &dwb));
+    Layout L;
+    layout_two(L, n, nbar);
+    ET_TRY(upload_tile_classes(ctx, L));
+    ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigma));
+    int nwords = 0;
+    ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
+    ET_TRY(run_pairs_rows(ctx, L, dim));
+    ET_TRY(run_perm_sums(ctx, L, dim, nwords));
+    et_perm_result r;
+    ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), T_perm, &r));
+    ET_TRY(end_call(ctx));
+    *out = r;
+    return ET_OK;
+}
+
+et_status et_podd_split(et_ctx *ctx, const double *pB, const double *pC, const double *pD, int64_t n, int is_conjugate,
+                        et_memspace mem, uint8_t *positive, int64_t *n_positive)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!pB || !pC || !pD || !positive || n < 1) return fail(ctx, ET_ERR_INVALID, "null pointer or n < 1");
+    ET_TRY(begin_call(ctx));
+    const void *dB, *dC, *dD;
+    ET_TRY(stage_in(ctx, pB, (size_t)n * 24, mem, ctx->in_mx, &dB));
+    ET_TRY(stage_in(ctx, pC, (size_t)n * 24, mem, ctx->in_mb, &dC));
+    ET_TRY(stage_in(ctx, pD, (size_t)n * 24, mem, ctx->in_aux, &dD));
+    uint8_t *dpos = positive;
+    if (mem == ET_HOST) { ET_TRY(ensure(ctx, ctx->posx, (size_t)n)); dpos = static_cast<uint8_t *>(ctx->posx.p); }
+    ET_TRY(ensure(ctx, ctx->count64, 8));
+    CUDA_TRY(cudaMemsetAsync(ctx->count64.p, 0, 8, ctx->stream));
+    k_podd_flags<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(static_cast<const double *>(dB), static_cast<const double *>(dC),
+                                                                    static_cast<const double *>(dD), n, 3, is_conjugate, dpos,
+                                                                    static_cast<unsigned long long *>(ctx->count64.p));
+    LAUNCH_CHECK();
+    if (mem == ET_HOST) CUDA_TRY(cudaMemcpyAsync(positive, dpos, (size_t)n, cudaMemcpyDeviceToHost, ctx->stream));
+    unsigned long long cnt = 0;
+    ET_TRY(fetch(ctx, ctx->count64.p, &cnt));
+    ET_TRY(end_call(ctx));
+    if (n_positive) *n_positive = (int64_t)cnt;
+    return ET_OK;
+}
+
+et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t n, const void *xbar, const double *mom_xbar,
+                       int64_t nbar, int dim, et_dtype dtype, et_memspace mem, double sigma, int64_t nperm, uint64_t seed,
+                       double *T_perm, et_podd_result *out)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!out || !T_perm || !mom_x || !mom_xbar) return fail(ctx, ET_ERR_INVALID, "null pointer");
+    if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
+    ET_TRY(begin_call(ctx));
+    const void *dx, *dxb, *dmx, *dmb;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, mom_x, (size_t)n * 72, mem, ctx->in_mx, &dmx));
+    ET_TRY(stage_in(ctx, mom_xbar, (size_t)nbar * 72, mem, ctx->in_mb, &dmb));
+    const long long N = n + nbar;
+
+    // H0: the split (Eq. 4) and the stable partition into the layout classes (I, IV | II, III)
+    ET_TRY(ensure(ctx, ctx->posx, (size_t)n));
+    ET_TRY(ensure(ctx, ctx->posb, (size_t)nbar));
+    ET_TRY(ensure(ctx, ctx->count64, 16));
+    CUDA_TRY(cudaMemsetAsync(ctx->count64.p, 0, 16, ctx->stream));
+    const double *mx = static_cast<const double *>(dmx), *mb = static_cast<const double *>(dmb);
+    k_podd_flags<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(mx, mx + 3, mx + 6, n, 9, 0, static_cast<uint8_t *>(ctx->posx.p),
+                                                                    static_cast<unsigned long long *>(ctx->count64.p));
+    LAUNCH_CHECK();
+    k_podd_flags<<<(unsigned)((nbar + 255) / 256), 256, 0, ctx->stream>>>(mb, mb + 3, mb + 6, nbar, 9, 1, static_cast<uint8_t *>(ctx->posb.p),
+                                                                       static_cast<unsigned long long *>(ctx->count64.p) + 1);
+    LAUNCH_CHECK();
+    unsigned long long pos_cnt[2];
+    ET_TRY(fetch(ctx, ctx->count64.p, &pos_cnt));
+    const long long nI = (long long)pos_cnt[0], nII = n - nI, nIII = (long long)pos_cnt[1], nIV = nbar - nIII;
+    const long long cnt[4] = {nI, nIV, nII, nIII};  // layout order
+    if (nI + nIV < 2 || nII + nIII < 2) return fail(ctx, ET_ERR_INVALID, "P-odd samples need >= 2 events each (I+IV = %lld, II+III = %lld)", nI + nIV, nII + nIII);
+    Layout L;
+    layout_four(L, n, nbar, cnt);
+    ET_TRY(upload_tile_classes(ctx, L));
+    const int nblk = (int)((N + kPartBlock - 1) / kPartBlock);
+    ET_TRY(ensure(ctx, ctx->blkcnt, (size_t)nblk * 4 * sizeof(int)));
+    ET_TRY(ensure(ctx, ctx->totals, 16 * sizeof(long long)));
+    ET_TRY(ensure(ctx, ctx->src, (size_t)L.npad * sizeof(int)));
+    k_fill_int<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<int *>(ctx->src.p), L.npad, -1);
+    LAUNCH_CHECK();
+    k_part_count<<<nblk, kPartBlock, 0, ctx->stream>>>(N, n, static_cast<const uint8_t *>(ctx->posx.p), static_cast<const uint8_t *>(ctx->posb.p),
+                                                      static_cast<int *>(ctx->blkcnt.p));
+    LAUNCH_CHECK();
+    k_part_scan<<<1, 32, 0, ctx->stream>>>(nblk, static_cast<int *>(ctx->blkcnt.p), static_cast<long long *>(ctx->totals.p));
+    LAUNCH_CHECK();
+    CUDA_TRY(cudaMemcpyAsync(static_cast<long long *>(ctx->totals.p) + 8, L.seg_pos, 4 * sizeof(long long), cudaMemcpyHostToDevice, ctx->stream));
+    k_part_scatter<<<nblk, kPartBlock, 0, ctx->stream>>>(N, n, static_cast<const uint8_t *>(ctx->posx.p), static_cast<const uint8_t *>(ctx->posb.p),
+                                                        static_cast<const int *>(ctx->blkcnt.p), static_cast<const long long *>(ctx->totals.p) + 8,
+                                                        static_cast<int *>(ctx->src.p));
+    LAUNCH_CHECK();
+
+    ET_TRY(run_prep(ctx, dx, dxb, nullptr, nullptr, static_cast<const int *>(ctx->src.p), L, dim, dtype, sigma));
+    ET_TRY(run_class_weights(ctx, L, dim));
+    int nwords = 0;
+    ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
+    ET_TRY(run_pairs_rows(ctx, L, dim));
+
+    // P-even T of (I+II) vs (III+IV) from the class-pair sums of the same pass: layout classes {0 (I), 2 (II)} = X
+    const int nt = (int)(L.npad / kPad);
+    ET_TRY(ensure(ctx, ctx->clssum, (size_t)nt * 4 * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->sums, 2 * kSumSlots * sizeof(double)));
+    k_class_sums<4><<<nt, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+                                                     static_cast<const double *>(ctx->rowsum.p), L.npad, static_cast<double *>(ctx->clssum.p));
+    LAUNCH_CHECK();
+    double *M = static_cast<double *>(ctx->sums.p) + kSumSlots;
+    CUDA_TRY(cudaMemsetAsync(M, 0, kSumSlots * sizeof(double), ctx->stream));
+    k_reduce_by_class<<<1, 16, 0, ctx->stream>>>(static_cast<const double *>(ctx->clssum.p), static_cast<const uint8_t *>(ctx->tilecls.p), nt, 4, M);
+    LAUNCH_CHECK();
+    k_sym_class_sums<<<1, 32, 0, ctx->stream>>>(M, 4, static_cast<double *>(ctx->sums.p));
+    LAUNCH_CHECK();
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
+    DevT *dev_even = reinterpret_cast<DevT *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm));
+    k_stat_from_sums<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), static_cast<const double *>(ctx->clsw.p), 4,
+                                                0x5u, pairs_two(n, nbar), dev_even);
+    LAUNCH_CHECK();
+
+    ET_TRY(run_perm_sums(ctx, L, dim, nwords));
+    et_perm_result pr;
+    ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(nI + nIV, nII + nIII), T_perm, &pr));
+    DevT even;
+    ET_TRY(fetch(ctx, dev_even, &even));
+    ET_TRY(end_call(ctx));
+    out->count[0] = nI; out->count[1] = nII; out->count[2] = nIII; out->count[3] = nIV;
+    out->p_even = even.r;
+    out->p_odd = pr;
+    return ET_OK;
+}
+
+et_status et_perm_labels(et_ctx *ctx, int64_t N, int64_t n, int64_t nperm, uint64_t seed, et_memspace mem, uint32_t *mask)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!mask || N < 1 || n < 1 || n > N || N >= (1ll << 31)) return fail(ctx, ET_ERR_INVALID, "bad label arguments");
+    if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
+    ET_TRY(begin_call(ctx));
+    ET_TRY(span_begin(ctx, 4));
+    ET_TRY(run_label_select(ctx, N, n, (int)nperm, seed));
+    const int nwords = (int)((nperm + 31) / 32);
+    uint32_t *dmask = mask;
+    const size_t bytes = (size_t)N * nwords * sizeof(uint32_t);
+    if (mem == ET_HOST) { ET_TRY(ensure(ctx, ctx->mask, bytes)); dmask = static_cast<uint32_t *>(ctx->mask.p); }
+    LabelOut lo{};
+    lo.stride_g = 1;
+    lo.stride_i = nwords;
+    lo.nseg = 0;
+    const dim3 grid((unsigned)((N + kThreads - 1) / kThreads), (unsigned)nwords);
+    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(N, n, (int)nperm, 0, nwords, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+                                                     static_cast<const SelState *>(ctx->sel.p), lo, dmask);
+    LAUNCH_CHECK();
+    ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
+    if (mem == ET_HOST) CUDA_TRY(cudaMemcpyAsync(mask, dmask, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    ET_TRY(end_call(ctx));
+    return ET_OK;
+}
+
+et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar, int64_t nbar,
+                      int dim, et_dtype dtype, et_memspace mem, double sigma, const int64_t *rows, int64_t nrows, double *r_x,
+                      double *r_xbar)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!rows || !r_x || !r_xbar || nrows < 1) return fail(ctx, ET_ERR_INVALID, "null pointer or nrows < 1");
+    if ((wx == nullptr) != (wxbar == nullptr)) return fail(ctx, ET_ERR_INVALID, "give both weight arrays or neither");
+    for (int64_t k = 0; k < nrows; ++k)
+        if (rows[k] < 0 || rows[k] >= n + nbar) return fail(ctx, ET_ERR_INVALID, "row index out of range");
+    ET_TRY(begin_call(ctx));
+    const void *dx, *dxb, *dwx, *dwb;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
+    ET_TRY(stage_in(ctx, wxbar, (size_t)nbar * 8, mem, ctx->in_wxbar, &dwb));
+    Layout L;
+    layout_two(L, n, nbar);
+    ET_TRY(upload_tile_classes(ctx, L));
+    ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigma));
+    ET_TRY(run_pairs_rows(ctx, L, dim));
+    std::vector<long long> pos((size_t)nrows);
+    for (int64_t k = 0; k < nrows; ++k) pos[(size_t)k] = rows[k] < n ? rows[k] : L.seg_pos[1] + (rows[k] - n);
+    ET_TRY(ensure(ctx, ctx->rows, (size_t)nrows * 8));
+    ET_TRY(ensure(ctx, ctx->rowsout, (size_t)nrows * 16));
+    CUDA_TRY(cudaMemcpyAsync(ctx->rows.p, pos.data(), (size_t)nrows * 8, cudaMemcpyHostToDevice, ctx->stream));
+    k_gather_rows<<<(unsigned)((nrows + 255) / 256), 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->rowsum.p), L.npad,
+                                                                         static_cast<const long long *>(ctx->rows.p), nrows, 2,
+                                                                         static_cast<double *>(ctx->rowsout.p));
+    LAUNCH_CHECK();
+    CUDA_TRY(cudaMemcpyAsync(r_x, ctx->rowsout.p, (size_t)nrows * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(r_xbar, static_cast<double *>(ctx->rowsout.p) + nrows, (size_t)nrows * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    ET_TRY(end_call(ctx));
+    return ET_OK;
+}
+
+}  // extern "C"

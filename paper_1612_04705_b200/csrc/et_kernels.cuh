@@ -1,0 +1,690 @@
+// et_kernels.cuh -- the CUDA kernels of libet.so (sm_100a).
+//
+// Pooled layout ("records"): events are grouped by class (2 classes X / Xbar, or the 4 classes of the Sect. 5
+// split), every class segment padded to a multiple of et::kPad rows.  Row r is rec_floats(dim) floats:
+// u[0..dim) = (x - centre) * sqrt(log2(e) / (2 sigma^2)) rounded to fp32, then the weight w (1 when unweighted,
+// 0 on padding rows), then zeros.  psi_ij = 2^(-|u_i - u_j|^2), padding contributes w = 0.
+#pragma once
+#include "et_device.cuh"
+
+namespace et {
+
+// ------------------------------------------------------------------------------------------------ prep
+// Bounding box of the coordinates (for the centre) and the non-finite check.  mm[2*k] = min, mm[2*k+1] = max as
+// order-preserving uint32 keys of the fp32-rounded values; flag[0] != 0 when a NaN/Inf was seen.
+__device__ __forceinline__ uint32_t f2key(float f)
+{
+    uint32_t b = __float_as_uint(f);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__host__ __device__ inline float key2f(uint32_t k)
+{
+    uint32_t b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k;
+#ifdef __CUDA_ARCH__
+    return __uint_as_float(b);
+#else
+    float f;
+    memcpy(&f, &b, 4);
+    return f;
+#endif
+}
+
+template <typename TIn>
+__global__ void k_minmax(const TIn *__restrict__ x, long long n, int dim, const double *__restrict__ w,
+                         uint32_t *__restrict__ mm, int *__restrict__ flag)
+{
+    uint32_t lo[8], hi[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { lo[k] = 0xffffffffu; hi[k] = 0u; }
+    bool bad = false;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if (k < dim) {
+                const double v = (double)x[i * dim + k];
+                if (!isfinite(v)) bad = true;
+                const uint32_t key = f2key((float)v);
+                lo[k] = min(lo[k], key);
+                hi[k] = max(hi[k], key);
+            }
+        if (w && !isfinite(w[i])) bad = true;
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+        if (k < dim) {
+            uint32_t a = lo[k], b = hi[k];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                a = min(a, __shfl_xor_sync(0xffffffffu, a, o));
+                b = max(b, __shfl_xor_sync(0xffffffffu, b, o));
+            }
+            if ((threadIdx.x & 31) == 0) {
+                atomicMin(&mm[2 * k], a);
+                atomicMax(&mm[2 * k + 1], b);
+            }
+        }
+    if (bad) atomicOr(flag, 1);
+}
+
+struct PrepParams {
+    double centre[8];
+    double scale;        // sqrt(log2(e) / (2 sigma^2))
+    long long n, nbar;   // sizes of the two source arrays
+    long long npad;      // rows of the pooled layout
+    int dim;
+    int ncls;
+    long long seg_pos[kMaxCls + 1];    // first padded row of each class segment (seg_pos[ncls] = npad)
+    long long seg_count[kMaxCls];      // real rows in each class segment
+};
+
+// Writes the pooled records.  src == nullptr: two classes, class 0 = x in input order, class 1 = xbar.
+// src != nullptr: src[row] is the pooled source index (0..n-1 -> x, n.. -> xbar) of a real row, -1 on padding.
+template <typename TIn>
+__global__ void k_prep(const TIn *__restrict__ x, const TIn *__restrict__ xbar, const double *__restrict__ wx,
+                       const double *__restrict__ wxbar, const int *__restrict__ src, PrepParams P,
+                       float *__restrict__ rec)
+{
+    const int F = rec_floats(P.dim);
+    for (long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x; row < P.npad;
+         row += (long long)gridDim.x * blockDim.x) {
+        long long s = -1;
+        if (src) {
+            s = src[row];
+        } else {
+            if (row < P.seg_pos[1]) { if (row < P.n) s = row; }
+            else if (row - P.seg_pos[1] < P.nbar) s = P.n + (row - P.seg_pos[1]);
+        }
+        float *o = rec + row * F;
+        if (s < 0) {
+            for (int k = 0; k < F; ++k) o[k] = 0.0f;
+            continue;
+        }
+        const TIn *p = s < P.n ? x + s * P.dim : xbar + (s - P.n) * P.dim;
+        for (int k = 0; k < P.dim; ++k) o[k] = (float)(((double)p[k] - P.centre[k]) * P.scale);
+        double w = 1.0;
+        if (wx) w = s < P.n ? wx[s] : wxbar[s - P.n];
+        o[P.dim] = (float)w;
+        for (int k = P.dim + 1; k < F; ++k) o[k] = 0.0f;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ all pairs
+// One j record from shared memory: coordinates and weight.
+template <int D>
+struct JRec {
+    float u[D];
+    float w;
+};
+template <int D>
+__device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int j)
+{
+    constexpr int F4 = rec_floats(D) / 4;
+    float v[F4 * 4];
+#pragma unroll
+    for (int q = 0; q < F4; ++q) {
+        const float4 t = sj[j * F4 + q];
+        v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+    }
+    JRec<D> r;
+#pragma unroll
+    for (int k = 0; k < D; ++k) r.u[k] = v[k];
+    r.w = v[D];
+    return r;
+}
+
+// K-T: class-pair block sums S[c1][c2] = sum over unordered pairs of w_i w_j psi_ij (Eq. 2's three sums, or the ten
+// of the four-class split), over the upper triangle of i-tiles.  Work unit = (I, J), I <= J, tiles of 256*R rows;
+// fp32 per pair and per 256-j partial row sum, fp64 from there on; per-unit block reduction in a fixed order, so the
+// result depends only on the grid size.
+template <int D, int R>
+__global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ rec, int nT,
+                                                     const uint8_t *__restrict__ tile_cls, long long nunits,
+                                                     double *__restrict__ partials)
+{
+    constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
+    __shared__ float4 sj[kTileJ * F4];
+    __shared__ double s_sum[kSumSlots];
+    __shared__ double s_warp[kThreads / 32];
+    const int tid = threadIdx.x;
+    if (tid < kSumSlots) s_sum[tid] = 0.0;
+
+    for (long long unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+        int I, J;
+        unit_to_pair(unit, nT, I, J);
+        float ui[R][D], wi[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
+            float v[F];
+#pragma unroll
+            for (int q = 0; q < F4; ++q) {
+                const float4 t = __ldg(p + q);
+                v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+            }
+#pragma unroll
+            for (int k = 0; k < D; ++k) ui[r][k] = v[k];
+            wi[r] = v[D];
+        }
+        double racc[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) racc[r] = 0.0;
+
+        for (int sub = 0; sub < TI / kTileJ; ++sub) {
+            __syncthreads();
+            {
+                const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)J * TI + sub * kTileJ + tid) * F);
+#pragma unroll
+                for (int q = 0; q < F4; ++q) sj[tid * F4 + q] = __ldg(p + q);
+            }
+            __syncthreads();
+            float acc[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+#pragma unroll 4
+            for (int j = 0; j < kTileJ; ++j) {
+                const JRec<D> rj = load_jrec<D>(sj, j);
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[r] = __fmaf_rn(psi_pair<D>(ui[r], rj.u), rj.w, acc[r]);
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) racc[r] += (double)acc[r];
+        }
+        double t = 0.0;
+        const bool diag = I == J;
+#pragma unroll
+        for (int r = 0; r < R; ++r) t += (double)wi[r] * (diag ? racc[r] - (double)wi[r] : racc[r]);
+        if (diag) t *= 0.5;
+        t = warp_sum(t);
+        if ((tid & 31) == 0) s_warp[tid >> 5] = t;
+        __syncthreads();
+        if (tid == 0) {
+            double s = 0.0;
+#pragma unroll
+            for (int w = 0; w < kThreads / 32; ++w) s += s_warp[w];
+            s_sum[tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad]] += s;
+        }
+    }
+    __syncthreads();
+    if (tid < kSumSlots) partials[(long long)blockIdx.x * kSumSlots + tid] = s_sum[tid];
+}
+
+// K-ROW: full row sums by class of j, rowsum[c][i] = sum_{j in class c, j != i} w_j psi_ij, for every pooled row.
+// Work unit = one i-tile of 256*R rows against all j; units handed out by an atomic counter (each row is summed by
+// one CTA in a fixed j order, so the result does not depend on the schedule).
+struct RowSegs {
+    int jt_begin[kMaxCls + 1];  // j sub-tile (kTileJ rows) range of each class segment
+};
+template <int D, int R, int C>
+__global__ void __launch_bounds__(kThreads) k_pairs_rows(const float *__restrict__ rec, int nT, long long npad,
+                                                        const uint8_t *__restrict__ tile_cls, RowSegs segs,
+                                                        int *__restrict__ counter, double *__restrict__ rowsum)
+{
+    constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
+    __shared__ float4 sj[kTileJ * F4];
+    __shared__ int s_unit;
+    const int tid = threadIdx.x;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_unit = atomicAdd(counter, 1);
+        __syncthreads();
+        const int I = s_unit;
+        if (I >= nT) break;
+        float ui[R][D], wi[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
+            float v[F];
+#pragma unroll
+            for (int q = 0; q < F4; ++q) {
+                const float4 t = __ldg(p + q);
+                v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+            }
+#pragma unroll
+            for (int k = 0; k < D; ++k) ui[r][k] = v[k];
+            wi[r] = v[D];
+        }
+        const int ci = tile_cls[(long long)I * TI / kPad];
+        double racc[R][C];
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) racc[r][c] = 0.0;
+            for (int jt = segs.jt_begin[c]; jt < segs.jt_begin[c + 1]; ++jt) {
+                __syncthreads();
+                {
+                    const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)jt * kTileJ + tid) * F);
+#pragma unroll
+                    for (int q = 0; q < F4; ++q) sj[tid * F4 + q] = __ldg(p + q);
+                }
+                __syncthreads();
+                float acc[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+#pragma unroll 4
+                for (int j = 0; j < kTileJ; ++j) {
+                    const JRec<D> rj = load_jrec<D>(sj, j);
+#pragma unroll
+                    for (int r = 0; r < R; ++r) acc[r] = __fmaf_rn(psi_pair<D>(ui[r], rj.u), rj.w, acc[r]);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) racc[r][c] += (double)acc[r];
+            }
+            // the row's own term w_i * psi_ii = w_i sits in its own class
+            if (c == ci) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) racc[r][c] -= (double)wi[r];
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) rowsum[(long long)c * npad + (long long)I * TI + r * kThreads + tid] = racc[r][c];
+        }
+    }
+}
+
+// K-PERM (CUDA cores): Q_c = sum_{i<j} a_ic a_jc w_i w_j psi_ij for the 32 label columns of one mask word, each psi
+// evaluated once and fanned out to 32 fp32 accumulators per row (y_ic = sum_j w_j a_jc psi_ij), over the upper
+// triangle of 512-row tiles.  fp32 over 256 j, then fp64 per thread across all its units; one block reduction at
+// the end.  Columns: c = 0 is the observed labelling, c = p + 1 permutation p.
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1) k_perm32(const float *__restrict__ rec, const uint32_t *__restrict__ maskg,
+                                                       int nT, long long nunits, double *__restrict__ partialQ)
+{
+    constexpr int R = 2, F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
+    __shared__ float4 sj[kTileJ * F4];
+    __shared__ float4 lab[kTileJ * 8];  // lab[j][c] = a_jc * w_j
+    const int tid = threadIdx.x;
+    double q[32];
+#pragma unroll
+    for (int c = 0; c < 32; ++c) q[c] = 0.0;
+
+    for (long long unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+        int I, J;
+        unit_to_pair(unit, nT, I, J);
+        float ui[R][D], wi[R];
+        uint32_t mi[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long row = (long long)I * TI + r * kThreads + tid;
+            const float4 *p = reinterpret_cast<const float4 *>(rec + row * F);
+            float v[F];
+#pragma unroll
+            for (int qq = 0; qq < F4; ++qq) {
+                const float4 t = __ldg(p + qq);
+                v[4 * qq] = t.x; v[4 * qq + 1] = t.y; v[4 * qq + 2] = t.z; v[4 * qq + 3] = t.w;
+            }
+#pragma unroll
+            for (int k = 0; k < D; ++k) ui[r][k] = v[k];
+            wi[r] = v[D];
+            mi[r] = __ldg(maskg + row);
+        }
+        const bool diag = I == J;
+        const double f = diag ? 0.5 : 1.0;
+        for (int sub = 0; sub < TI / kTileJ; ++sub) {
+            __syncthreads();
+            {
+                const long long row = (long long)J * TI + sub * kTileJ + tid;
+                const float4 *p = reinterpret_cast<const float4 *>(rec + row * F);
+                float wj = 0.f;
+#pragma unroll
+                for (int qq = 0; qq < F4; ++qq) {
+                    const float4 t = __ldg(p + qq);
+                    sj[tid * F4 + qq] = t;
+                    if (qq == D / 4) wj = (D % 4 == 0) ? t.x : (D % 4 == 1) ? t.y : (D % 4 == 2) ? t.z : t.w;
+                }
+                const uint32_t m = __ldg(maskg + row);
+#pragma unroll
+                for (int c4 = 0; c4 < 8; ++c4) {
+                    float4 l;
+                    l.x = (m >> (4 * c4) & 1u) ? wj : 0.f;
+                    l.y = (m >> (4 * c4 + 1) & 1u) ? wj : 0.f;
+                    l.z = (m >> (4 * c4 + 2) & 1u) ? wj : 0.f;
+                    l.w = (m >> (4 * c4 + 3) & 1u) ? wj : 0.f;
+                    lab[tid * 8 + c4] = l;
+                }
+            }
+            __syncthreads();
+            float y[R][32];
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int c = 0; c < 32; ++c) y[r][c] = 0.f;
+#pragma unroll 2
+            for (int j = 0; j < kTileJ; ++j) {
+                const JRec<D> rj = load_jrec<D>(sj, j);
+                float ps[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) ps[r] = psi_pair<D>(ui[r], rj.u);
+#pragma unroll
+                for (int c4 = 0; c4 < 8; ++c4) {
+                    const float4 l = lab[j * 8 + c4];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        y[r][4 * c4] = __fmaf_rn(ps[r], l.x, y[r][4 * c4]);
+                        y[r][4 * c4 + 1] = __fmaf_rn(ps[r], l.y, y[r][4 * c4 + 1]);
+                        y[r][4 * c4 + 2] = __fmaf_rn(ps[r], l.z, y[r][4 * c4 + 2]);
+                        y[r][4 * c4 + 3] = __fmaf_rn(ps[r], l.w, y[r][4 * c4 + 3]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double fw = f * (double)wi[r];
+#pragma unroll
+                for (int c = 0; c < 32; ++c)
+                    if (mi[r] >> c & 1u) q[c] += fw * (double)y[r][c];
+            }
+        }
+        if (diag) {  // remove the i == j terms: a_ic w_i^2 psi_ii, halved like the rest of the diagonal tile
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double s = 0.5 * (double)wi[r] * (double)wi[r];
+#pragma unroll
+                for (int c = 0; c < 32; ++c)
+                    if (mi[r] >> c & 1u) q[c] -= s;
+            }
+        }
+    }
+    // block reduction, fixed order
+    __shared__ double s_q[kThreads / 32][32];
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+        const double t = warp_sum(q[c]);
+        if ((tid & 31) == 0) s_q[tid >> 5][c] = t;
+    }
+    __syncthreads();
+    if (tid < 32) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; ++w) s += s_q[w][tid];
+        partialQ[(long long)blockIdx.x * 32 + tid] = s;
+    }
+}
+
+// out[c] = sum over blocks b (in order) of partials[b * ncol + c].
+__global__ void k_reduce_cols(const double *__restrict__ partials, int nblk, int ncol, double *__restrict__ out)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncol) return;
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) s += partials[(long long)b * ncol + c];
+    out[c] = s;
+}
+
+// R_c = sum_i a_ic w_i r_i and W_c = sum_i a_ic w_i for the 32 columns of mask word g = blockIdx.y, r_i the total
+// row sum; slot 32 of each partial holds the all-rows sums (2S and the total weight).  Lane = column.
+constexpr int kRWCols = 33;
+template <int C>
+__global__ void __launch_bounds__(kThreads) k_perm_RW(const float *__restrict__ rec, int F, int dim,
+                                                     const uint32_t *__restrict__ maskg, const double *__restrict__ rowsum,
+                                                     long long npad, int nchunk, double *__restrict__ partials)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = blockIdx.y;
+    const long long rows_per_chunk = (npad + nchunk - 1) / nchunk;
+    const long long r0 = blockIdx.x * rows_per_chunk, r1 = min(npad, r0 + rows_per_chunk);
+    double R = 0.0, W = 0.0, Rall = 0.0, Wall = 0.0;
+    for (long long i = r0 + warp; i < r1; i += kThreads / 32) {
+        const double w = (double)rec[i * F + dim];
+        double r = 0.0;
+#pragma unroll
+        for (int c = 0; c < C; ++c) r += rowsum[(long long)c * npad + i];
+        const uint32_t m = maskg[(long long)g * npad + i];
+        const double wr = w * r;
+        if (m >> lane & 1u) { R += wr; W += w; }
+        Rall += wr;
+        Wall += w;
+    }
+    __shared__ double s[kThreads / 32][2][kRWCols];
+    s[warp][0][lane] = R;
+    s[warp][1][lane] = W;
+    if (lane == 0) { s[warp][0][32] = Rall; s[warp][1][32] = Wall; }
+    __syncthreads();
+    if (threadIdx.x < 2 * kRWCols) {
+        const int which = threadIdx.x / kRWCols, col = threadIdx.x % kRWCols;
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; ++w) t += s[w][which][col];
+        // partials[g][chunk][which][col]
+        partials[(((long long)g * nchunk + blockIdx.x) * 2 + which) * kRWCols + col] = t;
+    }
+}
+
+// Class-pair sums from row sums: out[tile][c2] = sum_{i in tile} w_i rowsum[c2][i]  (tile = kPad rows, one class).
+template <int C>
+__global__ void __launch_bounds__(kThreads) k_class_sums(const float *__restrict__ rec, int F, int dim,
+                                                        const double *__restrict__ rowsum, long long npad,
+                                                        double *__restrict__ out)
+{
+    __shared__ double s[kThreads / 32][C];
+    const long long base = (long long)blockIdx.x * kPad;
+    double a[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) a[c] = 0.0;
+    for (int k = threadIdx.x; k < kPad; k += kThreads) {
+        const double w = (double)rec[(base + k) * F + dim];
+#pragma unroll
+        for (int c = 0; c < C; ++c) a[c] += w * rowsum[(long long)c * npad + base + k];
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+        const double t = warp_sum(a[c]);
+        if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5][c] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < C) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; ++w) t += s[w][threadIdx.x];
+        out[(long long)blockIdx.x * C + threadIdx.x] = t;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ labels
+// Radix select of the n-th smallest composite key per permutation, 8 bits per pass from the top (reading R4).
+// state[p] = {prefix (the digits fixed so far), rank (0-based rank still to locate inside the prefix bucket)}.
+struct SelState {
+    unsigned long long prefix;
+    long long rank;
+};
+
+__global__ void k_sel_init(SelState *st, int nperm, long long n_x)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < nperm) { st[p].prefix = 0ull; st[p].rank = n_x - 1; }
+}
+
+// pass d (0..7): histogram of digit d of the keys whose higher digits equal the prefix.  grid = (event chunks, nperm/4)
+__global__ void __launch_bounds__(kThreads) k_sel_hist(long long N, int nperm, uint32_t seed_lo, uint32_t seed_hi, int pass,
+                                                      const SelState *__restrict__ st, unsigned int *__restrict__ hist,
+                                                      int ev_per_thread)
+{
+    __shared__ unsigned int h[4][256];
+    for (int k = threadIdx.x; k < 1024; k += kThreads) (&h[0][0])[k] = 0u;
+    const int p4 = blockIdx.y;
+    unsigned long long pre[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) pre[q] = (4 * p4 + q < nperm) ? st[4 * p4 + q].prefix : 0ull;
+    __syncthreads();
+    const int shift = 56 - 8 * pass;
+    const long long base = (long long)blockIdx.x * kThreads * ev_per_thread;
+    for (int e = 0; e < ev_per_thread; ++e) {
+        const long long i = base + (long long)e * kThreads + threadIdx.x;
+        if (i >= N) break;
+        uint64_t K[4];
+        label_keys4((uint32_t)i, (uint32_t)p4, seed_lo, seed_hi, K);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (4 * p4 + q >= nperm) continue;
+            const bool match = pass == 0 || (K[q] >> (shift + 8)) == pre[q];
+            if (match) atomicAdd(&h[q][(K[q] >> shift) & 255u], 1u);
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < 1024; k += kThreads) {
+        const int q = k >> 8;
+        const unsigned int v = (&h[0][0])[k];
+        if (v && 4 * p4 + q < nperm) atomicAdd(&hist[(long long)(4 * p4 + q) * 256 + (k & 255)], v);
+    }
+}
+
+// one warp per permutation: locate the bucket holding the wanted rank, extend the prefix, clear the histogram
+__global__ void k_sel_pick(SelState *st, unsigned int *hist, int nperm)
+{
+    const int p = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (p >= nperm) return;
+    unsigned int *h = hist + (long long)p * 256;
+    long long c[8], tot = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { c[k] = h[lane * 8 + k]; tot += c[k]; }
+    long long incl = tot;  // inclusive scan over lanes
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const long long excl = incl - tot, rank = st[p].rank;
+    __syncwarp();
+    if (rank >= excl && rank < incl) {  // exactly one lane
+        long long cum = excl;
+        int b = 7;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (b == 7 && k < 7 && rank < cum + c[k]) b = k;
+            if (b == 7 && k < 7) cum += c[k];
+        }
+        st[p].prefix = (st[p].prefix << 8) | (unsigned long long)(lane * 8 + b);
+        st[p].rank = rank - cum;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < 8; ++k) h[lane * 8 + k] = 0u;
+}
+
+// Writes label words.  After the eight passes st[p].prefix is the n-th smallest composite K*_p; a_ip = (K_ip <= K*_p).
+// Column c of the output: c < col_off is the observed labelling (i < n_x), else permutation c - col_off.
+// Output word for pooled event i and word index g: out[g * stride_g + pos(i) * stride_i].
+struct LabelOut {
+    long long stride_g, stride_i;
+    int nseg;                          // pooled index -> row position, by segments
+    long long seg_first[kMaxCls + 1];  // first pooled index of each segment
+    long long seg_pos[kMaxCls];        // row position of that first index
+};
+__global__ void __launch_bounds__(kThreads) k_label_write(long long N, long long n_x, int nperm, int col_off, int nwords,
+                                                         uint32_t seed_lo, uint32_t seed_hi,
+                                                         const SelState *__restrict__ st, LabelOut L,
+                                                         uint32_t *__restrict__ out)
+{
+    const long long i = blockIdx.x * (long long)kThreads + threadIdx.x;
+    const int g = blockIdx.y;
+    if (i >= N) return;
+    uint32_t word = 0u;
+    uint64_t K[4];
+    int have_p4 = -1;
+    for (int b = 0; b < 32; ++b) {
+        const int c = 32 * g + b;
+        if (c < col_off) { if (i < n_x) word |= 1u << b; continue; }
+        const int p = c - col_off;
+        if (p >= nperm) break;
+        if ((p >> 2) != have_p4) { have_p4 = p >> 2; label_keys4((uint32_t)i, (uint32_t)have_p4, seed_lo, seed_hi, K); }
+        if (K[p & 3] <= st[p].prefix) word |= 1u << b;
+    }
+    long long pos = i;
+    for (int s = 0; s < L.nseg; ++s)
+        if (i >= L.seg_first[s] && i < L.seg_first[s + 1]) pos = L.seg_pos[s] + (i - L.seg_first[s]);
+    (void)nwords;
+    out[(long long)g * L.stride_g + pos * L.stride_i] = word;
+}
+
+// ------------------------------------------------------------------------------------------------ Sect. 5 split
+// positive[i] = 1 iff C = pB . (pC x pD) > 0 (or -C > 0 when conj), fp64 with the oracle's operation order and no
+// contraction, so the sign agrees bit for bit (reading R11: C == 0 is negative).
+__device__ __forceinline__ int triple_positive(const double *b, const double *c, const double *d, int conj)
+{
+    const double cx = __dsub_rn(__dmul_rn(c[1], d[2]), __dmul_rn(c[2], d[1]));
+    const double cy = __dsub_rn(__dmul_rn(c[2], d[0]), __dmul_rn(c[0], d[2]));
+    const double cz = __dsub_rn(__dmul_rn(c[0], d[1]), __dmul_rn(c[1], d[0]));
+    const double C = __dadd_rn(__dadd_rn(__dmul_rn(b[0], cx), __dmul_rn(b[1], cy)), __dmul_rn(b[2], cz));
+    const double v = conj ? -C : C;
+    return v > 0.0 ? 1 : 0;
+}
+
+// separate pB, pC, pD arrays [n][3] (stride 3) or one [n][3][3] array (stride 9, offsets 0, 3, 6)
+__global__ void k_podd_flags(const double *pB, const double *pC, const double *pD, long long n, int stride, int conj,
+                             uint8_t *positive, unsigned long long *count)
+{
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int f = 0;
+    if (i < n) {
+        f = triple_positive(pB + i * stride, pC + i * stride, pD + i * stride, conj);
+        positive[i] = (uint8_t)f;
+    }
+    const unsigned int b = __ballot_sync(0xffffffffu, f);
+    if ((threadIdx.x & 31) == 0 && b) atomicAdd(count, (unsigned long long)__popc(b));
+}
+
+// Stable partition of the pooled source events into the four class segments of the P-odd layout:
+// layout class 0 = I (D, C_T > 0), 1 = IV (Dbar, -Cbar_T <= 0), 2 = II, 3 = III; A = {0, 1}, B = {2, 3}.
+__device__ __forceinline__ int podd_layout_class(long long s, long long n, const uint8_t *posx, const uint8_t *posb)
+{
+    if (s < n) return posx[s] ? 0 : 2;
+    return posb[s - n] ? 3 : 1;
+}
+constexpr int kPartBlock = 1024;
+__global__ void __launch_bounds__(kPartBlock) k_part_count(long long N, long long n, const uint8_t *posx, const uint8_t *posb,
+                                                          int *__restrict__ blk_cnt)
+{
+    __shared__ int cnt[4];
+    if (threadIdx.x < 4) cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const long long s = blockIdx.x * (long long)kPartBlock + threadIdx.x;
+    if (s < N) atomicAdd(&cnt[podd_layout_class(s, n, posx, posb)], 1);
+    __syncthreads();
+    if (threadIdx.x < 4) blk_cnt[blockIdx.x * 4 + threadIdx.x] = cnt[threadIdx.x];
+}
+// single thread block: exclusive scan over blocks per class; totals[4]
+__global__ void k_part_scan(int nblk, int *__restrict__ blk_cnt, long long *__restrict__ totals)
+{
+    if (threadIdx.x < 4) {
+        long long run = 0;
+        for (int b = 0; b < nblk; ++b) {
+            const int v = blk_cnt[b * 4 + threadIdx.x];
+            blk_cnt[b * 4 + threadIdx.x] = (int)run;
+            run += v;
+        }
+        totals[threadIdx.x] = run;
+    }
+}
+// src[seg_pos[c] + rank] = s, ranks in increasing s (stable)
+__global__ void __launch_bounds__(kPartBlock) k_part_scatter(long long N, long long n, const uint8_t *posx, const uint8_t *posb,
+                                                            const int *__restrict__ blk_off, const long long *__restrict__ seg_pos,
+                                                            int *__restrict__ src)
+{
+    __shared__ int warp_cnt[kPartBlock / 32][4];
+    const long long s = blockIdx.x * (long long)kPartBlock + threadIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c = s < N ? podd_layout_class(s, n, posx, posb) : -1;
+    unsigned int bal[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) bal[k] = __ballot_sync(0xffffffffu, c == k);
+    if (lane < 4) warp_cnt[warp][lane] = __popc(bal[lane]);
+    __syncthreads();
+    if (c >= 0) {
+        int rank = __popc(bal[c] & ((1u << lane) - 1u));
+        for (int w = 0; w < warp; ++w) rank += warp_cnt[w][c];
+        src[seg_pos[c] + blk_off[blockIdx.x * 4 + c] + rank] = (int)s;
+    }
+}
+__global__ void k_fill_int(int *p, long long n, int v)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+
+// gather of the listed rows of rowsum (test hook et_row_sums)
+__global__ void k_gather_rows(const double *__restrict__ rowsum, long long npad, const long long *__restrict__ pos, long long nrows,
+                              int C, double *__restrict__ out)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= nrows) return;
+    for (int c = 0; c < C; ++c) out[c * nrows + k] = rowsum[(long long)c * npad + pos[k]];
+}
+
+}  // namespace et

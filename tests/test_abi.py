@@ -1,0 +1,66 @@
+"""The C-ABI library loads and exports every symbol include/et.h declares (no compute without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_1612_04705_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.lib()
+
+
+def header_functions():
+    src = open(os.path.join(ROOT, "include", "et.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(et_[a-zA-Z_]+)\s*\(", src)))
+
+
+def test_header_and_binding_list_the_same_symbols():
+    assert header_functions() == sorted(binding.SYMBOLS)
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in header_functions():
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.et_version()
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device et_create must fail loudly (ET_ERR_CUDA), never compute on the CPU."""
+    try:
+        import torch
+
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    if has_gpu:
+        pytest.skip("a GPU is present")
+    h = ctypes.c_void_p()
+    assert lib.et_create(ctypes.byref(h), 0, None) == -6
+    with pytest.raises(binding.EtError):
+        binding.Context(0)
+
+
+def test_product_does_not_import_oracle():
+    """The product path may not route through the oracle."""
+    pkg = os.path.join(ROOT, "paper_1612_04705_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "et_oracle" not in text, f
+
+
+def test_struct_sizes_match_header(lib):
+    # et_result: 9 doubles + int64; et_perm_result adds double + 3 int64; et_stats 3 doubles + 2 int64
+    assert ctypes.sizeof(binding._Result) == 80
+    assert ctypes.sizeof(binding._PermResult) == 80 + 32
+    assert ctypes.sizeof(binding._PoddResult) == 32 + 80 + 112
+    assert ctypes.sizeof(binding._Stats) == 40

@@ -1,0 +1,261 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle -- needs a B200 (-m gpu).
+
+Tolerances (north_star): |dT| <= 1e-6 (|T_XX| + |T_XbarXbar| + |T_XXbar|); labels, split flags, counts and
+p-values bit-exact.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1612_04705_b200 import binding, build
+from paper_1612_04705_b200 import datagen as dg
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    build.build()
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def assert_T_close(got, exp, tol=TOL):
+    scale = exp.term_scale
+    assert abs(got.T - exp.T) <= tol * scale, (got.T, exp.T, scale)
+    for k in ("T_xx", "T_bb", "T_xb"):
+        assert abs(getattr(got, k) - getattr(exp, k)) <= tol * scale, k
+    assert got.W == pytest.approx(exp.W, rel=1e-6) and got.Wbar == pytest.approx(exp.Wbar, rel=1e-6)
+    assert got.n_pairs == exp.n_pairs
+
+
+# ----------------------------------------------------------------------------- closed forms through the GPU
+def test_closed_forms(ctx):
+    sigma = 0.3
+    a = sigma * math.sqrt(2 * math.log(2))
+    assert ctx.T(np.array([[0, 0], [a, 0.0]]), np.array([[0, a], [a, a]]), sigma).T == pytest.approx(0.125, abs=1e-6)
+    r = ctx.T(np.array([[0.0], [a]]), np.array([[2 * a], [3 * a]]), sigma)
+    assert r.T == pytest.approx(0.34326171875, abs=1e-6)
+    A, B = np.zeros((3, 3)), np.zeros((5, 3))
+    B[:, 1] = 0.37
+    assert ctx.T(A, B, 0.5).T == pytest.approx(1 - math.exp(-0.37**2 / 0.5), abs=1e-6)
+    pt = np.full((7, 4), 0.3)
+    assert ctx.T(pt, pt[:4], 0.4).T == pytest.approx(0.0, abs=1e-6)
+
+
+# ----------------------------------------------------------------------------- et_T
+@pytest.mark.parametrize("dim", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_T_random_all_dims(ctx, dim, dtype):
+    rng = np.random.default_rng(100 + dim)
+    n, nbar = 1500 + 37 * dim, 1111  # ragged: not multiples of any tile, n != nbar
+    x = rng.uniform(size=(n, dim)).astype(dtype)
+    xb = (rng.uniform(size=(nbar, dim)) ** 1.1).astype(dtype)
+    sigma = 0.2 * math.sqrt(dim)
+    assert_T_close(ctx.T(x, xb, sigma), oracle.T(x, xb, sigma))
+
+
+def test_T_config0_full(ctx):
+    s = dg.make_sample(dg.config(0))
+    exp = oracle.T(s.x, s.xbar, 0.3)
+    got = ctx.T(s.x, s.xbar, 0.3)
+    assert_T_close(got, exp)
+    # the injected 5 % bump is seen (T well above the null fluctuation of ~2e-4)
+    assert got.T > 5e-4
+
+
+def test_T_tiny_and_edge_sizes(ctx):
+    rng = np.random.default_rng(3)
+    for n, nbar in [(2, 2), (2, 1025), (1024, 1024), (1025, 1023), (3000, 2)]:
+        x, xb = rng.normal(size=(n, 2)), rng.normal(0.2, 1.0, size=(nbar, 2))
+        assert_T_close(ctx.T(x, xb, 0.7), oracle.T(x, xb, 0.7))
+
+
+def test_T_device_pointers_match_host_pointers(ctx):
+    import torch
+
+    s = dg.make_sample(dg.config(0))
+    host = ctx.T(s.x, s.xbar, 0.3)
+    dev = ctx.T(torch.from_numpy(s.x).cuda(), torch.from_numpy(s.xbar).cuda(), 0.3)
+    assert host.T == dev.T and host.S_xb == dev.S_xb  # deterministic, bit for bit
+    again = ctx.T(s.x, s.xbar, 0.3)
+    assert again.T == host.T
+
+
+def test_T_symmetries_on_gpu(ctx):
+    rng = np.random.default_rng(5)
+    x, xb = rng.normal(size=(700, 3)), rng.normal(0.3, 1.2, size=(900, 3))
+    t0 = ctx.T(x, xb, 0.6)
+    sw = ctx.T(xb, x, 0.6)
+    assert abs(sw.T - t0.T) <= TOL * t0.term_scale and abs(sw.T_xx - t0.T_bb) <= TOL * t0.term_scale
+    assert abs(ctx.T(3.7 * x, 3.7 * xb, 3.7 * 0.6).T - t0.T) <= TOL * t0.term_scale
+    assert abs(ctx.T(x + 100.0, xb + 100.0, 0.6).T - t0.T) <= TOL * t0.term_scale
+
+
+def test_T_weighted(ctx):
+    c = dg.config(3, scale=0.01)
+    s = dg.make_sample(c)
+    for sigma in c.sigmas:
+        exp = oracle.T(s.x, s.xbar, sigma, s.wx, s.wxbar)
+        assert_T_close(ctx.T_weighted(s.x, s.wx, s.xbar, s.wxbar, sigma), exp)
+    ones = ctx.T_weighted(s.x, np.ones(c.n), s.xbar, np.ones(c.nbar), 0.3)
+    assert ones.T == ctx.T(s.x, s.xbar, 0.3).T  # P11: unit weights are Eq. 2, same kernel, bit for bit
+
+
+# ----------------------------------------------------------------------------- labels
+@pytest.mark.parametrize("N,n,nperm,seed", [(37, 11, 9, 0xE7E57), (4000, 2000, 50, 0xE7E57), (5003, 1, 33, 7),
+                                            (2049, 2048, 64, 2**63 + 5), (70001, 35000, 40, 99)])
+def test_labels_bit_exact(ctx, N, n, nperm, seed):
+    got = ctx.perm_labels(N, n, nperm, seed)
+    exp = oracle.labels(N, n, nperm, seed)
+    assert got.shape == exp.shape and (got == exp).all()
+    bits = ((got[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1).reshape(N, -1)[:, :nperm]
+    assert (bits.sum(0) == n).all()  # P10
+
+
+def test_labels_large_sampled(ctx):
+    """Config-4 sized label problem: every permutation has exactly n ones; a few permutations against the oracle."""
+    N, n, nperm, seed = 2_000_000, 1_000_000, 96, 0xE7E57 + 4
+    got = ctx.perm_labels(N, n, nperm, seed)
+    for w in range(got.shape[1]):
+        bits = (got[:, w, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1
+        assert (bits.sum(0) == n).all()
+    for p in (0, 37, 95):
+        exp = oracle.labels_range(N, n, p, 1, seed)[0]
+        assert (((got[:, p >> 5] >> (p & 31)) & 1) == exp).all()
+
+
+# ----------------------------------------------------------------------------- row sums
+def test_row_sums(ctx):
+    c = dg.config(2, scale=0.02)
+    s = dg.make_sample(c)
+    rows = np.random.default_rng(1).choice(c.n + c.nbar, 64, replace=False)
+    rx, rb = ctx.row_sums(s.x, s.xbar, 0.2, rows)
+    ex, eb = oracle.row_sums(s.x, s.xbar, 0.2, rows)
+    assert np.allclose(rx, ex, rtol=2e-6, atol=1e-9) and np.allclose(rb, eb, rtol=2e-6, atol=1e-9)
+    w = dg._rng(5).uniform(-0.5, 1.5, c.n + c.nbar)
+    rx, rb = ctx.row_sums(s.x, s.xbar, 0.2, rows, w[: c.n], w[c.n:])
+    ex, eb = oracle.row_sums(s.x, s.xbar, 0.2, rows, w[: c.n], w[c.n:])
+    assert np.allclose(rx, ex, rtol=2e-6, atol=1e-6) and np.allclose(rb, eb, rtol=2e-6, atol=1e-6)
+
+
+# ----------------------------------------------------------------------------- permutation test
+def check_perm(got, exp):
+    scale = exp.observed.term_scale
+    assert_T_close(got.observed, exp.observed)
+    assert np.isnan(got.T_perm).sum() == np.isnan(exp.T_perm).sum()
+    ok = np.isfinite(exp.T_perm)
+    assert np.abs(got.T_perm[ok] - exp.T_perm[ok]).max() <= TOL * scale
+    assert got.nperm == exp.nperm
+    # p-value exact unless a permutation T sits within the guard band of T_obs (reading R5)
+    assert abs(got.count_gt - exp.count_gt) <= got.n_near
+    if got.n_near == 0:
+        assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
+
+
+def test_perm_config0_full(ctx):
+    c = dg.config(0)
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, c.sigma, c.nperm, c.perm_seed)
+    got = ctx.permutation_test(s.x, s.xbar, c.sigma, c.nperm, c.perm_seed)
+    check_perm(got, exp)
+    # same ordering of the permutation T values (the p-value of any threshold is exact)
+    assert (np.argsort(got.T_perm) == np.argsort(exp.T_perm)).all()
+    assert got.n_near == 0
+    # the observed T of the permutation path agrees with et_T to rounding
+    assert abs(got.observed.T - ctx.T(s.x, s.xbar, c.sigma).T) <= 1e-8 * exp.observed.term_scale
+
+
+@pytest.mark.parametrize("n,nbar,dim,nperm", [(300, 500, 5, 70), (1030, 260, 2, 33), (64, 64, 8, 31)])
+def test_perm_small_unequal(ctx, n, nbar, dim, nperm):
+    rng = np.random.default_rng(n + dim)
+    x, xb = rng.uniform(size=(n, dim)), rng.uniform(size=(nbar, dim)) ** 1.2
+    sigma = 0.15 * math.sqrt(dim)
+    check_perm(ctx.permutation_test(x, xb, sigma, nperm, 12345), oracle.perm_test(x, xb, sigma, nperm, 12345))
+
+
+def test_perm_weighted(ctx):
+    c = dg.config(3, scale=0.004)  # 800 + 800 events, weights U[-0.5, 1.5]
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
+    got = ctx.permutation_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
+    check_perm(got, exp)
+
+
+def test_perm_null_sample_is_compatible_with_zero(ctx):
+    """identical distributions -> T fluctuates around zero and permutations straddle it."""
+    x = dg.dalitz_uniform(3000, dg._rng(1))
+    xb = dg.dalitz_uniform(2500, dg._rng(2))
+    r = ctx.permutation_test(x, xb, 0.3, 200, 5)
+    sd = r.T_perm.std()
+    assert abs(r.T_perm.mean()) < 4 * sd / math.sqrt(200)  # P6, statistically
+    assert abs(r.observed.T) < 5 * sd
+    assert 0.005 < r.p_value < 0.995
+
+
+# ----------------------------------------------------------------------------- Sect. 5
+def test_podd_split_bit_exact(ctx):
+    c = dg.config(4, scale=0.02)
+    s = dg.make_sample(c)
+    for mom, conj in ((s.mom_x, False), (s.mom_xbar, True)):
+        B, Cc, D = (np.ascontiguousarray(mom[:, k]) for k in range(3))
+        got, gcnt = ctx.podd_split(B, Cc, D, conj)
+        exp, ecnt = oracle.podd_split(B, Cc, D, conj)
+        assert (got == exp).all() and gcnt == ecnt
+
+
+def test_podd_test_parity(ctx):
+    c = dg.config(4, scale=0.0012)  # 1200 + 1200 events
+    s = dg.make_sample(c)
+    nperm = 40
+    got = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, nperm, c.perm_seed)
+    posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
+    posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
+    I, II, III, IV = s.x[posx == 1], s.x[posx == 0], s.xbar[posb == 1], s.xbar[posb == 0]
+    assert got.count == (len(I), len(II), len(III), len(IV))
+    A, B = np.vstack([I, IV]), np.vstack([II, III])
+    exp = oracle.perm_test(A, B, c.sigma, nperm, c.perm_seed)
+    check_perm(got.p_odd, exp)
+    assert_T_close(got.p_even, oracle.T(s.x, s.xbar, c.sigma))
+
+
+# ----------------------------------------------------------------------------- error behaviour
+def test_error_codes(ctx):
+    x = np.random.default_rng(0).normal(size=(10, 2))
+    with pytest.raises(binding.EtError) as e:
+        ctx.T(x[:1], x, 0.3)
+    assert e.value.status == -1
+    with pytest.raises(binding.EtError) as e:
+        ctx.T(x, x, 0.0)
+    assert e.value.status == -2
+    bad = x.copy()
+    bad[3, 1] = np.nan
+    with pytest.raises(binding.EtError) as e:
+        ctx.T(bad, x, 0.3)
+    assert e.value.status == -3
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_weighted(x, np.full(10, 0.05), x, np.ones(10), 0.3)
+    assert e.value.status == -4
+    with pytest.raises(binding.EtError) as e:
+        ctx.T(np.zeros((4, 9)), np.zeros((4, 9)), 0.3)
+    assert e.value.status == -1
+    # the context is still usable after an error
+    assert math.isfinite(ctx.T(x, x + 0.1, 0.3).T)
+
+
+# ----------------------------------------------------------------------------- BASELINE sizes, sampled
+@pytest.mark.parametrize("index", [1, 2, 3, 4])
+def test_full_size_row_sum_parity(ctx, index):
+    """At BASELINE sizes a full oracle T is too slow; compare per-row class sums on sampled rows."""
+    c = dg.config(index)
+    s = dg.make_sample(c)
+    N = c.n + c.nbar
+    rows = np.random.default_rng(index).choice(N, 24, replace=False)
+    rx, rb = ctx.row_sums(s.x, s.xbar, c.sigma, rows, s.wx, s.wxbar)
+    ex, eb = oracle.row_sums(s.x, s.xbar, c.sigma, rows, s.wx, s.wxbar)
+    assert np.allclose(rx, ex, rtol=3e-6, atol=1e-6) and np.allclose(rb, eb, rtol=3e-6, atol=1e-6)
