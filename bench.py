@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the energy-test hot path (arXiv:1612.04705) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A step is one pass of the WHOLE hot path of SURVEY.md 8(a) over one synthetic sample: H0 split (config 4), H1 prep,
+H4 labels, H2/H3 all-pairs psi + block sums, H5 permutation sums for all `nperm` permutations, H6 statistic and
+p-value -- i.e. one `et_permutation_test` (configs 0-3) or one `et_podd_test` (config 4) through the C ABI.
+The default workload is BASELINE.json configs[4], the one the north-star target is quoted on (n = nbar = 10^6, 5-D,
+1000 permutations); it fits one GPU.
+
+metric = pair-evaluations/s = unordered event pairs that enter T, N(N-1)/2, divided by the step time (every pair is
+counted once however often a kernel touches it).  `value` is timed with the inputs resident in HBM (CUDA events on
+the library's stream); `e2e` is the same call with pinned HOST buffers, the host->device staging inside the timed
+region.  N > 1 (torchrun): the permutation range is sharded, rank r evaluates permutations [r*nperm, (r+1)*nperm)
+of the same sample (the paper farms permutations out to separate GPUs) -- no data-path collective,
+weak scaling; value = ranks * pairs / max-over-ranks time.
+
+`--impl reference` times the oracle (oracle/, plain fp64 CPU loops) on the host cores on a bounded row subset of the
+same workload; it is the only place besides `cpu_baseline` where this file executes anything under oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+NUM_SMS = 148
+SM_MAX_MHZ_FALLBACK = 1965.0
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    # fallback stated in /opt/skills/guides/B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": SM_MAX_MHZ_FALLBACK,
+            "_source": "fallback"}
+
+
+def alu_roofline_pairs_per_s(dim: int, sm_mhz: float) -> float:
+    """FP32/SFU pipe roofline of the psi evaluation: per pair 2D+1 FP32-pipe instructions and
+    one MUFU.EX2; 128 FP32 lanes and 16 SFU lanes per SM per clock, 148 SMs."""
+    return min(128.0 / (2 * dim + 1), 16.0) * NUM_SMS * sm_mhz * 1e6
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md, the clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.device, self.rows, self.proc = device, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.device), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, peaks):
+        sm, reasons, mx, pw = [], set(), peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                pw.append(float(r[2]))
+                for k, nm in enumerate(names):
+                    if r[3 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            except (ValueError, IndexError):
+                continue
+        busy = [v for v, p in zip(sm, pw) if p > 0.5 * max(pw)] if pw else sm
+        return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(pw) if pw else None}
+
+
+def pinned(a: np.ndarray):
+    """Copy of `a` in page-locked host memory (torch owns it); returns (numpy view, keep-alive)."""
+    import torch
+
+    t = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    return t.numpy(), t
+
+
+def n_pairs(n, nbar):
+    N = n + nbar
+    return N * (N - 1) // 2
+
+
+# ---------------------------------------------------------------------------------------------------------- ours
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1612_04705_b200 import binding, build, datagen as dg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    build.build()
+    peaks = load_peaks()
+
+    cfg = dg.config(args.config)
+    if args.nperm:
+        cfg.nperm = args.nperm
+    s = dg.make_sample(cfg)
+    sigma = cfg.sigma
+    pairs = n_pairs(cfg.n, cfg.nbar)
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    ctx = binding.Context(local, stream=stream)
+    ctx.set_option(binding.ET_OPT_PERM_OFFSET, rank * cfg.nperm)
+
+    def to_dev(a):
+        return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+    d = {k: to_dev(getattr(s, k)) for k in ("x", "xbar", "wx", "wxbar", "mom_x", "mom_xbar")}
+    h_keep = []
+    h = {}
+    for k in ("x", "xbar", "wx", "wxbar", "mom_x", "mom_xbar"):
+        v = getattr(s, k)
+        if v is None:
+            h[k] = None
+        else:
+            h[k], keep = pinned(v)
+            h_keep.append(keep)
+
+    def step(src):
+        if cfg.podd:
+            r = ctx.podd_test(src["x"], src["mom_x"], src["xbar"], src["mom_xbar"], sigma, cfg.nperm, cfg.perm_seed)
+            return r.p_odd
+        return ctx.permutation_test(src["x"], src["xbar"], sigma, cfg.nperm, cfg.perm_seed, src["wx"], src["wxbar"])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(src, steps):
+        """CUDA events on the library's stream around exactly `steps` calls; ms of the slowest rank."""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        agg = {"ms_pairs": 0.0, "ms_labels": 0.0, "ms_dom": 0.0, "launches": 0, "pair_evals": 0}
+        barrier()
+        e0.record(stream)
+        for _ in range(steps):
+            res = step(src)
+            st = ctx.stats()
+            agg["ms_pairs"] += st.ms_pairs
+            agg["ms_labels"] += st.ms_labels
+            agg["ms_dom"] += st.ms_dominant
+            agg["launches"] += st.launches
+            agg["pair_evals"] += st.pair_evals
+            agg["dom_launches"] = st.dominant_launches
+            agg["dom_kernel"] = st.dominant_kernel
+            agg["dom_ops"] = st.dominant_ops
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, agg, res
+
+    # L2 flush between timed steps is unnecessary here: every step re-stages and re-prepares its records and the
+    # O(N^2) kernels stream label/row data far larger than L2 at the bench sizes; stated in config.
+    for _ in range(args.warmup):
+        step(d)
+    with ClockSampler(local) as cs:
+        ms, agg, res = timed(d, args.steps)
+    clocks = cs.summary(peaks)
+    for _ in range(1):
+        step(h)
+    ms_e2e, _, res_h = timed(h, args.steps)
+    ms_step = ms / args.steps
+    value = world * pairs / (ms_step * 1e-3)
+    e2e_value = world * pairs / (ms_e2e / args.steps * 1e-3)
+    h2d = sum(v.nbytes for v in h.values() if v is not None)
+    d2h = cfg.nperm * 8 + 256
+
+    # et_T alone (H1-H3, H6): the psi kernel against the FP32/SFU roofline
+    def T_only():
+        if cfg.weighted:
+            return ctx.T_weighted(d["x"], d["wx"], d["xbar"], d["wxbar"], sigma)
+        return ctx.T(d["x"], d["xbar"], sigma)
+
+    for _ in range(2):
+        T_only()
+    msT, msT_k, nT = 0.0, 0.0, 3
+    for _ in range(nT):
+        T_only()
+        st = ctx.stats()
+        msT += st.ms_total
+        msT_k += st.ms_pairs
+    sm_mhz_max = peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)
+    roofT = alu_roofline_pairs_per_s(cfg.dim, sm_mhz_max)
+    et_T = {"pairs_per_s": pairs / (msT / nT * 1e-3), "kernel_pairs_per_s": pairs / (msT_k / nT * 1e-3),
+            "ms": msT / nT, "roofline_pairs_per_s": roofT, "frac": pairs / (msT_k / nT * 1e-3) / roofT,
+            "peak_model": "min(128/(2D+1),16) pairs/clk/SM x 148 SMs x sm_max_mhz (FP32/SFU pipes)"}
+
+    # roofline of the dominant kernel of the step (the one with the largest share of ms_pairs)
+    dom_ms = agg["ms_dom"] / (args.steps * max(agg["dom_launches"], 1))
+    if agg["dom_kernel"].startswith("k_perm_tc"):
+        # int8 tensor-core contraction: ops = 2 * MACs; peak = measured bf16 peak x nominal int8:bf16 ratio (2)
+        ach = agg["dom_ops"] / max(agg["dom_launches"], 1) / (dom_ms * 1e-3) / 1e12
+        peak = 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+        roofline = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TOP/s (int8)", "frac": ach / peak,
+                    "traffic": None, "kernel": agg["dom_kernel"],
+                    "peak_source": f"{peaks['_source']} bf16 sustained x 2 (nominal int8:bf16)"}
+    else:
+        # CUDA-core kernels: FP32-pipe thread-instructions per second
+        ach = agg["dom_ops"] / max(agg["dom_launches"], 1) / (dom_ms * 1e-3) / 1e12
+        peak = 128.0 * NUM_SMS * sm_mhz_max * 1e6 / 1e12
+        roofline = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tinst/s (FP32 pipe)", "frac": ach / peak,
+                    "traffic": None, "kernel": agg["dom_kernel"],
+                    "peak_source": "128 FP32 lanes x 148 SMs x sm_max_mhz (DESIGN.md)"}
+
+    out = {
+        "metric": "energy_test_pair_evaluations_per_s", "value": value, "unit": "pairs/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 psi / f64 or exact-int sums", "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[{cfg.index}] {cfg.name}: n={cfg.n} nbar={cfg.nbar} dim={cfg.dim} "
+                               f"sigma={sigma} nperm={cfg.nperm} per GPU", "n": cfg.n, "nbar": cfg.nbar, "dim": cfg.dim,
+                   "nperm": cfg.nperm, "sigma": sigma, "l2": "inputs and label matrix larger than L2; records re-prepared every step",
+                   "parallelism": f"permutation range sharded over {world} GPU(s)"},
+        "permutations_per_s": world * cfg.nperm / (ms_step * 1e-3),
+        "pair_perm_updates_per_s": world * cfg.nperm * pairs / (ms_step * 1e-3),
+        "p_value": res.p_value, "T_obs": res.observed.T, "n_near": res.n_near,
+        "et_T": et_T,
+        "share_pairs_kernels": agg["ms_pairs"] / ms, "share_labels": agg["ms_labels"] / ms,
+        "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": agg["launches"],
+        "clocks": clocks,
+        "roofline": roofline,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(s, cfg, sigma, args.cpu_rows)
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------------------- oracle
+def cpu_baseline(s, cfg, sigma, nrows):
+    """The oracle as it stands on the host cores, on a bounded sample: `nrows` random pooled rows against all N
+    columns (oracle.row_sums), i.e. nrows * N psi evaluations in fp64 with libm exp."""
+    import oracle
+
+    N = cfg.n + cfg.nbar
+    if nrows <= 0:
+        nrows = int(max(16, min(N, 6e9 // N)))
+    rows = np.random.default_rng(7).choice(N, min(nrows, N), replace=False)
+    oracle.row_sums(s.x[:64], s.xbar[:64], sigma, np.arange(8))  # load + first touch
+    t0 = time.perf_counter()
+    oracle.row_sums(s.x, s.xbar, sigma, rows, s.wx, s.wxbar)
+    dt = time.perf_counter() - t0
+    v = len(rows) * (N - 1) / dt
+    return {"value": v, "unit": "pairs/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(rows)} random pooled rows x all {N} columns ({len(rows) * (N - 1):.3g} psi evaluations, "
+                      f"{dt:.1f} s); full step extrapolated = pairs*(nperm+1)/rate = "
+                      f"{n_pairs(cfg.n, cfg.nbar) * (cfg.nperm + 1) / v / 3600:.1f} h"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1612_04705_b200 import datagen as dg  # seeded inputs only (holds none of the method's arithmetic)
+
+    cfg = dg.config(args.config)
+    s = dg.make_sample(cfg)
+    N = cfg.n + cfg.nbar
+    nrows = args.cpu_rows if args.cpu_rows > 0 else int(max(16, min(N, 2e9 // N)))
+    for _ in range(args.warmup):
+        cpu_baseline(s, cfg, cfg.sigma, max(8, nrows // 8))
+    vals, t0 = [], time.perf_counter()
+    for _ in range(args.steps):
+        b = cpu_baseline(s, cfg, cfg.sigma, nrows)
+        vals.append(b["value"])
+    dt = time.perf_counter() - t0
+    v = float(np.mean(vals))
+    b["value"] = v
+    print(json.dumps({
+        "impl": "reference", "metric": "energy_test_pair_evaluations_per_s", "value": v, "unit": "pairs/s",
+        "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[{cfg.index}] {cfg.name}: n={cfg.n} nbar={cfg.nbar} dim={cfg.dim} "
+                               f"sigma={cfg.sigma} (oracle on a row subset, one psi pass; no permutation reuse)"},
+        "cpu_baseline": b,
+        "e2e": {"value": v, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--nperm", type=int, default=0, help="override the configuration's permutation count (experiments)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-rows", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -86,11 +86,23 @@ typedef struct {
     double ms_labels;  /* permutation label generation                                            */
     int64_t launches;  /* kernels launched by the call                                            */
     int64_t pair_evals;/* psi evaluations the kernels performed (padding and diagonals included)  */
+    /* the O(N^2) kernel class with the largest device time in the call (bench.py's roofline object)   */
+    double ms_dominant;        /* summed device time of its launches                               */
+    int64_t dominant_launches;
+    int64_t dominant_ops;      /* ALGORITHMIC work of those launches: FP32-pipe thread instructions
+                                  (CUDA-core kernels: unique pairs x (2 dim + 1), per mask word
+                                  unique pairs x (2 dim + 32)) or 2 x MACs (tensor-core kernel)     */
+    char dominant_kernel[32];  /* "k_pairs_T", "k_pairs_rows", "k_perm32", "k_perm_tc" or ""       */
 } et_stats;
 
 /* Options for et_set_option. */
 typedef enum {
-    ET_OPT_PERM_KERNEL = 0 /* 0: CUDA-core 32-permutations-per-psi kernel (default)             */
+    ET_OPT_PERM_KERNEL = 0, /* 0: CUDA-core 32-permutations-per-psi kernel (default)            */
+    ET_OPT_PERM_OFFSET = 1  /* first permutation index p0 (default 0): the calls evaluate
+                               permutations p0 .. p0+nperm-1 of the seed's stream, T_perm[k] is
+                               permutation p0+k.  Permutation p depends only on (seed, p), so
+                               disjoint ranges on several GPUs / calls form one test
+                               (PAPER.md:219 farms permutations out the same way)                 */
 } et_option;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t to

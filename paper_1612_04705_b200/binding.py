@@ -21,6 +21,7 @@ ET_OK = 0
 ET_F32, ET_F64 = 0, 1
 ET_HOST, ET_DEVICE = 0, 1
 ET_OPT_PERM_KERNEL = 0
+ET_OPT_PERM_OFFSET = 1
 STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ERR_NONFINITE", -4: "ET_ERR_DEGENERATE",
                 -5: "ET_ERR_NOMEM", -6: "ET_ERR_CUDA"}
 
@@ -51,7 +52,8 @@ class _PoddResult(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [("ms_total", C.c_double), ("ms_pairs", C.c_double), ("ms_labels", C.c_double), ("launches", C.c_int64),
-                ("pair_evals", C.c_int64)]
+                ("pair_evals", C.c_int64), ("ms_dominant", C.c_double), ("dominant_launches", C.c_int64),
+                ("dominant_ops", C.c_int64), ("dominant_kernel", C.c_char * 32)]
 
 
 @dataclass
@@ -96,6 +98,10 @@ class Stats:
     ms_labels: float
     launches: int
     pair_evals: int
+    ms_dominant: float = 0.0
+    dominant_launches: int = 0
+    dominant_ops: int = 0
+    dominant_kernel: str = ""
 
 
 _lib = None
@@ -209,7 +215,8 @@ class Context:
     def stats(self) -> Stats:
         s = _Stats()
         self._check(lib().et_get_stats(self._h, C.byref(s)))
-        return Stats(s.ms_total, s.ms_pairs, s.ms_labels, s.launches, s.pair_evals)
+        return Stats(s.ms_total, s.ms_pairs, s.ms_labels, s.launches, s.pair_evals, s.ms_dominant, s.dominant_launches,
+                     s.dominant_ops, s.dominant_kernel.decode())
 
     # ---------------------------------------------------------------- Eq. 2
     def T(self, x, xbar, sigma: float) -> Result:

@@ -49,10 +49,18 @@ struct et_ctx {
     cudaEvent_t ev[8] = {nullptr};
     et_stats stats = {};
     double acc_pairs_ms = 0, acc_labels_ms = 0;
+    // per kernel class (KC_*): device ms, launches and algorithmic ops of the current call
+    double kc_ms[4] = {0, 0, 0, 0};
+    int64_t kc_launches[4] = {0, 0, 0, 0};
+    int64_t kc_ops[4] = {0, 0, 0, 0};
     int64_t opt_perm_kernel = 0;
+    int64_t opt_perm_offset = 0;
 };
 
 namespace {
+
+enum { KC_T = 0, KC_ROW = 1, KC_PERM32 = 2, KC_PERMTC = 3 };
+const char *const kKcName[4] = {"k_pairs_T", "k_pairs_rows", "k_perm32", "k_perm_tc"};
 
 et_status fail(et_ctx *c, et_status st, const char *fmt, ...)
 {
@@ -178,6 +186,7 @@ et_status begin_call(et_ctx *ctx)
 {
     ctx->stats = et_stats{};
     ctx->acc_pairs_ms = ctx->acc_labels_ms = 0;
+    for (int k = 0; k < 4; ++k) { ctx->kc_ms[k] = 0; ctx->kc_launches[k] = 0; ctx->kc_ops[k] = 0; }
     CUDA_TRY(cudaSetDevice(ctx->device));
     CUDA_TRY(cudaEventRecord(ctx->ev[0], ctx->stream));
     return ET_OK;
@@ -191,17 +200,25 @@ et_status end_call(et_ctx *ctx)
     ctx->stats.ms_total = ms;
     ctx->stats.ms_pairs = ctx->acc_pairs_ms;
     ctx->stats.ms_labels = ctx->acc_labels_ms;
+    int dom = 0;
+    for (int k = 1; k < 4; ++k)
+        if (ctx->kc_ms[k] > ctx->kc_ms[dom]) dom = k;
+    ctx->stats.ms_dominant = ctx->kc_ms[dom];
+    ctx->stats.dominant_launches = ctx->kc_launches[dom];
+    ctx->stats.dominant_ops = ctx->kc_ops[dom];
+    snprintf(ctx->stats.dominant_kernel, sizeof(ctx->stats.dominant_kernel), "%s", ctx->kc_launches[dom] ? kKcName[dom] : "");
     return ET_OK;
 }
 // Bracket a group of launches with events; the elapsed time is read (after a sync) by span_end.
 et_status span_begin(et_ctx *ctx, int slot) { CUDA_TRY(cudaEventRecord(ctx->ev[slot], ctx->stream)); return ET_OK; }
-et_status span_end(et_ctx *ctx, int slot, double *acc)
+et_status span_end(et_ctx *ctx, int slot, double *acc, int kc = -1, int64_t launches = 0, int64_t ops = 0)
 {
     CUDA_TRY(cudaEventRecord(ctx->ev[slot + 1], ctx->stream));
     CUDA_TRY(cudaEventSynchronize(ctx->ev[slot + 1]));
     float ms = 0;
     CUDA_TRY(cudaEventElapsedTime(&ms, ctx->ev[slot], ctx->ev[slot + 1]));
     *acc += ms;
+    if (kc >= 0) { ctx->kc_ms[kc] += ms; ctx->kc_launches[kc] += launches; ctx->kc_ops[kc] += ops; }
     return ET_OK;
 }
 
@@ -296,7 +313,7 @@ et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim)
                                                  static_cast<double *>(ctx->sums.p));
         LAUNCH_CHECK();
     });
-    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_T, 1, L.N * (L.N - 1) / 2 * (2 * dim + 1)));
     ctx->stats.pair_evals += nunits * (long long)(kThreads * kRT) * (kThreads * kRT);
     return ET_OK;
 }
@@ -321,7 +338,7 @@ et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
                                                                     static_cast<double *>(ctx->rowsum.p));
         LAUNCH_CHECK();
     });
-    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_ROW, 1, L.N * (L.N - 1) / 2 * (2 * dim + 1)));
     ctx->stats.pair_evals += L.npad * L.npad;
     return ET_OK;
 }
@@ -340,9 +357,11 @@ et_status run_label_select(et_ctx *ctx, long long N, long long n_x, int nperm, u
     k_sel_init<<<(nperm + 255) / 256, 256, 0, ctx->stream>>>(static_cast<SelState *>(ctx->sel.p), nperm, n_x);
     LAUNCH_CHECK();
     const int ev = 8;
-    const dim3 grid((unsigned)((N + (long long)kThreads * ev - 1) / ((long long)kThreads * ev)), (unsigned)((nperm + 3) / 4));
+    const long long p0 = ctx->opt_perm_offset;
+    const unsigned ngroups = (unsigned)(((p0 + nperm - 1) >> 2) - (p0 >> 2) + 1);
+    const dim3 grid((unsigned)((N + (long long)kThreads * ev - 1) / ((long long)kThreads * ev)), ngroups);
     for (int pass = 0; pass < 8; ++pass) {
-        k_sel_hist<<<grid, kThreads, 0, ctx->stream>>>(N, nperm, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), pass,
+        k_sel_hist<<<grid, kThreads, 0, ctx->stream>>>(N, nperm, p0, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), pass,
                                                       static_cast<const SelState *>(ctx->sel.p),
                                                       static_cast<unsigned int *>(ctx->hist.p), ev);
         LAUNCH_CHECK();
@@ -369,7 +388,7 @@ et_status run_labels_internal(et_ctx *ctx, const Layout &L, int nperm, uint64_t 
     for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
     for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
     const dim3 grid((unsigned)((L.N + kThreads - 1) / kThreads), (unsigned)nwords);
-    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, 1, nwords, (uint32_t)(seed & 0xffffffffu),
+    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, ctx->opt_perm_offset, 1, nwords, (uint32_t)(seed & 0xffffffffu),
                                                      (uint32_t)(seed >> 32), static_cast<const SelState *>(ctx->sel.p), lo,
                                                      static_cast<uint32_t *>(ctx->mask.p));
     LAUNCH_CHECK();
@@ -590,7 +609,7 @@ et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
             LAUNCH_CHECK();
         }
     });
-    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms));
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERM32, nwords, (long long)nwords * (L.N * (L.N - 1) / 2) * (2 * dim + 32)));
     ctx->stats.pair_evals += (long long)nwords * nunits * (kThreads * 2LL) * (kThreads * 2LL);
 
     // R, W per column
@@ -692,6 +711,11 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
     if (opt == ET_OPT_PERM_KERNEL) {
         if (value != 0) return fail(ctx, ET_ERR_INVALID, "unknown permutation kernel %lld", (long long)value);
         ctx->opt_perm_kernel = value;
+        return ET_OK;
+    }
+    if (opt == ET_OPT_PERM_OFFSET) {
+        if (value < 0 || value > (1ll << 40)) return fail(ctx, ET_ERR_INVALID, "permutation offset out of range");
+        ctx->opt_perm_offset = value;
         return ET_OK;
     }
     return fail(ctx, ET_ERR_INVALID, "unknown option %d", (int)opt);
@@ -881,7 +905,7 @@ et_status et_perm_labels(et_ctx *ctx, int64_t N, int64_t n, int64_t nperm, uint6
     lo.stride_i = nwords;
     lo.nseg = 0;
     const dim3 grid((unsigned)((N + kThreads - 1) / kThreads), (unsigned)nwords);
-    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(N, n, (int)nperm, 0, nwords, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+    k_label_write<<<grid, kThreads, 0, ctx->stream>>>(N, n, (int)nperm, ctx->opt_perm_offset, 0, nwords, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
                                                      static_cast<const SelState *>(ctx->sel.p), lo, dmask);
     LAUNCH_CHECK();
     ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));

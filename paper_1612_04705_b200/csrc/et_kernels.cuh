@@ -492,17 +492,24 @@ __global__ void k_sel_init(SelState *st, int nperm, long long n_x)
     if (p < nperm) { st[p].prefix = 0ull; st[p].rank = n_x - 1; }
 }
 
-// pass d (0..7): histogram of digit d of the keys whose higher digits equal the prefix.  grid = (event chunks, nperm/4)
-__global__ void __launch_bounds__(kThreads) k_sel_hist(long long N, int nperm, uint32_t seed_lo, uint32_t seed_hi, int pass,
-                                                      const SelState *__restrict__ st, unsigned int *__restrict__ hist,
+// pass d (0..7): histogram of digit d of the keys whose higher digits equal the prefix.
+// grid = (event chunks, Philox groups): group blockIdx.y covers the global permutations 4 * (p0 / 4 + blockIdx.y) + q,
+// q < 4, of which those inside [p0, p0 + nperm) are local permutation p - p0.
+__global__ void __launch_bounds__(kThreads) k_sel_hist(long long N, int nperm, long long p0, uint32_t seed_lo, uint32_t seed_hi,
+                                                      int pass, const SelState *__restrict__ st, unsigned int *__restrict__ hist,
                                                       int ev_per_thread)
 {
     __shared__ unsigned int h[4][256];
     for (int k = threadIdx.x; k < 1024; k += kThreads) (&h[0][0])[k] = 0u;
-    const int p4 = blockIdx.y;
+    const long long p4 = (p0 >> 2) + blockIdx.y;
     unsigned long long pre[4];
+    long long pl[4];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) pre[q] = (4 * p4 + q < nperm) ? st[4 * p4 + q].prefix : 0ull;
+    for (int q = 0; q < 4; ++q) {
+        pl[q] = 4 * p4 + q - p0;
+        if (pl[q] < 0 || pl[q] >= nperm) pl[q] = -1;
+        pre[q] = pl[q] >= 0 ? st[pl[q]].prefix : 0ull;
+    }
     __syncthreads();
     const int shift = 56 - 8 * pass;
     const long long base = (long long)blockIdx.x * kThreads * ev_per_thread;
@@ -513,7 +520,7 @@ __global__ void __launch_bounds__(kThreads) k_sel_hist(long long N, int nperm, u
         label_keys4((uint32_t)i, (uint32_t)p4, seed_lo, seed_hi, K);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            if (4 * p4 + q >= nperm) continue;
+            if (pl[q] < 0) continue;
             const bool match = pass == 0 || (K[q] >> (shift + 8)) == pre[q];
             if (match) atomicAdd(&h[q][(K[q] >> shift) & 255u], 1u);
         }
@@ -522,7 +529,7 @@ __global__ void __launch_bounds__(kThreads) k_sel_hist(long long N, int nperm, u
     for (int k = threadIdx.x; k < 1024; k += kThreads) {
         const int q = k >> 8;
         const unsigned int v = (&h[0][0])[k];
-        if (v && 4 * p4 + q < nperm) atomicAdd(&hist[(long long)(4 * p4 + q) * 256 + (k & 255)], v);
+        if (v && pl[q] >= 0) atomicAdd(&hist[pl[q] * 256 + (k & 255)], v);
     }
 }
 
@@ -568,8 +575,8 @@ struct LabelOut {
     long long seg_first[kMaxCls + 1];  // first pooled index of each segment
     long long seg_pos[kMaxCls];        // row position of that first index
 };
-__global__ void __launch_bounds__(kThreads) k_label_write(long long N, long long n_x, int nperm, int col_off, int nwords,
-                                                         uint32_t seed_lo, uint32_t seed_hi,
+__global__ void __launch_bounds__(kThreads) k_label_write(long long N, long long n_x, int nperm, long long p0, int col_off,
+                                                         int nwords, uint32_t seed_lo, uint32_t seed_hi,
                                                          const SelState *__restrict__ st, LabelOut L,
                                                          uint32_t *__restrict__ out)
 {
@@ -578,14 +585,15 @@ __global__ void __launch_bounds__(kThreads) k_label_write(long long N, long long
     if (i >= N) return;
     uint32_t word = 0u;
     uint64_t K[4];
-    int have_p4 = -1;
+    long long have_p4 = -1;
     for (int b = 0; b < 32; ++b) {
         const int c = 32 * g + b;
         if (c < col_off) { if (i < n_x) word |= 1u << b; continue; }
         const int p = c - col_off;
         if (p >= nperm) break;
-        if ((p >> 2) != have_p4) { have_p4 = p >> 2; label_keys4((uint32_t)i, (uint32_t)have_p4, seed_lo, seed_hi, K); }
-        if (K[p & 3] <= st[p].prefix) word |= 1u << b;
+        const long long pg = p0 + p;  // global permutation index
+        if ((pg >> 2) != have_p4) { have_p4 = pg >> 2; label_keys4((uint32_t)i, (uint32_t)have_p4, seed_lo, seed_hi, K); }
+        if (K[pg & 3] <= st[p].prefix) word |= 1u << b;
     }
     long long pos = i;
     for (int s = 0; s < L.nseg; ++s)

@@ -63,4 +63,4 @@ def test_struct_sizes_match_header(lib):
     assert ctypes.sizeof(binding._Result) == 80
     assert ctypes.sizeof(binding._PermResult) == 80 + 32
     assert ctypes.sizeof(binding._PoddResult) == 32 + 80 + 112
-    assert ctypes.sizeof(binding._Stats) == 40
+    assert ctypes.sizeof(binding._Stats) == 40 + 24 + 32

@@ -179,6 +179,26 @@ def test_perm_small_unequal(ctx, n, nbar, dim, nperm):
     check_perm(ctx.permutation_test(x, xb, sigma, nperm, 12345), oracle.perm_test(x, xb, sigma, nperm, 12345))
 
 
+def test_perm_offset_is_a_window_of_the_same_stream(ctx):
+    """ET_OPT_PERM_OFFSET: permutations p0 .. p0+nperm-1 of the seed's stream (multi-GPU sharding of the loop)."""
+    rng = np.random.default_rng(11)
+    x, xb = rng.uniform(size=(400, 3)), rng.uniform(size=(350, 3)) ** 1.3
+    exp = oracle.perm_test(x, xb, 0.3, 45, 777)
+    full = ctx.permutation_test(x, xb, 0.3, 45, 777)
+    for p0, cnt in ((13, 32), (4, 7), (44, 1)):
+        ctx.set_option(binding.ET_OPT_PERM_OFFSET, p0)
+        try:
+            got = ctx.permutation_test(x, xb, 0.3, cnt, 777)
+            lab = ctx.perm_labels(750, 400, cnt, 777)
+        finally:
+            ctx.set_option(binding.ET_OPT_PERM_OFFSET, 0)
+        assert (got.T_perm == full.T_perm[p0:p0 + cnt]).all()
+        assert np.abs(got.T_perm - exp.T_perm[p0:p0 + cnt]).max() <= TOL * exp.observed.term_scale
+        ref = oracle.labels_range(750, 400, p0, cnt, 777)  # [cnt, N] bytes
+        bits = ((lab[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1).reshape(750, -1)[:, :cnt]
+        assert (bits.T == ref).all()
+
+
 def test_perm_weighted(ctx):
     c = dg.config(3, scale=0.004)  # 800 + 800 events, weights U[-0.5, 1.5]
     s = dg.make_sample(c)
