@@ -69,7 +69,9 @@ typedef struct {
     et_result observed;
     double p_value;   /* count_gt / nperm  (strict >; reading R3)                   */
     int64_t count_gt; /* #{p : T_p > T_obs}                                                       */
-    int64_t n_near;   /* #{p : |T_p - T_obs| <= 1e-9 (|T_xx|+|T_bb|+|T_xb|)} or T_p NaN (R5, R10) */
+    int64_t n_near;   /* #{p : |T_p - T_obs| <= guard} or T_p NaN (R5, R10); guard = 1e-9 (|T_xx|+
+                         |T_bb|+|T_xb|), plus, on the tensor-core path, 8 sigma of the 15-bit
+                         quantisation noise of T_p - T_obs.  count_gt is exact when 0 */
     int64_t nperm;
 } et_perm_result;
 
@@ -97,7 +99,10 @@ typedef struct {
 
 /* Options for et_set_option. */
 typedef enum {
-    ET_OPT_PERM_KERNEL = 0, /* 0: CUDA-core 32-permutations-per-psi kernel (default)            */
+    ET_OPT_PERM_KERNEL = 0, /* permutation sums: 0 (default) = tensor-core contraction (tcgen05
+                               kind::i8, psi quantised to 15 bits, exact integer sums) when the
+                               padded pooled size is >= 16384 rows, else the fp32 CUDA-core
+                               kernel; 1 = always CUDA cores; 2 = always tensor cores            */
     ET_OPT_PERM_OFFSET = 1  /* first permutation index p0 (default 0): the calls evaluate
                                permutations p0 .. p0+nperm-1 of the seed's stream, T_perm[k] is
                                permutation p0+k.  Permutation p depends only on (seed, p), so

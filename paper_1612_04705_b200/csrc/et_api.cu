@@ -7,10 +7,12 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "../../include/et.h"
 #include "et_kernels.cuh"
+#include "et_tc.cuh"
 
 using namespace et;
 
@@ -55,6 +57,9 @@ struct et_ctx {
     int64_t kc_ops[4] = {0, 0, 0, 0};
     int64_t opt_perm_kernel = 0;
     int64_t opt_perm_offset = 0;
+    double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
+    Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW;
+    bool tc_attr_set = false;
 };
 
 namespace {
@@ -233,22 +238,24 @@ template <typename TIn>
 et_status run_prep_t(et_ctx *ctx, const TIn *x, const TIn *xbar, const double *wx, const double *wxbar, const int *src,
                      const Layout &L, int dim, double sigma)
 {
-    ET_TRY(ensure(ctx, ctx->mm, 16 * sizeof(uint32_t)));
+    ET_TRY(ensure(ctx, ctx->mm, 18 * sizeof(uint32_t)));
     ET_TRY(ensure(ctx, ctx->flag, sizeof(int)));
     ET_TRY(ensure_pinned(ctx, 4096));
     uint32_t *h = static_cast<uint32_t *>(ctx->pinned);
-    for (int k = 0; k < 8; ++k) { h[2 * k] = 0xffffffffu; h[2 * k + 1] = 0u; }
-    CUDA_TRY(cudaMemcpyAsync(ctx->mm.p, h, 16 * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+    for (int k = 0; k < 9; ++k) { h[2 * k] = 0xffffffffu; h[2 * k + 1] = 0u; }
+    CUDA_TRY(cudaMemcpyAsync(ctx->mm.p, h, 18 * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
     CUDA_TRY(cudaMemsetAsync(ctx->flag.p, 0, sizeof(int), ctx->stream));
     const int grid = ctx->num_sms * 4;
     k_minmax<TIn><<<grid, 256, 0, ctx->stream>>>(x, L.n, dim, wx, static_cast<uint32_t *>(ctx->mm.p), static_cast<int *>(ctx->flag.p));
     LAUNCH_CHECK();
     k_minmax<TIn><<<grid, 256, 0, ctx->stream>>>(xbar, L.nbar, dim, wxbar, static_cast<uint32_t *>(ctx->mm.p), static_cast<int *>(ctx->flag.p));
     LAUNCH_CHECK();
-    CUDA_TRY(cudaMemcpyAsync(h + 32, ctx->mm.p, 16 * sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(h + 32, ctx->mm.p, 18 * sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
     CUDA_TRY(cudaMemcpyAsync(h + 64, ctx->flag.p, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CUDA_TRY(cudaStreamSynchronize(ctx->stream));
     if (h[64] != 0) return fail(ctx, ET_ERR_NONFINITE, "NaN or Inf in coordinates or weights");
+    ctx->wmin = ctx->wmax = 1.0;
+    if (wx) { ctx->wmin = (double)key2f(h[32 + 16]); ctx->wmax = (double)key2f(h[32 + 17]); }
 
     PrepParams P{};
     for (int k = 0; k < dim; ++k) P.centre[k] = 0.5 * ((double)key2f(h[32 + 2 * k]) + (double)key2f(h[32 + 2 * k + 1]));
@@ -654,6 +661,204 @@ et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, 
     return ET_OK;
 }
 
+
+// ---- tensor-core permutation sums (K-PERM-TC) -------------------------------------------------------------
+// T for every label column of the TC layout (et_tc.cuh): chunk ch, column c at index ch * 512 + c.
+__global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__ Q, const double *__restrict__ R, const double *__restrict__ W,
+                                                     int nperm, long long npairs_obs, long long npairs_second, double qstep,
+                                                     double nA, double nB, double *__restrict__ T_perm, DevPerm *out, DevT *second)
+{
+    __shared__ DevT obs;
+    __shared__ unsigned long long s_cnt, s_near;
+    const double S = Q[2], Wtot = W[2];  // the all-ones column
+    if (threadIdx.x == 0) {
+        form_result(Q[0], S - R[0] + Q[0], R[0] - 2.0 * Q[0], W[0], Wtot - W[0], npairs_obs, &obs);
+        DevT sec;
+        form_result(Q[1], S - R[1] + Q[1], R[1] - 2.0 * Q[1], W[1], Wtot - W[1], npairs_second, &sec);
+        *second = sec;
+        s_cnt = 0ull;
+        s_near = 0ull;
+    }
+    __syncthreads();
+    const double Tobs = obs.r.T;
+    // guard band (reading R5): 1e-9 of the term scale plus 8 sigma of the quantisation noise of T_p - T_obs; every
+    // pair carries an independent rounding error of variance qstep^2 / 12, so
+    // var(T) = qstep^2/12 [ pairs_xx / (W(W-1))^2 + pairs_bb / (Wb(Wb-1))^2 + pairs_xb / (W Wb)^2 ].
+    const double Wo = obs.r.W, Wb = obs.r.Wbar;
+    const double var = 0.5 * nA * (nA - 1.0) / ((Wo * (Wo - 1.0)) * (Wo * (Wo - 1.0))) + 0.5 * nB * (nB - 1.0) / ((Wb * (Wb - 1.0)) * (Wb * (Wb - 1.0))) +
+                       nA * nB / ((Wo * Wb) * (Wo * Wb));
+    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb)) + 8.0 * 1.4142135623730951 * qstep * sqrt(var / 12.0);
+    unsigned long long cnt = 0, near = 0;
+    for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
+        const int k = (p / tc::kPermsPerChunk) * tc::kCols + tc::kSpecial + p % tc::kPermsPerChunk;
+        // S of the chunk the column lives in: identical integers in every chunk (same quantised Psi), use chunk 0
+        const double q = Q[k], r = R[k], w = W[k];
+        DevT t;
+        form_result(q, S - r + q, r - 2.0 * q, w, Wtot - w, npairs_obs, &t);
+        T_perm[p] = t.r.T;
+        if (t.status != 0) { near += 1; continue; }
+        if (t.r.T > Tobs) cnt += 1;
+        if (fabs(t.r.T - Tobs) <= guard) near += 1;
+    }
+    atomicAdd(&s_cnt, cnt);
+    atomicAdd(&s_near, near);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        out->r.observed = obs.r;
+        out->r.count_gt = (long long)s_cnt;
+        out->r.n_near = (long long)s_near;
+        out->r.nperm = nperm;
+        out->r.p_value = (double)s_cnt / (double)nperm;
+        out->status = obs.status;
+    }
+}
+
+template <int D>
+et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted)
+{
+    if (weighted) {
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemTC));
+        tc::k_perm_tc<D, true><<<grid, tc::kThreadsTC, tc::kSmemTC, ctx->stream>>>(P);
+    } else {
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemTC));
+        tc::k_perm_tc<D, false><<<grid, tc::kThreadsTC, tc::kSmemTC, ctx->stream>>>(P);
+    }
+    LAUNCH_CHECK();
+    return ET_OK;
+}
+
+// Labels (TC layout), the contraction for every 512-column chunk, W_c, then the statistic.
+// lab2_classes: class segments that form sample X of the second labelling (column 1).
+et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted, unsigned lab2_classes,
+                      long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second)
+{
+    const int nchunks = (nperm + tc::kPermsPerChunk - 1) / tc::kPermsPerChunk;
+    const int words_total = nchunks * tc::kWordsPerChunk;
+    // labels
+    ET_TRY(span_begin(ctx, 4));
+    ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
+    ET_TRY(ensure(ctx, ctx->maskT, (size_t)L.npad * words_total * sizeof(uint32_t)));
+    CUDA_TRY(cudaMemsetAsync(ctx->maskT.p, 0, (size_t)L.npad * words_total * sizeof(uint32_t), ctx->stream));
+    LabelOut lo{};
+    lo.nseg = L.ncls;
+    for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
+    for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
+    {
+        const dim3 grid((unsigned)((L.N + kThreads - 1) / kThreads), (unsigned)words_total);
+        tc::k_label_write_tc<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, ctx->opt_perm_offset, (uint32_t)(seed & 0xffffffffu),
+                                                                (uint32_t)(seed >> 32), static_cast<const SelState *>(ctx->sel.p), lo,
+                                                                lab2_classes, words_total, static_cast<uint32_t *>(ctx->maskT.p));
+        LAUNCH_CHECK();
+    }
+    ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
+
+    // unit table: row tile I against K blocks [2 I, NK) in pieces of <= Lmax, longest first, unit u -> CTA u % grid
+    const int nT = (int)(L.npad / tc::kTM), NK = (int)(L.npad / tc::kKB);
+    long long total_kb = 0;
+    for (int I = 0; I < nT; ++I) total_kb += NK - 2 * I;
+    long long Lmax = (total_kb + (long long)ctx->num_sms * 24 - 1) / ((long long)ctx->num_sms * 24);
+    if (Lmax < 8) Lmax = 8;
+    if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
+    std::vector<tc::Unit> full, tail;
+    for (int I = 0; I < nT; ++I)
+        for (int kb = 2 * I; kb < NK; kb += (int)Lmax) {
+            tc::Unit u{I, kb, (int)std::min<long long>(NK, kb + Lmax), 0};
+            (u.kb_end - u.kb_begin == Lmax ? full : tail).push_back(u);
+        }
+    std::stable_sort(tail.begin(), tail.end(), [](const tc::Unit &a, const tc::Unit &b) { return a.kb_end - a.kb_begin > b.kb_end - b.kb_begin; });
+    full.insert(full.end(), tail.begin(), tail.end());
+    const int nunits = (int)full.size();
+    ET_TRY(ensure(ctx, ctx->units, full.size() * sizeof(tc::Unit)));
+    CUDA_TRY(cudaMemcpyAsync(ctx->units.p, full.data(), full.size() * sizeof(tc::Unit), cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // `full` goes out of scope
+
+    // quantisation scale: v ~ sc Psi, 0 <= v < 2^15 (unsigned hi digit) or |v| < 2^14 (signed hi digit)
+    double sc;
+    bool hi_signed = false;
+    if (!weighted) sc = 32767.0;
+    else if (ctx->wmin >= 0.0) sc = 32767.0 / std::max(ctx->wmax, 1e-30);
+    else { hi_signed = true; sc = 16383.0 / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
+
+    const int grid = std::min(ctx->num_sms, nunits);
+    const size_t part_bytes = (size_t)grid * tc::kProducerWarps * 8 * 32 * 2 * 8;
+    ET_TRY(ensure(ctx, ctx->tcpart, part_bytes));
+    ET_TRY(ensure(ctx, ctx->tcQ, (size_t)nchunks * tc::kCols * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
+    ET_TRY(span_begin(ctx, 2));
+    for (int ch = 0; ch < nchunks; ++ch) {
+        tc::TCParams P{};
+        P.rec = static_cast<const float *>(ctx->rec.p);
+        P.maskT = static_cast<const uint32_t *>(ctx->maskT.p);
+        P.words_total = words_total;
+        P.word0 = ch * tc::kWordsPerChunk;
+        P.units = static_cast<const tc::Unit *>(ctx->units.p);
+        P.nunits = nunits;
+        P.sc2 = (float)(2.0 * sc);
+        P.idesc_hi = tc::umma_idesc_i8(hi_signed);
+        P.partial = ctx->tcpart.p;
+        DISPATCH_DIM(dim, ET_TRY(launch_perm_tc<D>(ctx, P, grid, weighted)));
+        // the scale actually applied is the fp32 value of 2 sc
+        const double inv_sc = 2.0 / (double)P.sc2;
+        if (weighted)
+            tc::k_tc_reduce<true><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
+                                                            static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
+        else
+            tc::k_tc_reduce<false><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
+                                                             static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
+        LAUNCH_CHECK();
+    }
+    {
+        const long long pairs = L.N * (L.N - 1) / 2;
+        ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * tc::kCols * nchunks));
+        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM * tc::kKB;
+    }
+
+    // W_c
+    const int nchunkW = 64;
+    ET_TRY(ensure(ctx, ctx->tcWpart, (size_t)words_total * nchunkW * 32 * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->tcW, (size_t)words_total * 32 * sizeof(double)));
+    {
+        const dim3 gridW((unsigned)nchunkW, (unsigned)words_total);
+        tc::k_perm_W_tc<<<gridW, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+                                                            static_cast<const uint32_t *>(ctx->maskT.p), words_total, L.npad, nchunkW,
+                                                            static_cast<double *>(ctx->tcWpart.p));
+        LAUNCH_CHECK();
+        for (int wd = 0; wd < words_total; ++wd) {
+            k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->tcWpart.p) + (long long)wd * nchunkW * 32, nchunkW, 32,
+                                                     static_cast<double *>(ctx->tcW.p) + wd * 32);
+            LAUNCH_CHECK();
+        }
+    }
+    // statistic
+    const double wabs = std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin));
+    const double qstep = wabs / sc;  // one rounding step of w_j psi_ij, times |w_i| <= wabs
+    ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
+    DevT *dev_second = reinterpret_cast<DevT *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm));
+    k_perm_stat_tc<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->tcQ.p), static_cast<const double *>(ctx->tcR.p),
+                                               static_cast<const double *>(ctx->tcW.p), nperm, npairs_obs, npairs_second, qstep,
+                                               (double)L.n_a, (double)(L.N - L.n_a),
+                                               static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p), dev_second);
+    LAUNCH_CHECK();
+    DevPerm r;
+    ET_TRY(fetch(ctx, ctx->result.p, &r));
+    if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "weighted normalisation degenerate: W = %g, Wbar = %g (need > 1)", r.r.observed.W, r.r.observed.Wbar);
+    DevT sec;
+    ET_TRY(fetch(ctx, dev_second, &sec));
+    CUDA_TRY(cudaMemcpyAsync(T_perm, ctx->tperm.p, (size_t)nperm * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    *out = r.r;
+    if (second) *second = sec.r;
+    return ET_OK;
+}
+
+bool use_tc(const et_ctx *ctx, const Layout &L)
+{
+    if (ctx->opt_perm_kernel == 1) return false;
+    if (ctx->opt_perm_kernel == 2) return true;
+    return L.npad >= 16384;
+}
+
 }  // namespace
 
 // =============================================================================================== C ABI
@@ -693,7 +898,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->tilecls, &ctx->partials, &ctx->sums, &ctx->rowsum, &ctx->mask, &ctx->sel, &ctx->hist, &ctx->partQ,
                    &ctx->Q, &ctx->partRW, &ctx->RW, &ctx->mm, &ctx->flag, &ctx->counter, &ctx->src, &ctx->posx, &ctx->posb,
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
-                   &ctx->count64};
+                   &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
@@ -709,7 +914,7 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
 {
     if (!ctx) return ET_ERR_INVALID;
     if (opt == ET_OPT_PERM_KERNEL) {
-        if (value != 0) return fail(ctx, ET_ERR_INVALID, "unknown permutation kernel %lld", (long long)value);
+        if (value < 0 || value > 2) return fail(ctx, ET_ERR_INVALID, "unknown permutation kernel %lld", (long long)value);
         ctx->opt_perm_kernel = value;
         return ET_OK;
     }
@@ -762,12 +967,16 @@ et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int6
     layout_two(L, n, nbar);
     ET_TRY(upload_tile_classes(ctx, L));
     ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigma));
-    int nwords = 0;
-    ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
-    ET_TRY(run_pairs_rows(ctx, L, dim));
-    ET_TRY(run_perm_sums(ctx, L, dim, nwords));
     et_perm_result r;
-    ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), T_perm, &r));
+    if (use_tc(ctx, L)) {
+        ET_TRY(run_perm_tc(ctx, L, dim, (int)nperm, seed, wx != nullptr, 0x1u, pairs_two(n, nbar), pairs_two(n, nbar), T_perm, &r, nullptr));
+    } else {
+        int nwords = 0;
+        ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
+        ET_TRY(run_pairs_rows(ctx, L, dim));
+        ET_TRY(run_perm_sums(ctx, L, dim, nwords));
+        ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), T_perm, &r));
+    }
     ET_TRY(end_call(ctx));
     *out = r;
     return ET_OK;
@@ -852,6 +1061,17 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
     LAUNCH_CHECK();
 
     ET_TRY(run_prep(ctx, dx, dxb, nullptr, nullptr, static_cast<const int *>(ctx->src.p), L, dim, dtype, sigma));
+    if (use_tc(ctx, L)) {
+        // layout classes: 0 = I, 1 = IV, 2 = II, 3 = III; P-even sample X = I + II = classes {0, 2}
+        et_perm_result pr;
+        et_result even;
+        ET_TRY(run_perm_tc(ctx, L, dim, (int)nperm, seed, false, 0x5u, pairs_two(nI + nIV, nII + nIII), pairs_two(n, nbar), T_perm, &pr, &even));
+        ET_TRY(end_call(ctx));
+        out->count[0] = nI; out->count[1] = nII; out->count[2] = nIII; out->count[3] = nIV;
+        out->p_even = even;
+        out->p_odd = pr;
+        return ET_OK;
+    }
     ET_TRY(run_class_weights(ctx, L, dim));
     int nwords = 0;
     ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));

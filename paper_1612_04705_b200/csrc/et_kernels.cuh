@@ -11,7 +11,8 @@ namespace et {
 
 // ------------------------------------------------------------------------------------------------ prep
 // Bounding box of the coordinates (for the centre) and the non-finite check.  mm[2*k] = min, mm[2*k+1] = max as
-// order-preserving uint32 keys of the fp32-rounded values; flag[0] != 0 when a NaN/Inf was seen.
+// order-preserving uint32 keys of the fp32-rounded values (mm[16], mm[17]: min / max of the fp32-rounded weights);
+// flag[0] != 0 when a NaN/Inf was seen.
 __device__ __forceinline__ uint32_t f2key(float f)
 {
     uint32_t b = __float_as_uint(f);
@@ -37,6 +38,7 @@ __global__ void k_minmax(const TIn *__restrict__ x, long long n, int dim, const 
 #pragma unroll
     for (int k = 0; k < 8; ++k) { lo[k] = 0xffffffffu; hi[k] = 0u; }
     bool bad = false;
+    uint32_t wlo = 0xffffffffu, whi = 0u;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
 #pragma unroll
         for (int k = 0; k < 8; ++k)
@@ -47,7 +49,23 @@ __global__ void k_minmax(const TIn *__restrict__ x, long long n, int dim, const 
                 lo[k] = min(lo[k], key);
                 hi[k] = max(hi[k], key);
             }
-        if (w && !isfinite(w[i])) bad = true;
+        if (w) {
+            if (!isfinite(w[i])) bad = true;
+            const uint32_t key = f2key((float)w[i]);
+            wlo = min(wlo, key);
+            whi = max(whi, key);
+        }
+    }
+    if (w) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            wlo = min(wlo, __shfl_xor_sync(0xffffffffu, wlo, o));
+            whi = max(whi, __shfl_xor_sync(0xffffffffu, whi, o));
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicMin(&mm[16], wlo);
+            atomicMax(&mm[17], whi);
+        }
     }
 #pragma unroll
     for (int k = 0; k < 8; ++k)

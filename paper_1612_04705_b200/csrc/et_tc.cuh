@@ -1,0 +1,529 @@
+// et_tc.cuh -- K-PERM-TC: the permutation sums of SURVEY 8(a) H5 on the sm_100a tensor cores (tcgen05, kind::i8).
+//
+// Identity: with label columns a_jc in {0,1} and
+//   Y_ic = sum_{j > i} Psi_ij a_jc,            Psi_ij = w_j psi_ij   (w = 1 when unweighted),
+// the three sums every column needs are row reductions of Y:
+//   Q_c = sum_{i<j} w_i w_j psi_ij a_ic a_jc           = sum_i a_ic w_i Y_ic
+//   R_c = sum_{i<j} w_i w_j psi_ij (a_ic + a_jc)       = sum_i real_i w_i Y_ic + sum_i a_ic w_i Y_i,ones
+//   S   = sum_{i<j} w_i w_j psi_ij                     = Q of the all-ones column
+// and S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q.  Y = Psi A is a GEMM whose left operand is
+// never stored: each CTA evaluates a 128 x 64 tile of psi in fp32 (packed FFMA2 + MUFU.EX2), quantises
+// Psi_ij = w_j psi_ij to a 15-bit fixed-point integer v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7)
+// into shared memory in the UMMA K-major SWIZZLE_64B layout and multiplies them by the label tile (bytes 128 a and a,
+// MN-major SWIZZLE_128B, expanded from the bit masks) with tcgen05.mma kind::i8 into ONE int32 accumulator per column in
+// TMEM.  Integer accumulation is exact, so S, R and Q are sums of the SAME quantised Psi whatever the schedule
+// (hard part 3 "consistency"), and the unweighted result is bit-reproducible.
+//
+// Columns of one launch (512): 0 = observed labelling, 1 = second labelling (P-even grouping of Sect. 5, else a copy
+// of column 0), 2 = all ones, 3.. = 509 permutations.
+#pragma once
+#include <type_traits>
+
+#include "et_kernels.cuh"
+
+namespace et {
+namespace tc {
+
+constexpr int kTM = 128;                 // rows (i) per row tile = UMMA M
+constexpr int kKB = 64;                  // j per K block
+constexpr int kCols = 512;               // label columns per launch (2 accumulators of N = 256)
+constexpr int kSpecial = 3;              // observed, second labelling, ones
+constexpr int kPermsPerChunk = kCols - kSpecial;
+constexpr int kWordsPerChunk = kCols / 32;
+constexpr int kProducerWarps = 8;
+constexpr int kProducers = kProducerWarps * 32;
+constexpr int kThreadsTC = kProducers + 32;  // + the MMA warp
+constexpr int kStages = 2;
+constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles
+constexpr int kBBytes = 2 * 2 * 2 * 8192;    // [q 2][digit 2][h 2][8 KB]
+constexpr int kUJStride = 80;                // bytes per j of the duplicated record (dim <= 8: 9 float2 = 72 -> 80)
+constexpr int kUJBytes = kKB * kUJStride;
+constexpr int kStageBytes = kABytes + kBBytes + kUJBytes;
+constexpr int kLutBytes = 2 * 256 * 8;
+constexpr int kSmemTC = kStages * kStageBytes + kLutBytes + 1024 /*alignment slack*/;
+// 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
+// complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
+// of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
+// tie bias in the block sums.
+constexpr float kMagic = 12582912.0f;
+constexpr int kMaxUnitKB = 512;               // K blocks per unit: |Y| <= 32767 * 64 * 512 < 2^31
+
+struct Unit {
+    int I;         // row tile
+    int kb_begin;  // first K block (64 j each), >= 2 I
+    int kb_end;
+    int pad;
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint64_t pack2(float a, float b)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+// round-toward-zero FMA: with the magic constant the sum is positive, so the low mantissa bits hold floor(a b) + 2
+__device__ __forceinline__ uint64_t fma2_rz(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t r;
+    asm("fma.rz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    }
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// UMMA shared-memory descriptor (sm_100): start >> 4, LBO >> 4 at bit 16, SBO >> 4 at bit 32, version 1 at bit 46,
+// layout type at bit 61 (2 = SWIZZLE_128B, 4 = SWIZZLE_64B).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr >> 4) & 0x3fff);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)layout << 61;
+    return d;
+}
+// kind::i8 instruction descriptor: D = s32, A u8/s8 K-major, B u8 MN-major, M = 128, N = 256.
+__host__ __device__ constexpr uint32_t umma_idesc_i8(bool a_signed)
+{
+    return (2u << 4) | ((a_signed ? 1u : 0u) << 7) | (0u << 10) | (0u << 15) | (1u << 16) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, "
+        "%20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr)
+{
+    uint32_t v;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    return v;
+}
+
+// Sum over the 32 lanes of x[b] for every b: lane L returns the total of element L (31 shuffles).
+template <typename T>
+__device__ __forceinline__ T lane_transpose_sum(T (&x)[32], int lane)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        const bool upper = (lane & s) != 0;
+#pragma unroll
+        for (int k = 0; k < s; ++k) {
+            const T send = upper ? x[k] : x[k + s];
+            const T keep = upper ? x[k + s] : x[k];
+            x[k] = keep + __shfl_xor_sync(0xffffffffu, send, s);
+        }
+    }
+    return x[0];
+}
+
+struct TCParams {
+    const float *rec;        // pooled records [npad][F]
+    const uint32_t *maskT;   // labels [npad][words_total], this launch uses words [word0, word0 + 16)
+    int words_total;
+    int word0;
+    const Unit *units;
+    int nunits;
+    float sc2;               // 2 * sc: Psi_ij = w_j psi_ij is quantised to v ~ sc Psi (15 bits)
+    uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
+    void *partial;           // [gridDim.x][8 warps][8 groups][32 lanes][2] of Acc
+};
+
+// One launch = 512 label columns.  Grid: persistent, one CTA per SM; unit u is processed by CTA u % gridDim.x.
+// WEIGHTED: accumulate w_i Y in double; else exact int64.
+template <int D, bool WEIGHTED>
+__global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
+{
+    using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
+    constexpr int F = rec_floats(D);
+    constexpr int NP = D + 1;               // float2 entries per j: -u_k duplicated, then s_j duplicated
+    constexpr int NLD = (NP + 1) / 2;       // LDS.128 per j
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t *lut = reinterpret_cast<uint64_t *>(smem + kStages * kStageBytes);
+    __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty;
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], kProducerWarps); mbar_init(&bar_empty[s], 1); }
+        mbar_init(&bar_accfull, 1);
+        mbar_init(&bar_accempty, kProducerWarps);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == kProducerWarps) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    // byte -> 8 bytes lookup tables: lut[x] byte k = bit k of x; lut[256 + x] = 128 * that
+    for (int x = tid; x < 256; x += kThreadsTC) {
+        uint64_t v = 0;
+        for (int k = 0; k < 8; ++k) v |= (uint64_t)((x >> k) & 1) << (8 * k);
+        lut[x] = v;
+        lut[256 + x] = v << 7;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_s;
+
+    if (warp == kProducerWarps) {
+        // =========================================================================== MMA issuer (one lane)
+        if (lane == 0) {
+            const uint32_t idesc_lo = umma_idesc_i8(false), idesc_hi = P.idesc_hi;
+            uint32_t it = 0, un = 0;
+            for (int u = blockIdx.x; u < P.nunits; u += gridDim.x, ++un) {
+                const Unit U = P.units[u];
+                mbar_wait(&bar_accempty, (un & 1) ^ 1);  // epilogue of the previous unit has drained TMEM
+                tc_fence_after();
+                for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+                    const int s = it & 1;
+                    mbar_wait(&bar_full[s], (it >> 1) & 1);
+                    tc_fence_after();
+                    const uint32_t a_base = smem_u32(smem + s * kStageBytes);
+                    const uint32_t b_base = a_base + kABytes;
+#pragma unroll
+                    for (int q = 0; q < 2; ++q)
+#pragma unroll
+                        for (int d = 0; d < 2; ++d)
+#pragma unroll
+                            for (int ks = 0; ks < 2; ++ks) {
+                                const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
+                                const uint64_t db = umma_desc(b_base + ((q * 2 + d) * 2) * 8192 + ks * 4 * 1024, 8192, 1024, 2);
+                                const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
+                                umma_i8(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
+                            }
+                    umma_commit(&bar_empty[s]);  // frees the stage when these MMAs have read it
+                }
+                umma_commit(&bar_accfull);
+            }
+        }
+    } else {
+        // =========================================================================== producers + epilogue
+        const int q_epi = warp >> 2;                 // column half read by this warp in the epilogue
+        const int lane_base = 32 * (warp & 3);       // TMEM lanes this warp may access
+        Acc accQ[8], accR[8];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) { accQ[g] = 0; accR[g] = 0; }
+        // dither constants: slot parity (t + lane) & 1 selects (k, 1 - k) for the two rows of a packed pair
+        const uint64_t magic2[2] = {pack2(kMagic + (float)(lane & 1), kMagic + (float)((lane & 1) ^ 1)),
+                                    pack2(kMagic + (float)((lane & 1) ^ 1), kMagic + (float)(lane & 1))};
+        uint32_t it = 0, un = 0;
+        for (int u = blockIdx.x; u < P.nunits; u += gridDim.x, ++un) {
+            const Unit U = P.units[u];
+            const long long row0 = (long long)U.I * kTM;
+            // this thread's four i rows: lane, lane + 32, lane + 64, lane + 96, packed as (r0, r1), (r2, r3)
+            uint64_t ui2[2][D];
+            {
+                float ur[4][D];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (row0 + lane + 32 * r) * F);
+                    float v[F];
+#pragma unroll
+                    for (int qq = 0; qq < F / 4; ++qq) {
+                        const float4 t = __ldg(p + qq);
+                        v[4 * qq] = t.x; v[4 * qq + 1] = t.y; v[4 * qq + 2] = t.z; v[4 * qq + 3] = t.w;
+                    }
+#pragma unroll
+                    for (int k = 0; k < D; ++k) ur[r][k] = v[k];
+                }
+#pragma unroll
+                for (int k = 0; k < D; ++k) { ui2[0][k] = pack2(ur[0][k], ur[1][k]); ui2[1][k] = pack2(ur[2][k], ur[3][k]); }
+            }
+            for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+                const int s = it & 1;
+                uint8_t *stA = smem + s * kStageBytes;
+                uint8_t *stB = stA + kABytes;
+                uint8_t *stU = stB + kBBytes;
+                const long long j0 = (long long)kb * kKB;
+                // loads for this K block: one record per loader thread, four mask words per thread
+                float rj[F];
+                if (tid < kKB) {
+                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + tid) * F);
+#pragma unroll
+                    for (int qq = 0; qq < F / 4; ++qq) {
+                        const float4 t = __ldg(p + qq);
+                        rj[4 * qq] = t.x; rj[4 * qq + 1] = t.y; rj[4 * qq + 2] = t.z; rj[4 * qq + 3] = t.w;
+                    }
+                }
+                const int jj = 8 * warp + (lane >> 2);  // j (local) of this thread's label tasks
+                uint32_t mw[4];
+                {
+                    const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + (lane & 3);
+#pragma unroll
+                    for (int G = 0; G < 4; ++G) mw[G] = __ldg(mp + 4 * G);
+                }
+                mbar_wait(&bar_empty[s], ((it >> 1) & 1) ^ 1);
+                if (tid < kKB) {
+                    uint64_t *o = reinterpret_cast<uint64_t *>(stU + tid * kUJStride);
+#pragma unroll
+                    for (int k = 0; k < D; ++k) o[k] = pack2(-rj[k], -rj[k]);
+                    const float sj = __fmul_rn(rj[D], P.sc2);
+                    o[D] = pack2(sj, sj);
+                    if (NP & 1) o[NP] = 0ull;
+                }
+                asm volatile("bar.sync 1, %0;" ::"n"(kProducers) : "memory");
+
+                // ---- psi tile: rows {lane + 32 r}, j = 8 warp .. 8 warp + 7 --------------------------------
+                const bool diag = j0 < row0 + kTM;  // K block overlaps the row tile: keep only j > i
+                uint32_t fq[4][8];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const ulonglong2 *up = reinterpret_cast<const ulonglong2 *>(stU + (8 * warp + t) * kUJStride);
+                    uint64_t nu[2 * NLD];
+#pragma unroll
+                    for (int qq = 0; qq < NLD; ++qq) {
+                        const ulonglong2 v = up[qq];
+                        nu[2 * qq] = v.x;
+                        nu[2 * qq + 1] = v.y;
+                    }
+#pragma unroll
+                    for (int pr = 0; pr < 2; ++pr) {
+                        uint64_t dd = add2(ui2[pr][0], nu[0]);
+                        uint64_t e = mul2(dd, dd);
+#pragma unroll
+                        for (int k = 1; k < D; ++k) {
+                            dd = add2(ui2[pr][k], nu[k]);
+                            e = fma2(dd, dd, e);
+                        }
+                        float e0, e1;
+                        unpack2(e, e0, e1);
+                        const uint64_t f2 = fma2(pack2(ex2_approx(-e0), ex2_approx(-e1)), nu[D], magic2[(t + pr) & 1]);
+                        float f0, f1;
+                        unpack2(f2, f0, f1);
+                        fq[2 * pr][t] = __float_as_uint(f0);
+                        fq[2 * pr + 1][t] = __float_as_uint(f1);
+                    }
+                }
+                if (diag) {
+                    const uint32_t zero = __float_as_uint(kMagic);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+#pragma unroll
+                        for (int t = 0; t < 8; ++t)
+                            if (j0 + 8 * warp + t <= row0 + lane + 32 * r) fq[r][t] = zero;
+                }
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int m = lane + 32 * r;
+                    const uint32_t p01 = __byte_perm(fq[r][0], fq[r][1], 0x5140), p23 = __byte_perm(fq[r][2], fq[r][3], 0x5140);
+                    const uint32_t p45 = __byte_perm(fq[r][4], fq[r][5], 0x5140), p67 = __byte_perm(fq[r][6], fq[r][7], 0x5140);
+                    uint2 lo, hi;
+                    lo.x = (__byte_perm(p01, p23, 0x5410) >> 1) & 0x7f7f7f7fu;
+                    lo.y = (__byte_perm(p45, p67, 0x5410) >> 1) & 0x7f7f7f7fu;
+                    hi.x = __byte_perm(p01, p23, 0x7632);
+                    hi.y = __byte_perm(p45, p67, 0x7632);
+                    const int off = (m >> 3) * 512 + (m & 7) * 64 + (((warp >> 1) ^ ((m >> 1) & 3)) << 4) + ((warp & 1) << 3);
+                    *reinterpret_cast<uint2 *>(stA + off) = hi;
+                    *reinterpret_cast<uint2 *>(stA + kTM * kKB + off) = lo;
+                }
+                // ---- label tile: j = jj, words 4 G + (lane & 3) -> 32 columns each, bytes a (lo) and 128 a (hi)
+                {
+                    const int g = warp, r = lane >> 2, c = 2 * (lane & 3);
+#pragma unroll
+                    for (int G = 0; G < 4; ++G) {
+                        const uint32_t m = mw[G];
+                        const uint64_t l0 = lut[m & 255u], l1 = lut[(m >> 8) & 255u], l2 = lut[(m >> 16) & 255u], l3 = lut[m >> 24];
+                        const int qh = G;  // q = G >> 1, h = G & 1
+                        uint8_t *bh = stB + (((qh >> 1) * 2 + 0) * 2 + (qh & 1)) * 8192 + g * 1024 + r * 128;
+                        uint8_t *bl = stB + (((qh >> 1) * 2 + 1) * 2 + (qh & 1)) * 8192 + g * 1024 + r * 128;
+                        const int o0 = ((c ^ r) << 4), o1 = (((c + 1) ^ r) << 4);
+                        *reinterpret_cast<ulonglong2 *>(bl + o0) = make_ulonglong2(l0, l1);
+                        *reinterpret_cast<ulonglong2 *>(bl + o1) = make_ulonglong2(l2, l3);
+                        *reinterpret_cast<ulonglong2 *>(bh + o0) = make_ulonglong2(l0 << 7, l1 << 7);
+                        *reinterpret_cast<ulonglong2 *>(bh + o1) = make_ulonglong2(l2 << 7, l3 << 7);
+                    }
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bar_full[s]);
+            }
+            // ---- epilogue of the unit -------------------------------------------------------------------
+            mbar_wait(&bar_accfull, un & 1);
+            tc_fence_after();
+            {
+                const long long row = row0 + lane_base + lane;
+                const uint32_t *mp = P.maskT + row * P.words_total + P.word0;
+                const uint32_t w0 = __ldg(mp);
+                const bool real = (w0 >> 2) & 1u;
+                const float wf = P.rec[row * F + D];
+                const uint32_t taddr = tmem + ((uint32_t)lane_base << 16);
+                const int yones = (int)tmem_ld1(taddr + 2);
+                Acc wi, zi;
+                if (WEIGHTED) { wi = (Acc)wf; zi = wi * (Acc)yones; }
+                else { wi = 1; zi = (Acc)yones; }
+#pragma unroll 1
+                for (int g = 0; g < 8; ++g) {
+                    const uint32_t mword = __ldg(mp + 8 * q_epi + g);
+                    uint32_t v[32];
+                    tmem_ld32(taddr + q_epi * 256 + 32 * g, v);
+                    Acc x[32];
+#pragma unroll
+                    for (int b = 0; b < 32; ++b) x[b] = ((mword >> b) & 1u) ? wi * (Acc)(int)v[b] : (Acc)0;
+                    const Acc qs = lane_transpose_sum(x, lane);
+#pragma unroll
+                    for (int b = 0; b < 32; ++b) x[b] = (real ? wi * (Acc)(int)v[b] : (Acc)0) + (((mword >> b) & 1u) ? zi : (Acc)0);
+                    const Acc rs = lane_transpose_sum(x, lane);
+                    // accQ / accR are indexed by a runtime g: keep them in registers with a switch-free select
+#pragma unroll
+                    for (int gg = 0; gg < 8; ++gg)
+                        if (gg == g) { accQ[gg] += qs; accR[gg] += rs; }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_accempty);
+        }
+        // per-warp partial column sums: partial[cta][warp][g][lane][2]
+        Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * 8 * 32 * 2;
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+            out[(g * 32 + lane) * 2] = accQ[g];
+            out[(g * 32 + lane) * 2 + 1] = accR[g];
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == kProducerWarps) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+}
+
+// Column sums over CTAs and warps, fixed order: column c = 256 q + 32 g + lane is held by warps 4 q .. 4 q + 3.
+// out[c] = {Q, R} as doubles in units of psi (divided by sc).
+template <bool WEIGHTED>
+__global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double *__restrict__ outQ, double *__restrict__ outR)
+{
+    using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= kCols) return;
+    const int q = c >> 8, g = (c >> 5) & 7, lane = c & 31;
+    const Acc *p = reinterpret_cast<const Acc *>(partial);
+    Acc sq = 0, sr = 0;
+    for (int b = 0; b < ncta; ++b)
+        for (int w = 4 * q; w < 4 * q + 4; ++w) {
+            const Acc *e = p + (((long long)b * kProducerWarps + w) * 8 * 32 + g * 32 + lane) * 2;
+            sq += e[0];
+            sr += e[1];
+        }
+    outQ[c] = (double)sq * inv_sc;
+    outR[c] = (double)sr * inv_sc;
+}
+
+// Label words of the TC layout: maskT[pos][chunk * 16 + W], column c = 32 W + b of chunk ch:
+// c = 0 observed (pooled index < n_x), c = 1 second labelling (class segment of i in `lab2_classes`), c = 2 ones,
+// c >= 3 permutation p = ch * 509 + c - 3 (local index; global p0 + p) if p < nperm.  grid = (events, chunks * 16).
+__global__ void __launch_bounds__(kThreads) k_label_write_tc(long long N, long long n_x, int nperm, long long p0, uint32_t seed_lo,
+                                                            uint32_t seed_hi, const SelState *__restrict__ st, LabelOut L,
+                                                            unsigned lab2_classes, int words_total, uint32_t *__restrict__ maskT)
+{
+    const long long i = blockIdx.x * (long long)kThreads + threadIdx.x;
+    const int ch = blockIdx.y / kWordsPerChunk, W = blockIdx.y % kWordsPerChunk;
+    if (i >= N) return;
+    long long pos = i;
+    int cls = 0;
+    for (int s = 0; s < L.nseg; ++s)
+        if (i >= L.seg_first[s] && i < L.seg_first[s + 1]) { pos = L.seg_pos[s] + (i - L.seg_first[s]); cls = s; }
+    uint32_t word = 0u;
+    uint64_t K[4];
+    long long have_p4 = -1;
+    for (int b = 0; b < 32; ++b) {
+        const int c = 32 * W + b;
+        if (c == 0) { if (i < n_x) word |= 1u; continue; }
+        if (c == 1) { if ((lab2_classes >> cls) & 1u) word |= 2u; continue; }
+        if (c == 2) { word |= 4u; continue; }
+        const int p = ch * kPermsPerChunk + c - kSpecial;
+        if (p >= nperm) break;
+        const long long pg = p0 + p;
+        if ((pg >> 2) != have_p4) { have_p4 = pg >> 2; label_keys4((uint32_t)i, (uint32_t)have_p4, seed_lo, seed_hi, K); }
+        if (K[pg & 3] <= st[p].prefix) word |= 1u << b;
+    }
+    maskT[pos * words_total + blockIdx.y] = word;
+}
+
+// W_c = sum_i a_ic w_i for every column of the TC layout.  grid = (row chunks, words_total); lane = bit.
+__global__ void __launch_bounds__(kThreads) k_perm_W_tc(const float *__restrict__ rec, int F, int dim, const uint32_t *__restrict__ maskT,
+                                                       int words_total, long long npad, int nchunk, double *__restrict__ partials)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wd = blockIdx.y;
+    const long long rows_per_chunk = (npad + nchunk - 1) / nchunk;
+    const long long r0 = blockIdx.x * rows_per_chunk, r1 = min(npad, r0 + rows_per_chunk);
+    double W = 0.0;
+    for (long long i = r0 + warp; i < r1; i += kThreads / 32) {
+        const uint32_t m = maskT[i * words_total + wd];
+        if (m >> lane & 1u) W += (double)rec[i * F + dim];
+    }
+    __shared__ double s[kThreads / 32][32];
+    s[warp][lane] = W;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < kThreads / 32; ++w) t += s[w][threadIdx.x];
+        partials[((long long)wd * nchunk + blockIdx.x) * 32 + threadIdx.x] = t;
+    }
+}
+
+}  // namespace tc
+}  // namespace et

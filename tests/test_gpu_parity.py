@@ -218,6 +218,87 @@ def test_perm_null_sample_is_compatible_with_zero(ctx):
     assert 0.005 < r.p_value < 0.995
 
 
+# ----------------------------------------------------------------------------- tensor-core permutation sums
+class force_kernel:
+    """ET_OPT_PERM_KERNEL: 1 = CUDA cores, 2 = tensor cores (tcgen05 kind::i8, 15-bit psi)."""
+
+    def __init__(self, ctx, which):
+        self.ctx, self.which = ctx, which
+
+    def __enter__(self):
+        self.ctx.set_option(binding.ET_OPT_PERM_KERNEL, self.which)
+
+    def __exit__(self, *exc):
+        self.ctx.set_option(binding.ET_OPT_PERM_KERNEL, 0)
+
+
+@pytest.mark.parametrize("n,nbar,dim,nperm", [(2000, 2000, 2, 50), (2100, 1900, 5, 70), (1500, 2600, 8, 33), (2048, 2048, 3, 600)])
+def test_perm_tc_matches_oracle(ctx, n, nbar, dim, nperm):
+    """K-PERM-TC (quantised psi, exact integer sums) against the from-scratch oracle; several units per row tile,
+    ragged padding, one and two 512-column chunks."""
+    rng = np.random.default_rng(n + dim)
+    x, xb = rng.uniform(size=(n, dim)), rng.uniform(size=(nbar, dim)) ** 1.15
+    sigma = 0.15 * math.sqrt(dim)
+    exp = oracle.perm_test(x, xb, sigma, nperm, 4242)
+    with force_kernel(ctx, 2):
+        got = ctx.permutation_test(x, xb, sigma, nperm, 4242)
+        assert ctx.stats().dominant_kernel == "k_perm_tc"
+    check_perm(got, exp)
+    with force_kernel(ctx, 1):
+        cc = ctx.permutation_test(x, xb, sigma, nperm, 4242)
+        assert ctx.stats().dominant_kernel in ("k_perm32", "k_pairs_rows")
+    assert np.abs(cc.T_perm - got.T_perm).max() <= TOL * exp.observed.term_scale
+
+
+def test_perm_tc_is_bit_reproducible(ctx):
+    """Integer accumulation: the unweighted tensor-core result does not depend on the schedule."""
+    s = dg.make_sample(dg.config(0))
+    with force_kernel(ctx, 2):
+        a = ctx.permutation_test(s.x, s.xbar, 0.3, 50, 7)
+        b = ctx.permutation_test(s.x, s.xbar, 0.3, 50, 7)
+    assert (a.T_perm == b.T_perm).all() and a.observed.T == b.observed.T
+
+
+def test_perm_tc_weighted(ctx):
+    c = dg.config(3, scale=0.012)  # 2400 + 2400 events, weights U[-0.5, 1.5]: signed hi digit
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
+    with force_kernel(ctx, 2):
+        got = ctx.permutation_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
+    check_perm(got, exp)
+    pos = np.abs(s.wx), np.abs(s.wxbar)  # non-negative weights: unsigned hi digit
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, 20, 3, *pos)
+    with force_kernel(ctx, 2):
+        got = ctx.permutation_test(s.x, s.xbar, 0.3, 20, 3, *pos)
+    check_perm(got, exp)
+
+
+def test_perm_tc_default_path_midsize(ctx):
+    """N = 40000 pooled (the default dispatch picks the tensor cores); 8 permutations from scratch in the oracle."""
+    c = dg.config(1, scale=0.2)
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, 8, c.perm_seed)
+    got = ctx.permutation_test(s.x, s.xbar, 0.3, 8, c.perm_seed)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    check_perm(got, exp)
+    assert abs(got.observed.T - ctx.T(s.x, s.xbar, 0.3).T) <= TOL * exp.observed.term_scale
+
+
+def test_podd_tc_parity(ctx):
+    c = dg.config(4, scale=0.003)  # 3000 + 3000 events
+    s = dg.make_sample(c)
+    nperm = 40
+    with force_kernel(ctx, 2):
+        got = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, nperm, c.perm_seed)
+    posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
+    posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
+    I, II, III, IV = s.x[posx == 1], s.x[posx == 0], s.xbar[posb == 1], s.xbar[posb == 0]
+    assert got.count == (len(I), len(II), len(III), len(IV))
+    exp = oracle.perm_test(np.vstack([I, IV]), np.vstack([II, III]), c.sigma, nperm, c.perm_seed)
+    check_perm(got.p_odd, exp)
+    assert_T_close(got.p_even, oracle.T(s.x, s.xbar, c.sigma))
+
+
 # ----------------------------------------------------------------------------- Sect. 5
 def test_podd_split_bit_exact(ctx):
     c = dg.config(4, scale=0.02)
