@@ -37,10 +37,10 @@ constexpr int kStages = 2;
 constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles
 constexpr int kBBytes = 2 * 2 * 2 * 8192;    // [q 2][digit 2][h 2][8 KB]
 constexpr int kUJStride = 80;                // bytes per j of the duplicated record (dim <= 8: 9 float2 = 72 -> 80)
-constexpr int kUJBytes = kKB * kUJStride;
-constexpr int kStageBytes = kABytes + kBBytes + kUJBytes;
+constexpr int kUJBytes = kKB * kUJStride;     // one private 8-record region per producer warp
+constexpr int kStageBytes = kABytes + kBBytes;
 constexpr int kLutBytes = 2 * 256 * 8;
-constexpr int kSmemTC = kStages * kStageBytes + kLutBytes + 1024 /*alignment slack*/;
+constexpr int kSmemTC = kStages * kStageBytes + kLutBytes + kUJBytes + 1024 /*alignment slack*/;
 // 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
 // complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
 // of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
@@ -199,9 +199,11 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
     constexpr int F = rec_floats(D);
     constexpr int NP = D + 1;               // float2 entries per j: -u_k duplicated, then s_j duplicated
     constexpr int NLD = (NP + 1) / 2;       // LDS.128 per j
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
+    uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t *lut = reinterpret_cast<uint64_t *>(smem + kStages * kStageBytes);
+    uint8_t *ujw = smem + kStages * kStageBytes + kLutBytes;  // per-warp j records [8 warps][8 j][kUJStride]
     __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty;
     __shared__ uint32_t tmem_base_s;
 
@@ -267,15 +269,17 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
         Acc accQ[8], accR[8];
 #pragma unroll
         for (int g = 0; g < 8; ++g) { accQ[g] = 0; accR[g] = 0; }
-        // dither constants: slot parity (t + lane) & 1 selects (k, 1 - k) for the two rows of a packed pair
-        const uint64_t magic2[2] = {pack2(kMagic + (float)(lane & 1), kMagic + (float)((lane & 1) ^ 1)),
-                                    pack2(kMagic + (float)((lane & 1) ^ 1), kMagic + (float)(lane & 1))};
+        // dither constants: slot parity (t + pr + lane) & 1 selects (k, 1 - k) for the two rows of a packed pair
+        const float2 magic2[2] = {make_float2(kMagic + (float)(lane & 1), kMagic + (float)((lane & 1) ^ 1)),
+                                  make_float2(kMagic + (float)((lane & 1) ^ 1), kMagic + (float)(lane & 1))};
+        uint8_t *uj_mine = ujw + warp * (8 * kUJStride);
+        const int jj = 8 * warp + (lane >> 2);  // j (local) of this thread's label tasks; lanes 0..7 load record 8 warp + lane
         uint32_t it = 0, un = 0;
         for (int u = blockIdx.x; u < P.nunits; u += gridDim.x, ++un) {
             const Unit U = P.units[u];
             const long long row0 = (long long)U.I * kTM;
             // this thread's four i rows: lane, lane + 32, lane + 64, lane + 96, packed as (r0, r1), (r2, r3)
-            uint64_t ui2[2][D];
+            float2 ui2[2][D];
             {
                 float ur[4][D];
 #pragma unroll
@@ -291,71 +295,78 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                     for (int k = 0; k < D; ++k) ur[r][k] = v[k];
                 }
 #pragma unroll
-                for (int k = 0; k < D; ++k) { ui2[0][k] = pack2(ur[0][k], ur[1][k]); ui2[1][k] = pack2(ur[2][k], ur[3][k]); }
+                for (int k = 0; k < D; ++k) {
+                    // "+ 0" materialises each pair in an aligned register pair once per unit (ptxas otherwise re-forms the
+                    // pairs from the scalar load registers with two moves at every use inside the K-block loop)
+                    ui2[0][k] = __fadd2_rn(make_float2(ur[0][k], ur[1][k]), make_float2(0.f, 0.f));
+                    ui2[1][k] = __fadd2_rn(make_float2(ur[2][k], ur[3][k]), make_float2(0.f, 0.f));
+                }
             }
+            // loads of K block kb: lanes 0..7 one record each, every lane four label words; prefetched one block ahead
+            float4 rj[F / 4];
+            uint32_t mw[4];
+            auto load_block = [&](int kb) {
+                const long long j0 = (long long)kb * kKB;
+                if (lane < 8) {
+                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + 8 * warp + lane) * F);
+#pragma unroll
+                    for (int qq = 0; qq < F / 4; ++qq) rj[qq] = __ldg(p + qq);
+                }
+                const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + (lane & 3);
+#pragma unroll
+                for (int G = 0; G < 4; ++G) mw[G] = __ldg(mp + 4 * G);
+            };
+            load_block(U.kb_begin);
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
                 const int s = it & 1;
                 uint8_t *stA = smem + s * kStageBytes;
                 uint8_t *stB = stA + kABytes;
-                uint8_t *stU = stB + kBBytes;
                 const long long j0 = (long long)kb * kKB;
-                // loads for this K block: one record per loader thread, four mask words per thread
-                float rj[F];
-                if (tid < kKB) {
-                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + tid) * F);
+                // this warp's eight j records -> shared (negated, duplicated for the packed FP32 pipe)
+                __syncwarp();
+                if (lane < 8) {
+                    float v[F];
 #pragma unroll
-                    for (int qq = 0; qq < F / 4; ++qq) {
-                        const float4 t = __ldg(p + qq);
-                        rj[4 * qq] = t.x; rj[4 * qq + 1] = t.y; rj[4 * qq + 2] = t.z; rj[4 * qq + 3] = t.w;
-                    }
-                }
-                const int jj = 8 * warp + (lane >> 2);  // j (local) of this thread's label tasks
-                uint32_t mw[4];
-                {
-                    const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + (lane & 3);
+                    for (int qq = 0; qq < F / 4; ++qq) { v[4 * qq] = rj[qq].x; v[4 * qq + 1] = rj[qq].y; v[4 * qq + 2] = rj[qq].z; v[4 * qq + 3] = rj[qq].w; }
+                    float2 *o = reinterpret_cast<float2 *>(uj_mine + lane * kUJStride);
 #pragma unroll
-                    for (int G = 0; G < 4; ++G) mw[G] = __ldg(mp + 4 * G);
+                    for (int k = 0; k < D; ++k) o[k] = make_float2(-v[k], -v[k]);
+                    const float sj = __fmul_rn(v[D], P.sc2);
+                    o[D] = make_float2(sj, sj);
+                    if (NP & 1) o[NP] = make_float2(0.f, 0.f);
                 }
+                uint32_t mcur[4];
+#pragma unroll
+                for (int G = 0; G < 4; ++G) mcur[G] = mw[G];
+                __syncwarp();
+                if (kb + 1 < U.kb_end) load_block(kb + 1);
                 mbar_wait(&bar_empty[s], ((it >> 1) & 1) ^ 1);
-                if (tid < kKB) {
-                    uint64_t *o = reinterpret_cast<uint64_t *>(stU + tid * kUJStride);
-#pragma unroll
-                    for (int k = 0; k < D; ++k) o[k] = pack2(-rj[k], -rj[k]);
-                    const float sj = __fmul_rn(rj[D], P.sc2);
-                    o[D] = pack2(sj, sj);
-                    if (NP & 1) o[NP] = 0ull;
-                }
-                asm volatile("bar.sync 1, %0;" ::"n"(kProducers) : "memory");
 
                 // ---- psi tile: rows {lane + 32 r}, j = 8 warp .. 8 warp + 7 --------------------------------
                 const bool diag = j0 < row0 + kTM;  // K block overlaps the row tile: keep only j > i
                 uint32_t fq[4][8];
 #pragma unroll
                 for (int t = 0; t < 8; ++t) {
-                    const ulonglong2 *up = reinterpret_cast<const ulonglong2 *>(stU + (8 * warp + t) * kUJStride);
-                    uint64_t nu[2 * NLD];
+                    const float4 *up = reinterpret_cast<const float4 *>(uj_mine + t * kUJStride);
+                    float2 nu[2 * NLD];
 #pragma unroll
                     for (int qq = 0; qq < NLD; ++qq) {
-                        const ulonglong2 v = up[qq];
-                        nu[2 * qq] = v.x;
-                        nu[2 * qq + 1] = v.y;
+                        const float4 v = up[qq];
+                        nu[2 * qq] = make_float2(v.x, v.y);
+                        nu[2 * qq + 1] = make_float2(v.z, v.w);
                     }
 #pragma unroll
                     for (int pr = 0; pr < 2; ++pr) {
-                        uint64_t dd = add2(ui2[pr][0], nu[0]);
-                        uint64_t e = mul2(dd, dd);
+                        float2 dd = __fadd2_rn(ui2[pr][0], nu[0]);
+                        float2 e = __fmul2_rn(dd, dd);
 #pragma unroll
                         for (int k = 1; k < D; ++k) {
-                            dd = add2(ui2[pr][k], nu[k]);
-                            e = fma2(dd, dd, e);
+                            dd = __fadd2_rn(ui2[pr][k], nu[k]);
+                            e = __ffma2_rn(dd, dd, e);
                         }
-                        float e0, e1;
-                        unpack2(e, e0, e1);
-                        const uint64_t f2 = fma2(pack2(ex2_approx(-e0), ex2_approx(-e1)), nu[D], magic2[(t + pr) & 1]);
-                        float f0, f1;
-                        unpack2(f2, f0, f1);
-                        fq[2 * pr][t] = __float_as_uint(f0);
-                        fq[2 * pr + 1][t] = __float_as_uint(f1);
+                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magic2[(t + pr) & 1]);
+                        fq[2 * pr][t] = __float_as_uint(f2.x);
+                        fq[2 * pr + 1][t] = __float_as_uint(f2.y);
                     }
                 }
                 if (diag) {
@@ -382,19 +393,19 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                 }
                 // ---- label tile: j = jj, words 4 G + (lane & 3) -> 32 columns each, bytes a (lo) and 128 a (hi)
                 {
-                    const int g = warp, r = lane >> 2, c = 2 * (lane & 3);
+                    const int r = lane >> 2, c = 2 * (lane & 3);
+                    const int o0 = warp * 1024 + r * 128 + ((c ^ r) << 4), o1 = warp * 1024 + r * 128 + (((c + 1) ^ r) << 4);
 #pragma unroll
                     for (int G = 0; G < 4; ++G) {
-                        const uint32_t m = mw[G];
-                        const uint64_t l0 = lut[m & 255u], l1 = lut[(m >> 8) & 255u], l2 = lut[(m >> 16) & 255u], l3 = lut[m >> 24];
-                        const int qh = G;  // q = G >> 1, h = G & 1
-                        uint8_t *bh = stB + (((qh >> 1) * 2 + 0) * 2 + (qh & 1)) * 8192 + g * 1024 + r * 128;
-                        uint8_t *bl = stB + (((qh >> 1) * 2 + 1) * 2 + (qh & 1)) * 8192 + g * 1024 + r * 128;
-                        const int o0 = ((c ^ r) << 4), o1 = (((c + 1) ^ r) << 4);
-                        *reinterpret_cast<ulonglong2 *>(bl + o0) = make_ulonglong2(l0, l1);
-                        *reinterpret_cast<ulonglong2 *>(bl + o1) = make_ulonglong2(l2, l3);
-                        *reinterpret_cast<ulonglong2 *>(bh + o0) = make_ulonglong2(l0 << 7, l1 << 7);
-                        *reinterpret_cast<ulonglong2 *>(bh + o1) = make_ulonglong2(l2 << 7, l3 << 7);
+                        const uint32_t m = mcur[G];
+                        const uint2 l0 = *reinterpret_cast<const uint2 *>(&lut[m & 255u]), l1 = *reinterpret_cast<const uint2 *>(&lut[(m >> 8) & 255u]);
+                        const uint2 l2 = *reinterpret_cast<const uint2 *>(&lut[(m >> 16) & 255u]), l3 = *reinterpret_cast<const uint2 *>(&lut[m >> 24]);
+                        uint8_t *bh = stB + (((G >> 1) * 2 + 0) * 2 + (G & 1)) * 8192;  // q = G >> 1, digit, h = G & 1
+                        uint8_t *bl = stB + (((G >> 1) * 2 + 1) * 2 + (G & 1)) * 8192;
+                        *reinterpret_cast<uint4 *>(bl + o0) = make_uint4(l0.x, l0.y, l1.x, l1.y);
+                        *reinterpret_cast<uint4 *>(bl + o1) = make_uint4(l2.x, l2.y, l3.x, l3.y);
+                        *reinterpret_cast<uint4 *>(bh + o0) = make_uint4(l0.x << 7, l0.y << 7, l1.x << 7, l1.y << 7);
+                        *reinterpret_cast<uint4 *>(bh + o1) = make_uint4(l2.x << 7, l2.y << 7, l3.x << 7, l3.y << 7);
                     }
                 }
                 fence_async_smem();
@@ -427,7 +438,6 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
 #pragma unroll
                     for (int b = 0; b < 32; ++b) x[b] = (real ? wi * (Acc)(int)v[b] : (Acc)0) + (((mword >> b) & 1u) ? zi : (Acc)0);
                     const Acc rs = lane_transpose_sum(x, lane);
-                    // accQ / accR are indexed by a runtime g: keep them in registers with a switch-free select
 #pragma unroll
                     for (int gg = 0; gg < 8; ++gg)
                         if (gg == g) { accQ[gg] += qs; accR[gg] += rs; }
