@@ -152,15 +152,22 @@ __device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int 
 
 // K-T: class-pair block sums S[c1][c2] = sum over unordered pairs of w_i w_j psi_ij (Eq. 2's three sums, or the ten
 // of the four-class split), over the upper triangle of i-tiles.  Work unit = (I, J), I <= J, tiles of 256*R rows;
-// fp32 per pair and per 256-j partial row sum, fp64 from there on; per-unit block reduction in a fixed order, so the
+// fp32 per pair and per 128-j partial row sum, fp64 from there on; per-unit block reduction in a fixed order, so the
 // result depends only on the grid size.
+// Packed FP32 pipe, two j per instruction: the j records are staged in shared memory as PAIRS, float2 k of pair p =
+// (-u_{2p,k}, -u_{2p+1,k}), float2 D = (w_2p, w_2p+1), and every thread keeps its R i rows duplicated, (u_ik, u_ik), so that one FADD2 / FFMA2 does the
+// subtraction / square-accumulate of (i, 2p) and (i, 2p+1) at once.  Each half of a packed instruction rounds like the
+// scalar one (u_i + (-u_j) == u_i - u_j exactly), so psi is bit-identical to psi_pair<D>.  The packed instructions
+// halve the issue slots per pair (2D+1 FP32 lane-ops and one MUFU.EX2 per pair stay): measured 2.3 -> 2.8e12 pairs/s
+// at D = 5 (profiles/r01_pipe_probes.md).
 template <int D, int R>
 __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ rec, int nT,
                                                      const uint8_t *__restrict__ tile_cls, long long nunits,
                                                      double *__restrict__ partials)
 {
     constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
-    __shared__ float4 sj[kTileJ * F4];
+    constexpr int NP = D + 1, NLD = (NP + 1) / 2;  // float2 entries / LDS.128 per j pair
+    __shared__ float4 sj[kTileJ / 2 * NLD];
     __shared__ double s_sum[kSumSlots];
     __shared__ double s_warp[kThreads / 32];
     const int tid = threadIdx.x;
@@ -169,7 +176,8 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
     for (long long unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
         int I, J;
         unit_to_pair(unit, nT, I, J);
-        float ui[R][D], wi[R];
+        float2 ui[R][D];
+        float wi[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
@@ -179,8 +187,9 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
                 const float4 t = __ldg(p + q);
                 v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
             }
+            // "+ 0" materialises the duplicated pair in an aligned register pair once per unit
 #pragma unroll
-            for (int k = 0; k < D; ++k) ui[r][k] = v[k];
+            for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             wi[r] = v[D];
         }
         double racc[R];
@@ -191,21 +200,45 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
             __syncthreads();
             {
                 const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)J * TI + sub * kTileJ + tid) * F);
+                float v[F];
 #pragma unroll
-                for (int q = 0; q < F4; ++q) sj[tid * F4 + q] = __ldg(p + q);
+                for (int q = 0; q < F4; ++q) {
+                    const float4 t = __ldg(p + q);
+                    v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+                }
+                float *o = reinterpret_cast<float *>(sj) + (tid >> 1) * (NLD * 4) + (tid & 1);
+#pragma unroll
+                for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
+                o[2 * D] = v[D];
+                if (NP & 1) o[2 * NP] = 0.f;
             }
             __syncthreads();
-            float acc[R];
+            float2 acc[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+            for (int r = 0; r < R; ++r) acc[r] = make_float2(0.f, 0.f);
 #pragma unroll 4
-            for (int j = 0; j < kTileJ; ++j) {
-                const JRec<D> rj = load_jrec<D>(sj, j);
+            for (int jp = 0; jp < kTileJ / 2; ++jp) {
+                float2 nu[2 * NLD];
 #pragma unroll
-                for (int r = 0; r < R; ++r) acc[r] = __fmaf_rn(psi_pair<D>(ui[r], rj.u), rj.w, acc[r]);
+                for (int q = 0; q < NLD; ++q) {
+                    const float4 t = sj[jp * NLD + q];
+                    nu[2 * q] = make_float2(t.x, t.y);
+                    nu[2 * q + 1] = make_float2(t.z, t.w);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    float2 d = __fadd2_rn(ui[r][0], nu[0]);
+                    float2 e = __fmul2_rn(d, d);
+#pragma unroll
+                    for (int k = 1; k < D; ++k) {
+                        d = __fadd2_rn(ui[r][k], nu[k]);
+                        e = __ffma2_rn(d, d, e);
+                    }
+                    acc[r] = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], acc[r]);
+                }
             }
 #pragma unroll
-            for (int r = 0; r < R; ++r) racc[r] += (double)acc[r];
+            for (int r = 0; r < R; ++r) racc[r] += (double)acc[r].x + (double)acc[r].y;
         }
         double t = 0.0;
         const bool diag = I == J;
