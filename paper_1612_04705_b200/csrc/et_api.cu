@@ -752,16 +752,18 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     }
     ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
 
-    // unit table: row tile I against K blocks [2 I, NK) in pieces of <= Lmax, longest first, unit u -> CTA u % grid
-    const int nT = (int)(L.npad / tc::kTM), NK = (int)(L.npad / tc::kKB);
+    // unit table: 256-row tile I (one CTA pair) against K blocks [4 I, NK) in pieces of <= Lmax, longest first,
+    // unit u -> cluster u % nclusters
+    const int nclusters_max = ctx->num_sms / 2;
+    const int nT = (int)(L.npad / tc::kTM2), NK = (int)(L.npad / tc::kKB);
     long long total_kb = 0;
-    for (int I = 0; I < nT; ++I) total_kb += NK - 2 * I;
-    long long Lmax = (total_kb + (long long)ctx->num_sms * 24 - 1) / ((long long)ctx->num_sms * 24);
+    for (int I = 0; I < nT; ++I) total_kb += NK - 4 * I;
+    long long Lmax = (total_kb + (long long)nclusters_max * 24 - 1) / ((long long)nclusters_max * 24);
     if (Lmax < 8) Lmax = 8;
     if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
     std::vector<tc::Unit> full, tail;
     for (int I = 0; I < nT; ++I)
-        for (int kb = 2 * I; kb < NK; kb += (int)Lmax) {
+        for (int kb = 4 * I; kb < NK; kb += (int)Lmax) {
             tc::Unit u{I, kb, (int)std::min<long long>(NK, kb + Lmax), 0};
             (u.kb_end - u.kb_begin == Lmax ? full : tail).push_back(u);
         }
@@ -779,7 +781,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     else if (ctx->wmin >= 0.0) sc = 32767.0 / std::max(ctx->wmax, 1e-30);
     else { hi_signed = true; sc = 16383.0 / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
 
-    const int grid = std::min(ctx->num_sms, nunits);
+    const int grid = 2 * std::min(nclusters_max, nunits);  // CTA pairs
     const size_t part_bytes = (size_t)grid * tc::kProducerWarps * 8 * 32 * 2 * 8;
     ET_TRY(ensure(ctx, ctx->tcpart, part_bytes));
     ET_TRY(ensure(ctx, ctx->tcQ, (size_t)nchunks * tc::kCols * sizeof(double)));
@@ -810,7 +812,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     {
         const long long pairs = L.N * (L.N - 1) / 2;
         ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * tc::kCols * nchunks));
-        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM * tc::kKB;
+        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM2 * tc::kKB;
     }
 
     // W_c

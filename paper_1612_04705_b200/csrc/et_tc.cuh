@@ -7,15 +7,20 @@
 //   R_c = sum_{i<j} w_i w_j psi_ij (a_ic + a_jc)       = sum_i real_i w_i Y_ic + sum_i a_ic w_i Y_i,ones
 //   S   = sum_{i<j} w_i w_j psi_ij                     = Q of the all-ones column
 // and S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q.  Y = Psi A is a GEMM whose left operand is
-// never stored: each CTA evaluates a 128 x 64 tile of psi in fp32 (packed FFMA2 + MUFU.EX2), quantises
-// Psi_ij = w_j psi_ij to a 15-bit fixed-point integer v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7)
-// into shared memory in the UMMA K-major SWIZZLE_64B layout and multiplies them by the label tile (bytes 128 a and a,
-// MN-major SWIZZLE_128B, expanded from the bit masks) with tcgen05.mma kind::i8 into ONE int32 accumulator per column in
-// TMEM.  Integer accumulation is exact, so S, R and Q are sums of the SAME quantised Psi whatever the schedule
+// never stored.  A cluster of two CTAs (one SM pair) works on a 256-row tile; per block of 64 j each CTA evaluates its
+// 128 x 64 tile of psi in fp32 (packed FFMA2 + MUFU.EX2), quantises Psi_ij = w_j psi_ij to a 15-bit fixed-point integer
+// v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7) into its shared memory in the UMMA K-major SWIZZLE_64B
+// layout, and expands ITS HALF of the label columns from the bit masks into the B tile (bytes 128 a and a, MN-major
+// SWIZZLE_128B).  One thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M = 256, N = 256, K = 32):
+// the pair's tensor cores read A from their own SM and each half of B from one SM of the pair, so a label byte is
+// written and read once per 256 rows instead of once per 128 (the kernel is bound by shared-memory bandwidth, not by
+// the tensor pipe: profiles/r01a_README.md).  Accumulation is ONE int32 per column in TMEM (all 512 columns of each
+// SM).  Integer accumulation is exact, so S, R and Q are sums of the SAME quantised Psi whatever the schedule
 // (hard part 3 "consistency"), and the unweighted result is bit-reproducible.
 //
 // Columns of one launch (512): 0 = observed labelling, 1 = second labelling (P-even grouping of Sect. 5, else a copy
-// of column 0), 2 = all ones, 3.. = 509 permutations.
+// of column 0), 2 = all ones, 3.. = 509 permutations.  Inside a 32-column mask word the B tile / TMEM column p holds
+// label bit beta(p) = (p >> 2) + 8 (p & 3), so that four label bytes come out of one shift and one mask.
 #pragma once
 #include <type_traits>
 
@@ -24,7 +29,8 @@
 namespace et {
 namespace tc {
 
-constexpr int kTM = 128;                 // rows (i) per row tile = UMMA M
+constexpr int kTM = 128;                 // rows (i) per CTA = UMMA M / 2
+constexpr int kTM2 = 2 * kTM;            // rows per cluster (work unit)
 constexpr int kKB = 64;                  // j per K block
 constexpr int kCols = 512;               // label columns per launch (2 accumulators of N = 256)
 constexpr int kSpecial = 3;              // observed, second labelling, ones
@@ -33,14 +39,13 @@ constexpr int kWordsPerChunk = kCols / 32;
 constexpr int kProducerWarps = 8;
 constexpr int kProducers = kProducerWarps * 32;
 constexpr int kThreadsTC = kProducers + 32;  // + the MMA warp
-constexpr int kStages = 2;
-constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles
-constexpr int kBBytes = 2 * 2 * 2 * 8192;    // [q 2][digit 2][h 2][8 KB]
-constexpr int kUJStride = 80;                // bytes per j of the duplicated record (dim <= 8: 9 float2 = 72 -> 80)
-constexpr int kUJBytes = kKB * kUJStride;     // one private 8-record region per producer warp
+constexpr int kStages = 4;
+constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (16 KB)
+constexpr int kBBytes = 2 * 2 * 8192;        // this CTA's half of B: [q 2][digit 2][64 j x 128 columns] (32 KB)
 constexpr int kStageBytes = kABytes + kBBytes;
-constexpr int kLutBytes = 2 * 256 * 8;
-constexpr int kSmemTC = kStages * kStageBytes + kLutBytes + kUJBytes + 1024 /*alignment slack*/;
+constexpr int kUJWarpBytes = 8 * 80;         // per producer warp: 8 j pairs x (dim + 1 <= 9 float2 -> 5 float4)
+constexpr int kUJBytes = kProducerWarps * kUJWarpBytes;
+constexpr int kSmemTC = kStages * kStageBytes + kUJBytes + 1024 /*alignment slack*/;
 // 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
 // complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
 // of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
@@ -48,9 +53,12 @@ constexpr int kSmemTC = kStages * kStageBytes + kLutBytes + kUJBytes + 1024 /*al
 constexpr float kMagic = 12582912.0f;
 constexpr int kMaxUnitKB = 512;               // K blocks per unit: |Y| <= 32767 * 64 * 512 < 2^31
 
+// label bit held by byte / TMEM column p of a 32-column word
+__host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
+
 struct Unit {
-    int I;         // row tile
-    int kb_begin;  // first K block (64 j each), >= 2 I
+    int I;         // 256-row tile
+    int kb_begin;  // first K block (64 j each), >= 4 I
     int kb_end;
     int pad;
 };
@@ -112,6 +120,58 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// ---- cluster (CTA pair) forms ------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of `local` (a shared::cta address) in the CTA of rank `rank`
+__device__ __forceinline__ uint32_t mapa_rank(uint32_t local, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr)
+{
+    // default semantics (release at CTA scope), as the CUTLASS cluster barriers use: the data the peer's MMAs read was
+    // published to the async proxy by this thread's fence.proxy.async; a .release.cluster here costs a MEMBAR.GPU +
+    // L1 invalidate per arrive (profiles/r01b)
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    }
+}
+// arrives (count 1) on the barrier at this shared-memory offset in BOTH CTAs of the pair once all prior MMAs are done
+__device__ __forceinline__ void umma_commit_pair(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+                 "h"((uint16_t)3)
+                 : "memory");
+}
+__device__ __forceinline__ void umma_i8_pair(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -128,10 +188,10 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes
     d |= (uint64_t)layout << 61;
     return d;
 }
-// kind::i8 instruction descriptor: D = s32, A u8/s8 K-major, B u8 MN-major, M = 128, N = 256.
+// kind::i8 instruction descriptor: D = s32, A u8/s8 K-major, B u8 MN-major, M = 256 (the CTA pair), N = 256.
 __host__ __device__ constexpr uint32_t umma_idesc_i8(bool a_signed)
 {
-    return (2u << 4) | ((a_signed ? 1u : 0u) << 7) | (0u << 10) | (0u << 15) | (1u << 16) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
+    return (2u << 4) | ((a_signed ? 1u : 0u) << 7) | (0u << 10) | (0u << 15) | (1u << 16) | ((256u >> 3) << 17) | ((256u >> 4) << 24);
 }
 __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate)
 {
@@ -190,59 +250,58 @@ struct TCParams {
     void *partial;           // [gridDim.x][8 warps][8 groups][32 lanes][2] of Acc
 };
 
-// One launch = 512 label columns.  Grid: persistent, one CTA per SM; unit u is processed by CTA u % gridDim.x.
+// One launch = 512 label columns.  Grid: persistent, one CTA per SM, clusters of 2 (an SM pair); unit u is processed
+// by cluster u % (gridDim.x / 2).  CTA rank r of the pair owns rows 256 I + 128 r .. + 127 (its psi tile, its half of
+// the accumulator rows in its own TMEM) and the label columns [256 q + 128 r, 256 q + 128 r + 128), q = 0, 1.
 // WEIGHTED: accumulate w_i Y in double; else exact int64.
 template <int D, bool WEIGHTED>
-__global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
     constexpr int F = rec_floats(D);
-    constexpr int NP = D + 1;               // float2 entries per j: -u_k duplicated, then s_j duplicated
-    constexpr int NLD = (NP + 1) / 2;       // LDS.128 per j
+    constexpr int NP = D + 1;               // float2 entries per j pair: (-u_j0k, -u_j1k), then (s_j0, s_j1)
+    constexpr int NLD = (NP + 1) / 2;       // LDS.128 per j pair
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    uint64_t *lut = reinterpret_cast<uint64_t *>(smem + kStages * kStageBytes);
-    uint8_t *ujw = smem + kStages * kStageBytes + kLutBytes;  // per-warp j records [8 warps][8 j][kUJStride]
+    uint8_t *ujw = smem + kStages * kStageBytes;  // per-warp j-pair records
     __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty;
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster_id = blockIdx.x >> 1, nclusters = gridDim.x >> 1;
 
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], kProducerWarps); mbar_init(&bar_empty[s], 1); }
+        // full / accempty are used in the leader only (arrivals from the producer warps of BOTH CTAs);
+        // empty / accfull receive one multicast tcgen05.commit arrival in each CTA
+        for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], 2 * kProducerWarps); mbar_init(&bar_empty[s], 1); }
         mbar_init(&bar_accfull, 1);
-        mbar_init(&bar_accempty, kProducerWarps);
+        mbar_init(&bar_accempty, 2 * kProducerWarps);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == kProducerWarps) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    // byte -> 8 bytes lookup tables: lut[x] byte k = bit k of x; lut[256 + x] = 128 * that
-    for (int x = tid; x < 256; x += kThreadsTC) {
-        uint64_t v = 0;
-        for (int k = 0; k < 8; ++k) v |= (uint64_t)((x >> k) & 1) << (8 * k);
-        lut[x] = v;
-        lut[256 + x] = v << 7;
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
     }
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();  // barrier inits of the peer are visible before any remote arrive
     tc_fence_after();
     const uint32_t tmem = tmem_base_s;
 
     if (warp == kProducerWarps) {
-        // =========================================================================== MMA issuer (one lane)
-        if (lane == 0) {
+        // =========================================================================== MMA issuer (leader CTA, one lane)
+        if (rank == 0 && lane == 0) {
             const uint32_t idesc_lo = umma_idesc_i8(false), idesc_hi = P.idesc_hi;
             uint32_t it = 0, un = 0;
-            for (int u = blockIdx.x; u < P.nunits; u += gridDim.x, ++un) {
+            for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
                 const Unit U = P.units[u];
-                mbar_wait(&bar_accempty, (un & 1) ^ 1);  // epilogue of the previous unit has drained TMEM
+                mbar_wait_cluster(&bar_accempty, (un & 1) ^ 1);  // both epilogues of the previous unit have drained TMEM
                 tc_fence_after();
                 for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                    const int s = it & 1;
-                    mbar_wait(&bar_full[s], (it >> 1) & 1);
+                    const int s = it % kStages;
+                    mbar_wait_cluster(&bar_full[s], (it / kStages) & 1);
                     tc_fence_after();
                     const uint32_t a_base = smem_u32(smem + s * kStageBytes);
                     const uint32_t b_base = a_base + kABytes;
@@ -253,101 +312,96 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
 #pragma unroll
                             for (int ks = 0; ks < 2; ++ks) {
                                 const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
-                                const uint64_t db = umma_desc(b_base + ((q * 2 + d) * 2) * 8192 + ks * 4 * 1024, 8192, 1024, 2);
+                                const uint64_t db = umma_desc(b_base + (q * 2 + d) * 8192 + ks * 4 * 1024, 8192, 1024, 2);
                                 const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
-                                umma_i8(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
+                                umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
                             }
-                    umma_commit(&bar_empty[s]);  // frees the stage when these MMAs have read it
+                    umma_commit_pair(&bar_empty[s]);  // frees the stage in both CTAs when these MMAs have read it
                 }
-                umma_commit(&bar_accfull);
+                umma_commit_pair(&bar_accfull);
             }
         }
     } else {
         // =========================================================================== producers + epilogue
+        // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < 4.  A half-warp holds
+        // 8 rows x 2 octets, so its 8-byte A-tile stores fall into 16 different bank pairs (no conflicts).
+        const int og = (lane >> 3) & 1, l8 = lane & 7;
+        const int oct = 2 * (warp & 3) + og;
+        const int mrow0 = 64 * (warp >> 2) + 8 * (lane >> 4) + l8;
         const int q_epi = warp >> 2;                 // column half read by this warp in the epilogue
         const int lane_base = 32 * (warp & 3);       // TMEM lanes this warp may access
         Acc accQ[8], accR[8];
 #pragma unroll
         for (int g = 0; g < 8; ++g) { accQ[g] = 0; accR[g] = 0; }
-        // dither constants: slot parity (t + pr + lane) & 1 selects (k, 1 - k) for the two rows of a packed pair
-        const float2 magic2[2] = {make_float2(kMagic + (float)(lane & 1), kMagic + (float)((lane & 1) ^ 1)),
-                                  make_float2(kMagic + (float)((lane & 1) ^ 1), kMagic + (float)(lane & 1))};
-        uint8_t *uj_mine = ujw + warp * (8 * kUJStride);
-        const int jj = 8 * warp + (lane >> 2);  // j (local) of this thread's label tasks; lanes 0..7 load record 8 warp + lane
+        // dither constants: k alternates with the row and with the parity of j
+        const float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
+        const float2 magicB = make_float2(magicA.y, magicA.x);
+        uint8_t *uj_mine = ujw + warp * kUJWarpBytes;   // this warp's 16 j of the K block as 8 pairs
+        const int jj = 8 * warp + (lane >> 2);          // j (local) of this thread's two label words
+        const int l3 = lane & 3;
+        const uint32_t full_remote0 = mapa_rank(smem_u32(&bar_full[0]), 0);
+        const uint32_t accempty_remote = mapa_rank(smem_u32(&bar_accempty), 0);
         uint32_t it = 0, un = 0;
-        for (int u = blockIdx.x; u < P.nunits; u += gridDim.x, ++un) {
+        for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
             const Unit U = P.units[u];
-            const long long row0 = (long long)U.I * kTM;
-            // this thread's four i rows: lane, lane + 32, lane + 64, lane + 96, packed as (r0, r1), (r2, r3)
-            float2 ui2[2][D];
-            {
-                float ur[4][D];
+            const long long row0 = (long long)U.I * kTM2 + (long long)rank * kTM;
+            // this thread's four i rows, duplicated for the packed FP32 pipe
+            float2 ui2[4][D];
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (row0 + lane + 32 * r) * F);
-                    float v[F];
+            for (int r = 0; r < 4; ++r) {
+                const float4 *p = reinterpret_cast<const float4 *>(P.rec + (row0 + mrow0 + 16 * r) * F);
+                float v[F];
 #pragma unroll
-                    for (int qq = 0; qq < F / 4; ++qq) {
-                        const float4 t = __ldg(p + qq);
-                        v[4 * qq] = t.x; v[4 * qq + 1] = t.y; v[4 * qq + 2] = t.z; v[4 * qq + 3] = t.w;
-                    }
-#pragma unroll
-                    for (int k = 0; k < D; ++k) ur[r][k] = v[k];
+                for (int qq = 0; qq < F / 4; ++qq) {
+                    const float4 t = __ldg(p + qq);
+                    v[4 * qq] = t.x; v[4 * qq + 1] = t.y; v[4 * qq + 2] = t.z; v[4 * qq + 3] = t.w;
                 }
+                // "+ 0" materialises each pair in an aligned register pair once per unit
 #pragma unroll
-                for (int k = 0; k < D; ++k) {
-                    // "+ 0" materialises each pair in an aligned register pair once per unit (ptxas otherwise re-forms the
-                    // pairs from the scalar load registers with two moves at every use inside the K-block loop)
-                    ui2[0][k] = __fadd2_rn(make_float2(ur[0][k], ur[1][k]), make_float2(0.f, 0.f));
-                    ui2[1][k] = __fadd2_rn(make_float2(ur[2][k], ur[3][k]), make_float2(0.f, 0.f));
-                }
+                for (int k = 0; k < D; ++k) ui2[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             }
-            // loads of K block kb: lanes 0..7 one record each, every lane four label words; prefetched one block ahead
+            // loads of K block kb: lanes 0..15 one record each, every lane two label words; prefetched one block ahead
             float4 rj[F / 4];
-            uint32_t mw[4];
+            uint32_t mw[2];
             auto load_block = [&](int kb) {
                 const long long j0 = (long long)kb * kKB;
-                if (lane < 8) {
-                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + 8 * warp + lane) * F);
+                if (lane < 16) {
+                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + 16 * (warp & 3) + lane) * F);
 #pragma unroll
                     for (int qq = 0; qq < F / 4; ++qq) rj[qq] = __ldg(p + qq);
                 }
-                const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + (lane & 3);
-#pragma unroll
-                for (int G = 0; G < 4; ++G) mw[G] = __ldg(mp + 4 * G);
+                const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + 4 * rank + l3;
+                mw[0] = __ldg(mp);
+                mw[1] = __ldg(mp + 8);
             };
             load_block(U.kb_begin);
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                const int s = it & 1;
+                const int s = it % kStages;
                 uint8_t *stA = smem + s * kStageBytes;
                 uint8_t *stB = stA + kABytes;
                 const long long j0 = (long long)kb * kKB;
-                // this warp's eight j records -> shared (negated, duplicated for the packed FP32 pipe)
+                // this warp's sixteen j records -> shared as pairs: float2 k = (-u_j0k, -u_j1k), float2 D = (s_j0, s_j1)
                 __syncwarp();
-                if (lane < 8) {
+                if (lane < 16) {
                     float v[F];
 #pragma unroll
                     for (int qq = 0; qq < F / 4; ++qq) { v[4 * qq] = rj[qq].x; v[4 * qq + 1] = rj[qq].y; v[4 * qq + 2] = rj[qq].z; v[4 * qq + 3] = rj[qq].w; }
-                    float2 *o = reinterpret_cast<float2 *>(uj_mine + lane * kUJStride);
+                    float *o = reinterpret_cast<float *>(uj_mine + (lane >> 1) * (NLD * 16)) + (lane & 1);
 #pragma unroll
-                    for (int k = 0; k < D; ++k) o[k] = make_float2(-v[k], -v[k]);
-                    const float sj = __fmul_rn(v[D], P.sc2);
-                    o[D] = make_float2(sj, sj);
-                    if (NP & 1) o[NP] = make_float2(0.f, 0.f);
+                    for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
+                    o[2 * D] = __fmul_rn(v[D], P.sc2);
+                    if (NP & 1) o[2 * NP] = 0.f;
                 }
-                uint32_t mcur[4];
-#pragma unroll
-                for (int G = 0; G < 4; ++G) mcur[G] = mw[G];
+                uint32_t mcur[2] = {mw[0], mw[1]};
                 __syncwarp();
                 if (kb + 1 < U.kb_end) load_block(kb + 1);
-                mbar_wait(&bar_empty[s], ((it >> 1) & 1) ^ 1);
+                mbar_wait(&bar_empty[s], ((it / kStages) & 1) ^ 1);
 
-                // ---- psi tile: rows {lane + 32 r}, j = 8 warp .. 8 warp + 7 --------------------------------
-                const bool diag = j0 < row0 + kTM;  // K block overlaps the row tile: keep only j > i
+                // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7 ------------------------------------
                 uint32_t fq[4][8];
 #pragma unroll
-                for (int t = 0; t < 8; ++t) {
-                    const float4 *up = reinterpret_cast<const float4 *>(uj_mine + t * kUJStride);
+                for (int tp = 0; tp < 4; ++tp) {
+                    const float4 *up = reinterpret_cast<const float4 *>(uj_mine + (4 * og + tp) * (NLD * 16));
                     float2 nu[2 * NLD];
 #pragma unroll
                     for (int qq = 0; qq < NLD; ++qq) {
@@ -356,30 +410,30 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                         nu[2 * qq + 1] = make_float2(v.z, v.w);
                     }
 #pragma unroll
-                    for (int pr = 0; pr < 2; ++pr) {
-                        float2 dd = __fadd2_rn(ui2[pr][0], nu[0]);
+                    for (int r = 0; r < 4; ++r) {
+                        float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
                         float2 e = __fmul2_rn(dd, dd);
 #pragma unroll
                         for (int k = 1; k < D; ++k) {
-                            dd = __fadd2_rn(ui2[pr][k], nu[k]);
+                            dd = __fadd2_rn(ui2[r][k], nu[k]);
                             e = __ffma2_rn(dd, dd, e);
                         }
-                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magic2[(t + pr) & 1]);
-                        fq[2 * pr][t] = __float_as_uint(f2.x);
-                        fq[2 * pr + 1][t] = __float_as_uint(f2.y);
+                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], (r & 1) ? magicB : magicA);
+                        fq[r][2 * tp] = __float_as_uint(f2.x);
+                        fq[r][2 * tp + 1] = __float_as_uint(f2.y);
                     }
                 }
-                if (diag) {
+                if (j0 < row0 + kTM) {  // K block overlaps (or lies below) the rows of this CTA: keep only j > i
                     const uint32_t zero = __float_as_uint(kMagic);
 #pragma unroll
                     for (int r = 0; r < 4; ++r)
 #pragma unroll
                         for (int t = 0; t < 8; ++t)
-                            if (j0 + 8 * warp + t <= row0 + lane + 32 * r) fq[r][t] = zero;
+                            if (j0 + 8 * oct + t <= row0 + mrow0 + 16 * r) fq[r][t] = zero;
                 }
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
-                    const int m = lane + 32 * r;
+                    const int m = mrow0 + 16 * r;
                     const uint32_t p01 = __byte_perm(fq[r][0], fq[r][1], 0x5140), p23 = __byte_perm(fq[r][2], fq[r][3], 0x5140);
                     const uint32_t p45 = __byte_perm(fq[r][4], fq[r][5], 0x5140), p67 = __byte_perm(fq[r][6], fq[r][7], 0x5140);
                     uint2 lo, hi;
@@ -387,32 +441,34 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                     lo.y = (__byte_perm(p45, p67, 0x5410) >> 1) & 0x7f7f7f7fu;
                     hi.x = __byte_perm(p01, p23, 0x7632);
                     hi.y = __byte_perm(p45, p67, 0x7632);
-                    const int off = (m >> 3) * 512 + (m & 7) * 64 + (((warp >> 1) ^ ((m >> 1) & 3)) << 4) + ((warp & 1) << 3);
+                    const int off = (m >> 3) * 512 + (m & 7) * 64 + (((oct >> 1) ^ ((m >> 1) & 3)) << 4) + ((oct & 1) << 3);
                     *reinterpret_cast<uint2 *>(stA + off) = hi;
                     *reinterpret_cast<uint2 *>(stA + kTM * kKB + off) = lo;
                 }
-                // ---- label tile: j = jj, words 4 G + (lane & 3) -> 32 columns each, bytes a (lo) and 128 a (hi)
+                // ---- label tile: j = jj, this CTA's words 8 q + 4 rank + l3 -> 32 columns each; byte p of a word
+                //      is label bit beta(p): register t = (m >> t) & 0x01010101 (bytes a), << 7 (bytes 128 a)
                 {
-                    const int r = lane >> 2, c = 2 * (lane & 3);
+                    const int r = lane >> 2, c = 2 * l3;
                     const int o0 = warp * 1024 + r * 128 + ((c ^ r) << 4), o1 = warp * 1024 + r * 128 + (((c + 1) ^ r) << 4);
 #pragma unroll
-                    for (int G = 0; G < 4; ++G) {
-                        const uint32_t m = mcur[G];
-                        const uint2 l0 = *reinterpret_cast<const uint2 *>(&lut[m & 255u]), l1 = *reinterpret_cast<const uint2 *>(&lut[(m >> 8) & 255u]);
-                        const uint2 l2 = *reinterpret_cast<const uint2 *>(&lut[(m >> 16) & 255u]), l3 = *reinterpret_cast<const uint2 *>(&lut[m >> 24]);
-                        uint8_t *bh = stB + (((G >> 1) * 2 + 0) * 2 + (G & 1)) * 8192;  // q = G >> 1, digit, h = G & 1
-                        uint8_t *bl = stB + (((G >> 1) * 2 + 1) * 2 + (G & 1)) * 8192;
-                        *reinterpret_cast<uint4 *>(bl + o0) = make_uint4(l0.x, l0.y, l1.x, l1.y);
-                        *reinterpret_cast<uint4 *>(bl + o1) = make_uint4(l2.x, l2.y, l3.x, l3.y);
-                        *reinterpret_cast<uint4 *>(bh + o0) = make_uint4(l0.x << 7, l0.y << 7, l1.x << 7, l1.y << 7);
-                        *reinterpret_cast<uint4 *>(bh + o1) = make_uint4(l2.x << 7, l2.y << 7, l3.x << 7, l3.y << 7);
+                    for (int q = 0; q < 2; ++q) {
+                        const uint32_t m = mcur[q];
+                        uint32_t a[8];
+#pragma unroll
+                        for (int t = 0; t < 8; ++t) a[t] = (m >> t) & 0x01010101u;
+                        uint8_t *bh = stB + (q * 2 + 0) * 8192;
+                        uint8_t *bl = stB + (q * 2 + 1) * 8192;
+                        *reinterpret_cast<uint4 *>(bl + o0) = make_uint4(a[0], a[1], a[2], a[3]);
+                        *reinterpret_cast<uint4 *>(bl + o1) = make_uint4(a[4], a[5], a[6], a[7]);
+                        *reinterpret_cast<uint4 *>(bh + o0) = make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7);
+                        *reinterpret_cast<uint4 *>(bh + o1) = make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7);
                     }
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bar_full[s]);
+                if (lane == 0) mbar_arrive_cluster(full_remote0 + 8 * s);
             }
-            // ---- epilogue of the unit -------------------------------------------------------------------
+            // ---- epilogue of the unit: this CTA's 128 rows x 512 columns -------------------------------------
             mbar_wait(&bar_accfull, un & 1);
             tc_fence_after();
             {
@@ -422,7 +478,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                 const bool real = (w0 >> 2) & 1u;
                 const float wf = P.rec[row * F + D];
                 const uint32_t taddr = tmem + ((uint32_t)lane_base << 16);
-                const int yones = (int)tmem_ld1(taddr + 2);
+                const int yones = (int)tmem_ld1(taddr + 8);  // label column 2 (all ones) is byte beta^-1(2) = 8 of word 0
                 Acc wi, zi;
                 if (WEIGHTED) { wi = (Acc)wf; zi = wi * (Acc)yones; }
                 else { wi = 1; zi = (Acc)yones; }
@@ -433,10 +489,10 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
                     tmem_ld32(taddr + q_epi * 256 + 32 * g, v);
                     Acc x[32];
 #pragma unroll
-                    for (int b = 0; b < 32; ++b) x[b] = ((mword >> b) & 1u) ? wi * (Acc)(int)v[b] : (Acc)0;
+                    for (int b = 0; b < 32; ++b) x[b] = ((mword >> beta(b)) & 1u) ? wi * (Acc)(int)v[b] : (Acc)0;
                     const Acc qs = lane_transpose_sum(x, lane);
 #pragma unroll
-                    for (int b = 0; b < 32; ++b) x[b] = (real ? wi * (Acc)(int)v[b] : (Acc)0) + (((mword >> b) & 1u) ? zi : (Acc)0);
+                    for (int b = 0; b < 32; ++b) x[b] = (real ? wi * (Acc)(int)v[b] : (Acc)0) + (((mword >> beta(b)) & 1u) ? zi : (Acc)0);
                     const Acc rs = lane_transpose_sum(x, lane);
 #pragma unroll
                     for (int gg = 0; gg < 8; ++gg)
@@ -445,9 +501,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_accempty);
+            if (lane == 0) mbar_arrive_cluster(accempty_remote);
         }
-        // per-warp partial column sums: partial[cta][warp][g][lane][2]
+        // per-warp partial column sums: partial[cta][warp][g][lane][2]; lane L of group g = TMEM column 32 g + L
         Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * 8 * 32 * 2;
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
@@ -457,11 +513,12 @@ __global__ void __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == kProducerWarps) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+    cluster_sync_all();  // the peer may still be reading this CTA's shared memory / TMEM through the pair's MMAs
+    if (warp == kProducerWarps) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem));
 }
 
-// Column sums over CTAs and warps, fixed order: column c = 256 q + 32 g + lane is held by warps 4 q .. 4 q + 3.
-// out[c] = {Q, R} as doubles in units of psi (divided by sc).
+// Column sums over CTAs and warps, fixed order: TMEM column 256 q + 32 g + lane is held by warps 4 q .. 4 q + 3 and is
+// label column c = 256 q + 32 g + beta(lane).  out[c] = {Q, R} as doubles in units of psi (divided by sc).
 template <bool WEIGHTED>
 __global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double *__restrict__ outQ, double *__restrict__ outR)
 {
@@ -477,8 +534,9 @@ __global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double
             sq += e[0];
             sr += e[1];
         }
-    outQ[c] = (double)sq * inv_sc;
-    outR[c] = (double)sr * inv_sc;
+    const int col = (c & ~31) + beta(lane);
+    outQ[col] = (double)sq * inv_sc;
+    outR[col] = (double)sr * inv_sc;
 }
 
 // Label words of the TC layout: maskT[pos][chunk * 16 + W], column c = 32 W + b of chunk ch:
