@@ -58,7 +58,7 @@ struct et_ctx {
     int64_t opt_perm_kernel = 0;
     int64_t opt_perm_offset = 0;
     double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
-    Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW;
+    Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP;
     bool tc_attr_set = false;
 };
 
@@ -782,11 +782,16 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     else { hi_signed = true; sc = 16383.0 / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
 
     const int grid = 2 * std::min(nclusters_max, nunits);  // CTA pairs
-    const size_t part_bytes = (size_t)grid * tc::kProducerWarps * 8 * 32 * 2 * 8;
+    const size_t part_bytes = (size_t)grid * tc::kProducerWarps * tc::kEpiGroups * 32 * 2 * 8;
     ET_TRY(ensure(ctx, ctx->tcpart, part_bytes));
     ET_TRY(ensure(ctx, ctx->tcQ, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(span_begin(ctx, 2));
+    const float sc2 = (float)(2.0 * sc);
+    ET_TRY(ensure(ctx, ctx->recP, (size_t)(L.npad / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
+    DISPATCH_DIM(dim, (tc::k_pair_records<D><<<(unsigned)((L.npad / 2 + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
+                          static_cast<const float *>(ctx->rec.p), L.npad / 2, sc2, static_cast<float4 *>(ctx->recP.p))));
+    LAUNCH_CHECK();
     for (int ch = 0; ch < nchunks; ++ch) {
         tc::TCParams P{};
         P.rec = static_cast<const float *>(ctx->rec.p);
@@ -795,7 +800,8 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         P.word0 = ch * tc::kWordsPerChunk;
         P.units = static_cast<const tc::Unit *>(ctx->units.p);
         P.nunits = nunits;
-        P.sc2 = (float)(2.0 * sc);
+        P.sc2 = sc2;
+        P.recP = static_cast<const float4 *>(ctx->recP.p);
         P.idesc_hi = tc::umma_idesc_i8(hi_signed);
         P.partial = ctx->tcpart.p;
         DISPATCH_DIM(dim, ET_TRY(launch_perm_tc<D>(ctx, P, grid, weighted)));
@@ -900,7 +906,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->tilecls, &ctx->partials, &ctx->sums, &ctx->rowsum, &ctx->mask, &ctx->sel, &ctx->hist, &ctx->partQ,
                    &ctx->Q, &ctx->partRW, &ctx->RW, &ctx->mm, &ctx->flag, &ctx->counter, &ctx->src, &ctx->posx, &ctx->posb,
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
-                   &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW};
+                   &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);

@@ -26,6 +26,10 @@
 
 #include "et_kernels.cuh"
 
+#ifndef ET_TC_DBG
+#define ET_TC_DBG 0  // timing experiments only (_work probes): 1 no tile generation, 2 no MMAs, 3 no label tile, 4 no psi tile
+#endif
+
 namespace et {
 namespace tc {
 
@@ -36,16 +40,18 @@ constexpr int kCols = 512;               // label columns per launch (2 accumula
 constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
-constexpr int kProducerWarps = 8;
+constexpr int kProducerWarps = 16;          // four per scheduler: the tile generation is latency-bound with two (profiles/r01b)
+constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // a thread evaluates 8 j x this many rows (2)
+constexpr int kEpiGroups = 16 / (kProducerWarps / 4);                 // 32-column groups per warp in the epilogue (4)
 constexpr int kProducers = kProducerWarps * 32;
-constexpr int kThreadsTC = kProducers + 32;  // + the MMA warp
+constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
 constexpr int kStages = 4;
 constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (16 KB)
 constexpr int kBBytes = 2 * 2 * 8192;        // this CTA's half of B: [q 2][digit 2][64 j x 128 columns] (32 KB)
 constexpr int kStageBytes = kABytes + kBBytes;
-constexpr int kUJWarpBytes = 8 * 80;         // per producer warp: 8 j pairs x (dim + 1 <= 9 float2 -> 5 float4)
-constexpr int kUJBytes = kProducerWarps * kUJWarpBytes;
-constexpr int kSmemTC = kStages * kStageBytes + kUJBytes + 1024 /*alignment slack*/;
+constexpr int kRecSlots = 8;                 // ring of j pair-record blocks (32 pairs each), filled by bulk copies
+constexpr int kRecSlotBytesMax = (kKB / 2) * 5 * 16;
+constexpr int kSmemTC = kStages * kStageBytes + kRecSlots * kRecSlotBytesMax + 1024 /*alignment slack*/;
 // 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
 // complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
 // of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
@@ -55,6 +61,9 @@ constexpr int kMaxUnitKB = 512;               // K blocks per unit: |Y| <= 32767
 
 // label bit held by byte / TMEM column p of a 32-column word
 __host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
+
+// float4 per pair record: dim + 1 float2 entries, padded to an even count
+__host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
 
 struct Unit {
     int I;         // 256-row tile
@@ -172,6 +181,17 @@ __device__ __forceinline__ void umma_i8_pair(uint32_t tmem_d, uint64_t da, uint6
         "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// bulk copy global -> this CTA's shared memory, completion counted in bytes on an mbarrier (one thread issues)
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
+                 "r"(smem_u32(bar))
+                 : "memory");
+}
+// hides a loop-invariant value from the optimiser (see the producer loop)
+__device__ __forceinline__ int keep(int x) { asm volatile("" : "+r"(x)); return x; }
+__device__ __forceinline__ float keep(float x) { asm volatile("" : "+f"(x)); return x; }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -238,16 +258,43 @@ __device__ __forceinline__ T lane_transpose_sum(T (&x)[32], int lane)
     return x[0];
 }
 
+// Pair records of the j side: recP[pair][entry] float2, entry k < D = (-u_{2 pair, k}, -u_{2 pair + 1, k}), entry D =
+// (s, s') with s = 2 sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
+// i rows duplicated in registers, d = u_i + (-u_j) and Psi = 2^(-e) s + magic are packed FADD2 / FFMA2 over two j.
+template <int D>
+__global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restrict__ rec, long long npairs, float sc2, float4 *__restrict__ recP)
+{
+    constexpr int F = rec_floats(D), NLD = pair_rec_f4(D);
+    const long long pr = blockIdx.x * (long long)kThreads + threadIdx.x;
+    if (pr >= npairs) return;
+    float a[F], b[F], o[4 * NLD];
+#pragma unroll
+    for (int q = 0; q < F / 4; ++q) {
+        const float4 ta = reinterpret_cast<const float4 *>(rec + 2 * pr * F)[q], tb = reinterpret_cast<const float4 *>(rec + (2 * pr + 1) * F)[q];
+        a[4 * q] = ta.x; a[4 * q + 1] = ta.y; a[4 * q + 2] = ta.z; a[4 * q + 3] = ta.w;
+        b[4 * q] = tb.x; b[4 * q + 1] = tb.y; b[4 * q + 2] = tb.z; b[4 * q + 3] = tb.w;
+    }
+#pragma unroll
+    for (int k = 0; k < 4 * NLD; ++k) o[k] = 0.f;
+#pragma unroll
+    for (int k = 0; k < D; ++k) { o[2 * k] = -a[k]; o[2 * k + 1] = -b[k]; }
+    o[2 * D] = __fmul_rn(a[D], sc2);
+    o[2 * D + 1] = __fmul_rn(b[D], sc2);
+#pragma unroll
+    for (int q = 0; q < NLD; ++q) recP[pr * NLD + q] = make_float4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
+}
+
 struct TCParams {
     const float *rec;        // pooled records [npad][F]
+    const float4 *recP;      // pair records [npad / 2][NLD] (k_pair_records)
     const uint32_t *maskT;   // labels [npad][words_total], this launch uses words [word0, word0 + 16)
     int words_total;
     int word0;
     const Unit *units;
     int nunits;
-    float sc2;               // 2 * sc: Psi_ij = w_j psi_ij is quantised to v ~ sc Psi (15 bits)
+    float sc2;               // 2 * sc: Psi_ij = w_j psi_ij is quantised to v ~ sc Psi (15 bits); applied in recP
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
-    void *partial;           // [gridDim.x][8 warps][8 groups][32 lanes][2] of Acc
+    void *partial;           // [gridDim.x][16 warps][4 groups][32 lanes][2] of Acc
 };
 
 // One launch = 512 label columns.  Grid: persistent, one CTA per SM, clusters of 2 (an SM pair); unit u is processed
@@ -259,13 +306,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
     constexpr int F = rec_floats(D);
-    constexpr int NP = D + 1;               // float2 entries per j pair: (-u_j0k, -u_j1k), then (s_j0, s_j1)
-    constexpr int NLD = (NP + 1) / 2;       // LDS.128 per j pair
+    constexpr int NLD = pair_rec_f4(D);     // 16-byte loads per j pair: float2 (-u_j0k, -u_j1k) k < D, then (s_j0, s_j1)
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    uint8_t *ujw = smem + kStages * kStageBytes;  // per-warp j-pair records
-    __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty;
+    __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty, bar_rec[kRecSlots];
+    constexpr uint32_t kRecSlotBytes = (kKB / 2) * NLD * 16;
+    uint8_t *recs = smem + kStages * kStageBytes;  // record ring
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -278,6 +325,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], 2 * kProducerWarps); mbar_init(&bar_empty[s], 1); }
         mbar_init(&bar_accfull, 1);
         mbar_init(&bar_accempty, 2 * kProducerWarps);
+        for (int s = 0; s < kRecSlots; ++s) mbar_init(&bar_rec[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == kProducerWarps) {
@@ -314,42 +362,67 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                                 const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
                                 const uint64_t db = umma_desc(b_base + (q * 2 + d) * 8192 + ks * 4 * 1024, 8192, 1024, 2);
                                 const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
-                                umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
+                                if (ET_TC_DBG != 2) umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
                             }
                     umma_commit_pair(&bar_empty[s]);  // frees the stage in both CTAs when these MMAs have read it
                 }
                 umma_commit_pair(&bar_accfull);
             }
         }
+    } else if (warp == kProducerWarps + 1) {
+        // =========================================================================== record loader (each CTA, one lane)
+        // The pair records of K block `it` go to ring slot it % 8 by one bulk copy, up to 8 blocks ahead of the MMAs:
+        // the slot was last read for block it - 8, whose stage has been released (bar_empty) once its MMAs were done.
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (int u = cluster_id; u < P.nunits; u += nclusters) {
+                const Unit U = P.units[u];
+                for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+                    if (it >= kRecSlots) mbar_wait(&bar_empty[(it - kRecSlots) & (kStages - 1)], ((it - kRecSlots) / kStages) & 1);
+                    const uint32_t slot = it & (kRecSlots - 1);
+                    bulk_g2s(smem_u32(recs + slot * kRecSlotBytes), P.recP + (long long)kb * (kKB / 2) * NLD, kRecSlotBytes, &bar_rec[slot]);
+                }
+            }
+        }
     } else {
         // =========================================================================== producers + epilogue
-        // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < 4.  A half-warp holds
+        // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < R.  A half-warp holds
         // 8 rows x 2 octets, so its 8-byte A-tile stores fall into 16 different bank pairs (no conflicts).
+        constexpr int R = kRowsPerThread, G = kEpiGroups;
         const int og = (lane >> 3) & 1, l8 = lane & 7;
         const int oct = 2 * (warp & 3) + og;
-        const int mrow0 = 64 * (warp >> 2) + 8 * (lane >> 4) + l8;
-        const int q_epi = warp >> 2;                 // column half read by this warp in the epilogue
+        const int mrow0 = 16 * R * (warp >> 2) + 8 * (lane >> 4) + l8;
+        const int grp0 = G * (warp >> 2);            // first of the 16 column groups (32 columns each) of this warp's epilogue
         const int lane_base = 32 * (warp & 3);       // TMEM lanes this warp may access
-        Acc accQ[8], accR[8];
+        Acc accQ[G], accR[G];
 #pragma unroll
-        for (int g = 0; g < 8; ++g) { accQ[g] = 0; accR[g] = 0; }
-        // dither constants: k alternates with the row and with the parity of j
-        const float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
-        const float2 magicB = make_float2(magicA.y, magicA.x);
-        uint8_t *uj_mine = ujw + warp * kUJWarpBytes;   // this warp's 16 j of the K block as 8 pairs
-        const int jj = 8 * warp + (lane >> 2);          // j (local) of this thread's two label words
+        for (int g = 0; g < G; ++g) { accQ[g] = 0; accR[g] = 0; }
+        // Thread constants of the main loop.  They are made opaque to the compiler (keep()), which otherwise
+        // rematerialises them from the lane index in every K block to save registers (~45 instructions, profiles/r01c).
+        // dither constant: k alternates with the row and with the parity of j
+        float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
+        magicA.x = keep(magicA.x);
+        magicA.y = keep(magicA.y);
+        const int jw = warp & 7, qw = warp >> 3;        // label task: 8 j of the K block, column half q
+        const int jj = 8 * jw + (lane >> 2);            // j (local) of this thread's label word
         const int l3 = lane & 3;
+        // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct; SWIZZLE_64B; row
+        // mrow0 + 16 r is 1024 r further) and B tile (j = jj, hi plane of column half qw, 16-byte chunk 2 l3 of the
+        // 128-column row; SWIZZLE_128B; chunk 2 l3 + 1 is at address ^ 16, the lo plane 8192 further)
+        const int offA = keep((mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3));
+        const int offB = keep(kABytes + qw * 16384 + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4));
+        const int offJ = keep(kStages * kStageBytes + 4 * oct * NLD * 16);  // its four j pairs inside a record slot
         const uint32_t full_remote0 = mapa_rank(smem_u32(&bar_full[0]), 0);
         const uint32_t accempty_remote = mapa_rank(smem_u32(&bar_accempty), 0);
         uint32_t it = 0, un = 0;
         for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
             const Unit U = P.units[u];
-            const long long row0 = (long long)U.I * kTM2 + (long long)rank * kTM;
-            // this thread's four i rows, duplicated for the packed FP32 pipe
-            float2 ui2[4][D];
+            const int row0 = U.I * kTM2 + (int)rank * kTM;   // npad < 2^31
+            // this thread's i rows, duplicated for the packed FP32 pipe
+            float2 ui2[R][D];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const float4 *p = reinterpret_cast<const float4 *>(P.rec + (row0 + mrow0 + 16 * r) * F);
+            for (int r = 0; r < R; ++r) {
+                const float4 *p = reinterpret_cast<const float4 *>(P.rec + (long long)(row0 + mrow0 + 16 * r) * F);
                 float v[F];
 #pragma unroll
                 for (int qq = 0; qq < F / 4; ++qq) {
@@ -360,57 +433,39 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 #pragma unroll
                 for (int k = 0; k < D; ++k) ui2[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             }
-            // loads of K block kb: lanes 0..15 one record each, every lane two label words; prefetched one block ahead
-            float4 rj[F / 4];
-            uint32_t mw[2];
-            auto load_block = [&](int kb) {
-                const long long j0 = (long long)kb * kKB;
-                if (lane < 16) {
-                    const float4 *p = reinterpret_cast<const float4 *>(P.rec + (j0 + 16 * (warp & 3) + lane) * F);
-#pragma unroll
-                    for (int qq = 0; qq < F / 4; ++qq) rj[qq] = __ldg(p + qq);
-                }
-                const uint32_t *mp = P.maskT + (j0 + jj) * P.words_total + P.word0 + 4 * rank + l3;
-                mw[0] = __ldg(mp);
-                mw[1] = __ldg(mp + 8);
-            };
-            load_block(U.kb_begin);
+            // K blocks below kb_diag overlap (or lie below) the rows of this CTA: there only j > i is kept, i.e. element
+            // (r, t) of this thread's tile is dropped when kb * 64 + t <= dthr + 16 r
+            const int kb_diag = (row0 + kTM + kKB - 1) / kKB;
+            const int dthr = row0 + mrow0 - 8 * oct;
+            // this thread's label word of K block kb (element index < 2^32), prefetched one block ahead into a register
+            uint32_t im = (uint32_t)(U.kb_begin * kKB + jj) * (uint32_t)P.words_total + (uint32_t)(P.word0 + 8 * qw + 4 * (int)rank + l3);
+            const uint32_t im_step = (uint32_t)(kKB * P.words_total);
+            uint32_t mw = __ldg(P.maskT + im);
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                const int s = it % kStages;
-                uint8_t *stA = smem + s * kStageBytes;
-                uint8_t *stB = stA + kABytes;
-                const long long j0 = (long long)kb * kKB;
-                // this warp's sixteen j records -> shared as pairs: float2 k = (-u_j0k, -u_j1k), float2 D = (s_j0, s_j1)
-                __syncwarp();
-                if (lane < 16) {
-                    float v[F];
-#pragma unroll
-                    for (int qq = 0; qq < F / 4; ++qq) { v[4 * qq] = rj[qq].x; v[4 * qq + 1] = rj[qq].y; v[4 * qq + 2] = rj[qq].z; v[4 * qq + 3] = rj[qq].w; }
-                    float *o = reinterpret_cast<float *>(uj_mine + (lane >> 1) * (NLD * 16)) + (lane & 1);
-#pragma unroll
-                    for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
-                    o[2 * D] = __fmul_rn(v[D], P.sc2);
-                    if (NP & 1) o[2 * NP] = 0.f;
+                uint8_t *st = smem + (it & (kStages - 1)) * kStageBytes;
+                const float4 *pj = reinterpret_cast<const float4 *>(smem + offJ + (it & (kRecSlots - 1)) * kRecSlotBytes);
+                const uint32_t mcur = mw;
+                if (kb + 1 < U.kb_end) {
+                    im += im_step;
+                    mw = __ldg(P.maskT + im);
                 }
-                uint32_t mcur[2] = {mw[0], mw[1]};
-                __syncwarp();
-                if (kb + 1 < U.kb_end) load_block(kb + 1);
-                mbar_wait(&bar_empty[s], ((it / kStages) & 1) ^ 1);
+                mbar_wait(&bar_rec[it & (kRecSlots - 1)], (it / kRecSlots) & 1);
+                mbar_wait(&bar_empty[it & (kStages - 1)], ((it / kStages) & 1) ^ 1);
 
                 // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7 ------------------------------------
-                uint32_t fq[4][8];
+                if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
+                uint32_t fq[R][8];
 #pragma unroll
                 for (int tp = 0; tp < 4; ++tp) {
-                    const float4 *up = reinterpret_cast<const float4 *>(uj_mine + (4 * og + tp) * (NLD * 16));
                     float2 nu[2 * NLD];
 #pragma unroll
                     for (int qq = 0; qq < NLD; ++qq) {
-                        const float4 v = up[qq];
+                        const float4 v = pj[tp * NLD + qq];
                         nu[2 * qq] = make_float2(v.x, v.y);
                         nu[2 * qq + 1] = make_float2(v.z, v.w);
                     }
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
+                    for (int r = 0; r < R; ++r) {
                         float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
                         float2 e = __fmul2_rn(dd, dd);
 #pragma unroll
@@ -418,22 +473,23 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             dd = __fadd2_rn(ui2[r][k], nu[k]);
                             e = __ffma2_rn(dd, dd, e);
                         }
-                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], (r & 1) ? magicB : magicA);
+                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magicA);
                         fq[r][2 * tp] = __float_as_uint(f2.x);
                         fq[r][2 * tp + 1] = __float_as_uint(f2.y);
                     }
                 }
-                if (j0 < row0 + kTM) {  // K block overlaps (or lies below) the rows of this CTA: keep only j > i
+                if (kb < kb_diag) {
                     const uint32_t zero = __float_as_uint(kMagic);
+                    const int x = kb * kKB - dthr;
 #pragma unroll
-                    for (int r = 0; r < 4; ++r)
+                    for (int r = 0; r < R; ++r)
 #pragma unroll
                         for (int t = 0; t < 8; ++t)
-                            if (j0 + 8 * oct + t <= row0 + mrow0 + 16 * r) fq[r][t] = zero;
+                            if (x <= 16 * r - t) fq[r][t] = zero;
                 }
+                uint8_t *pa = st + offA;
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int m = mrow0 + 16 * r;
+                for (int r = 0; r < R; ++r) {
                     const uint32_t p01 = __byte_perm(fq[r][0], fq[r][1], 0x5140), p23 = __byte_perm(fq[r][2], fq[r][3], 0x5140);
                     const uint32_t p45 = __byte_perm(fq[r][4], fq[r][5], 0x5140), p67 = __byte_perm(fq[r][6], fq[r][7], 0x5140);
                     uint2 lo, hi;
@@ -441,38 +497,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     lo.y = (__byte_perm(p45, p67, 0x5410) >> 1) & 0x7f7f7f7fu;
                     hi.x = __byte_perm(p01, p23, 0x7632);
                     hi.y = __byte_perm(p45, p67, 0x7632);
-                    const int off = (m >> 3) * 512 + (m & 7) * 64 + (((oct >> 1) ^ ((m >> 1) & 3)) << 4) + ((oct & 1) << 3);
-                    *reinterpret_cast<uint2 *>(stA + off) = hi;
-                    *reinterpret_cast<uint2 *>(stA + kTM * kKB + off) = lo;
+                    *reinterpret_cast<uint2 *>(pa + 1024 * r) = hi;
+                    *reinterpret_cast<uint2 *>(pa + kTM * kKB + 1024 * r) = lo;
                 }
-                // ---- label tile: j = jj, this CTA's words 8 q + 4 rank + l3 -> 32 columns each; byte p of a word
+                }
+                // ---- label tile: j = jj, this CTA's word 8 qw + 4 rank + l3 -> 32 columns; byte p of a word
                 //      is label bit beta(p): register t = (m >> t) & 0x01010101 (bytes a), << 7 (bytes 128 a)
-                {
-                    const int r = lane >> 2, c = 2 * l3;
-                    const int o0 = warp * 1024 + r * 128 + ((c ^ r) << 4), o1 = warp * 1024 + r * 128 + (((c + 1) ^ r) << 4);
+                if (ET_TC_DBG != 1 && ET_TC_DBG != 3) {
+                    uint32_t a[8];
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        const uint32_t m = mcur[q];
-                        uint32_t a[8];
-#pragma unroll
-                        for (int t = 0; t < 8; ++t) a[t] = (m >> t) & 0x01010101u;
-                        uint8_t *bh = stB + (q * 2 + 0) * 8192;
-                        uint8_t *bl = stB + (q * 2 + 1) * 8192;
-                        *reinterpret_cast<uint4 *>(bl + o0) = make_uint4(a[0], a[1], a[2], a[3]);
-                        *reinterpret_cast<uint4 *>(bl + o1) = make_uint4(a[4], a[5], a[6], a[7]);
-                        *reinterpret_cast<uint4 *>(bh + o0) = make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7);
-                        *reinterpret_cast<uint4 *>(bh + o1) = make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7);
-                    }
+                    for (int t = 0; t < 8; ++t) a[t] = (mcur >> t) & 0x01010101u;
+                    uint8_t *b0 = st + offB;
+                    uint8_t *b1 = smem + ((uint32_t)(b0 - smem) ^ 16u);
+                    *reinterpret_cast<uint4 *>(b0 + 8192) = make_uint4(a[0], a[1], a[2], a[3]);
+                    *reinterpret_cast<uint4 *>(b1 + 8192) = make_uint4(a[4], a[5], a[6], a[7]);
+                    *reinterpret_cast<uint4 *>(b0) = make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7);
+                    *reinterpret_cast<uint4 *>(b1) = make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7);
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(full_remote0 + 8 * s);
+                if (lane == 0) mbar_arrive_cluster(full_remote0 + 8 * (it & (kStages - 1)));
             }
             // ---- epilogue of the unit: this CTA's 128 rows x 512 columns -------------------------------------
             mbar_wait(&bar_accfull, un & 1);
             tc_fence_after();
             {
-                const long long row = row0 + lane_base + lane;
+                const long long row = (long long)row0 + lane_base + lane;
                 const uint32_t *mp = P.maskT + row * P.words_total + P.word0;
                 const uint32_t w0 = __ldg(mp);
                 const bool real = (w0 >> 2) & 1u;
@@ -483,10 +533,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 if (WEIGHTED) { wi = (Acc)wf; zi = wi * (Acc)yones; }
                 else { wi = 1; zi = (Acc)yones; }
 #pragma unroll 1
-                for (int g = 0; g < 8; ++g) {
-                    const uint32_t mword = __ldg(mp + 8 * q_epi + g);
+                for (int g = 0; g < G; ++g) {
+                    const uint32_t mword = __ldg(mp + grp0 + g);
                     uint32_t v[32];
-                    tmem_ld32(taddr + q_epi * 256 + 32 * g, v);
+                    tmem_ld32(taddr + 32 * (grp0 + g), v);
                     Acc x[32];
 #pragma unroll
                     for (int b = 0; b < 32; ++b) x[b] = ((mword >> beta(b)) & 1u) ? wi * (Acc)(int)v[b] : (Acc)0;
@@ -495,7 +545,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     for (int b = 0; b < 32; ++b) x[b] = (real ? wi * (Acc)(int)v[b] : (Acc)0) + (((mword >> beta(b)) & 1u) ? zi : (Acc)0);
                     const Acc rs = lane_transpose_sum(x, lane);
 #pragma unroll
-                    for (int gg = 0; gg < 8; ++gg)
+                    for (int gg = 0; gg < G; ++gg)
                         if (gg == g) { accQ[gg] += qs; accR[gg] += rs; }
                 }
             }
@@ -503,10 +553,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(accempty_remote);
         }
-        // per-warp partial column sums: partial[cta][warp][g][lane][2]; lane L of group g = TMEM column 32 g + L
-        Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * 8 * 32 * 2;
+        // per-warp partial column sums: partial[cta][warp][g][lane][2]; lane L of group g = TMEM column 32 (grp0 + g) + L
+        Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * G * 32 * 2;
 #pragma unroll
-        for (int g = 0; g < 8; ++g) {
+        for (int g = 0; g < G; ++g) {
             out[(g * 32 + lane) * 2] = accQ[g];
             out[(g * 32 + lane) * 2 + 1] = accR[g];
         }
@@ -517,20 +567,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
     if (warp == kProducerWarps) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem));
 }
 
-// Column sums over CTAs and warps, fixed order: TMEM column 256 q + 32 g + lane is held by warps 4 q .. 4 q + 3 and is
-// label column c = 256 q + 32 g + beta(lane).  out[c] = {Q, R} as doubles in units of psi (divided by sc).
+// Column sums over CTAs and warps, fixed order: TMEM column 32 gc + lane (gc = c >> 5) is held by the four warps
+// 4 (gc / G) .. + 3 as their group gc % G, and is label column c = 32 gc + beta(lane).  out[c] = {Q, R} as doubles in
+// units of psi (divided by sc).
 template <bool WEIGHTED>
 __global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double *__restrict__ outQ, double *__restrict__ outR)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= kCols) return;
-    const int q = c >> 8, g = (c >> 5) & 7, lane = c & 31;
+    constexpr int G = kEpiGroups;
+    const int gc = c >> 5, g = gc % G, lane = c & 31;
     const Acc *p = reinterpret_cast<const Acc *>(partial);
     Acc sq = 0, sr = 0;
     for (int b = 0; b < ncta; ++b)
-        for (int w = 4 * q; w < 4 * q + 4; ++w) {
-            const Acc *e = p + (((long long)b * kProducerWarps + w) * 8 * 32 + g * 32 + lane) * 2;
+        for (int w = 4 * (gc / G); w < 4 * (gc / G) + 4; ++w) {
+            const Acc *e = p + (((long long)b * kProducerWarps + w) * G * 32 + g * 32 + lane) * 2;
             sq += e[0];
             sr += e[1];
         }
