@@ -145,7 +145,7 @@ __device__ __forceinline__ void cluster_sync_all()
 __device__ __forceinline__ uint32_t mapa_rank(uint32_t local, uint32_t rank)
 {
     uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
+    asm("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
     return r;
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr)
@@ -188,6 +188,18 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
                  "r"(smem_u32(bar))
                  : "memory");
+}
+// shared-memory accesses by 32-bit shared-space address (immediate offsets fold into the instruction)
+__device__ __forceinline__ float4 lds128(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts64(uint32_t a, uint2 v) { asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a), "r"(v.x), "r"(v.y) : "memory"); }
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 // hides a loop-invariant value from the optimiser (see the producer loop)
 __device__ __forceinline__ int keep(int x) { asm volatile("" : "+r"(x)); return x; }
@@ -409,11 +421,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct; SWIZZLE_64B; row
         // mrow0 + 16 r is 1024 r further) and B tile (j = jj, hi plane of column half qw, 16-byte chunk 2 l3 of the
         // 128-column row; SWIZZLE_128B; chunk 2 l3 + 1 is at address ^ 16, the lo plane 8192 further)
-        const int offA = keep((mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3));
-        const int offB = keep(kABytes + qw * 16384 + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4));
-        const int offJ = keep(kStages * kStageBytes + 4 * oct * NLD * 16);  // its four j pairs inside a record slot
-        const uint32_t full_remote0 = mapa_rank(smem_u32(&bar_full[0]), 0);
-        const uint32_t accempty_remote = mapa_rank(smem_u32(&bar_accempty), 0);
+        const int offA = (mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3);
+        const int offB = kABytes + qw * 16384 + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
+        const int offJ = kStages * kStageBytes + 4 * oct * NLD * 16;  // its four j pairs inside a record slot
+        // running shared-memory addresses of the current stage / record slot (advanced and wrapped every K block)
+        uint32_t paA = smem_u32(smem) + offA, pbB = smem_u32(smem) + offB, pjJ = smem_u32(smem) + offJ;
         uint32_t it = 0, un = 0;
         for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
             const Unit U = P.units[u];
@@ -439,14 +451,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             const int dthr = row0 + mrow0 - 8 * oct;
             // this thread's label word of K block kb (element index < 2^32), prefetched one block ahead into a register
             uint32_t im = (uint32_t)(U.kb_begin * kKB + jj) * (uint32_t)P.words_total + (uint32_t)(P.word0 + 8 * qw + 4 * (int)rank + l3);
-            const uint32_t im_step = (uint32_t)(kKB * P.words_total);
             uint32_t mw = __ldg(P.maskT + im);
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                uint8_t *st = smem + (it & (kStages - 1)) * kStageBytes;
-                const float4 *pj = reinterpret_cast<const float4 *>(smem + offJ + (it & (kRecSlots - 1)) * kRecSlotBytes);
                 const uint32_t mcur = mw;
                 if (kb + 1 < U.kb_end) {
-                    im += im_step;
+                    im += (uint32_t)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
                 }
                 mbar_wait(&bar_rec[it & (kRecSlots - 1)], (it / kRecSlots) & 1);
@@ -460,7 +469,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     float2 nu[2 * NLD];
 #pragma unroll
                     for (int qq = 0; qq < NLD; ++qq) {
-                        const float4 v = pj[tp * NLD + qq];
+                        const float4 v = lds128(pjJ + (tp * NLD + qq) * 16);
                         nu[2 * qq] = make_float2(v.x, v.y);
                         nu[2 * qq + 1] = make_float2(v.z, v.w);
                     }
@@ -487,7 +496,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                         for (int t = 0; t < 8; ++t)
                             if (x <= 16 * r - t) fq[r][t] = zero;
                 }
-                uint8_t *pa = st + offA;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const uint32_t p01 = __byte_perm(fq[r][0], fq[r][1], 0x5140), p23 = __byte_perm(fq[r][2], fq[r][3], 0x5140);
@@ -497,8 +505,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     lo.y = (__byte_perm(p45, p67, 0x5410) >> 1) & 0x7f7f7f7fu;
                     hi.x = __byte_perm(p01, p23, 0x7632);
                     hi.y = __byte_perm(p45, p67, 0x7632);
-                    *reinterpret_cast<uint2 *>(pa + 1024 * r) = hi;
-                    *reinterpret_cast<uint2 *>(pa + kTM * kKB + 1024 * r) = lo;
+                    sts64(paA + 1024 * r, hi);
+                    sts64(paA + kTM * kKB + 1024 * r, lo);
                 }
                 }
                 // ---- label tile: j = jj, this CTA's word 8 qw + 4 rank + l3 -> 32 columns; byte p of a word
@@ -507,16 +515,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     uint32_t a[8];
 #pragma unroll
                     for (int t = 0; t < 8; ++t) a[t] = (mcur >> t) & 0x01010101u;
-                    uint8_t *b0 = st + offB;
-                    uint8_t *b1 = smem + ((uint32_t)(b0 - smem) ^ 16u);
-                    *reinterpret_cast<uint4 *>(b0 + 8192) = make_uint4(a[0], a[1], a[2], a[3]);
-                    *reinterpret_cast<uint4 *>(b1 + 8192) = make_uint4(a[4], a[5], a[6], a[7]);
-                    *reinterpret_cast<uint4 *>(b0) = make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7);
-                    *reinterpret_cast<uint4 *>(b1) = make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7);
+                    const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
+                    sts128(pbB + 8192, make_uint4(a[0], a[1], a[2], a[3]));
+                    sts128(pbB1 + 8192, make_uint4(a[4], a[5], a[6], a[7]));
+                    sts128(pbB, make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7));
+                    sts128(pbB1, make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7));
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(full_remote0 + 8 * (it & (kStages - 1)));
+                if (lane == 0) mbar_arrive_cluster(mapa_rank(smem_u32(&bar_full[it & (kStages - 1)]), 0));
+                const bool wrapS = ((it + 1) & (kStages - 1)) == 0, wrapJ = ((it + 1) & (kRecSlots - 1)) == 0;
+                paA += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
+                pbB += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
+                pjJ += wrapJ ? kRecSlotBytes - kRecSlots * kRecSlotBytes : kRecSlotBytes;
             }
             // ---- epilogue of the unit: this CTA's 128 rows x 512 columns -------------------------------------
             mbar_wait(&bar_accfull, un & 1);
@@ -551,7 +562,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(accempty_remote);
+            if (lane == 0) mbar_arrive_cluster(mapa_rank(smem_u32(&bar_accempty), 0));
         }
         // per-warp partial column sums: partial[cta][warp][g][lane][2]; lane L of group g = TMEM column 32 (grp0 + g) + L
         Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * G * 32 * 2;
