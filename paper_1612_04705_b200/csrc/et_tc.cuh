@@ -125,6 +125,17 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
             : "memory");
     }
 }
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar_addr, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done)
+            : "r"(bar_addr), "r"(parity)
+            : "memory");
+    }
+}
 __device__ __forceinline__ void umma_commit(uint64_t *bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -322,7 +333,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    __shared__ uint64_t bar_full[kStages], bar_empty[kStages], bar_accfull, bar_accempty, bar_rec[kRecSlots];
+    // one array, so that the hot loop addresses every barrier as bar0 + constant + 8 * index
+    __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + kRecSlots];
+    uint64_t *const bar_full = bars_s, *const bar_empty = bars_s + kStages, *const bar_rec = bars_s + 2 * kStages + 2;
+    uint64_t &bar_accfull = bars_s[2 * kStages], &bar_accempty = bars_s[2 * kStages + 1];
     constexpr uint32_t kRecSlotBytes = (kKB / 2) * NLD * 16;
     uint8_t *recs = smem + kStages * kStageBytes;  // record ring
     __shared__ uint32_t tmem_base_s;
@@ -425,6 +439,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         const int offB = kABytes + qw * 16384 + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
         const int offJ = kStages * kStageBytes + 4 * oct * NLD * 16;  // its four j pairs inside a record slot
         // running shared-memory addresses of the current stage / record slot (advanced and wrapped every K block)
+        const uint32_t bar0 = smem_u32(bars_s);
         uint32_t paA = smem_u32(smem) + offA, pbB = smem_u32(smem) + offB, pjJ = smem_u32(smem) + offJ;
         uint32_t it = 0, un = 0;
         for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
@@ -458,8 +473,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     im += (uint32_t)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
                 }
-                mbar_wait(&bar_rec[it & (kRecSlots - 1)], (it / kRecSlots) & 1);
-                mbar_wait(&bar_empty[it & (kStages - 1)], ((it / kStages) & 1) ^ 1);
+                mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
+                mbar_wait_a(bar0 + 8 * kStages + 8 * (it & (kStages - 1)), ((it / kStages) & 1) ^ 1);
 
                 // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7 ------------------------------------
                 if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
@@ -513,17 +528,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 //      is label bit beta(p): register t = (m >> t) & 0x01010101 (bytes a), << 7 (bytes 128 a)
                 if (ET_TC_DBG != 1 && ET_TC_DBG != 3) {
                     uint32_t a[8];
+                    // both planes straight from the word: (m >> t) & 0x01.. and (m << (7 - t)) & 0x80.. (measured faster than
+                    // a << 7 from opaque a, and than SHF.L instead of the compiler's IMAD.SHL: profiles/r01c_README.md)
 #pragma unroll
                     for (int t = 0; t < 8; ++t) a[t] = (mcur >> t) & 0x01010101u;
+                    uint32_t h[8];
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) h[t] = (mcur << (7 - t)) & 0x80808080u;
                     const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
                     sts128(pbB + 8192, make_uint4(a[0], a[1], a[2], a[3]));
                     sts128(pbB1 + 8192, make_uint4(a[4], a[5], a[6], a[7]));
-                    sts128(pbB, make_uint4(a[0] << 7, a[1] << 7, a[2] << 7, a[3] << 7));
-                    sts128(pbB1, make_uint4(a[4] << 7, a[5] << 7, a[6] << 7, a[7] << 7));
+                    sts128(pbB, make_uint4(h[0], h[1], h[2], h[3]));
+                    sts128(pbB1, make_uint4(h[4], h[5], h[6], h[7]));
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(mapa_rank(smem_u32(&bar_full[it & (kStages - 1)]), 0));
+                if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * (it & (kStages - 1)), 0));
                 const bool wrapS = ((it + 1) & (kStages - 1)) == 0, wrapJ = ((it + 1) & (kRecSlots - 1)) == 0;
                 paA += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
                 pbB += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
