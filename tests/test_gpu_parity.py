@@ -360,3 +360,34 @@ def test_full_size_row_sum_parity(ctx, index):
     rx, rb = ctx.row_sums(s.x, s.xbar, c.sigma, rows, s.wx, s.wxbar)
     ex, eb = oracle.row_sums(s.x, s.xbar, c.sigma, rows, s.wx, s.wxbar)
     assert np.allclose(rx, ex, rtol=3e-6, atol=1e-6) and np.allclose(rb, eb, rtol=3e-6, atol=1e-6)
+
+
+def test_full_size_podd_tc_properties(ctx):
+    """BASELINE configs[4] in the launch configuration bench.py times (n = nbar = 10^6, 1000 permutations, tensor-core
+    path).  A from-scratch oracle T_p is 17 CPU-minutes each at this size, so: the split is compared with the oracle
+    bit for bit, the observed statistics of both labellings (columns 0 and 1 of K-PERM-TC) with the fp32/fp64
+    all-pairs kernel on the regrouped samples (itself pinned to the oracle at this size by the sampled row sums
+    above), and the permutation distribution through properties that hold at any size (pin P6: E_perm[T] = 0;
+    count = #{T_p > T_obs}; no two permutations alike)."""
+    c = dg.config(4)
+    s = dg.make_sample(c)
+    got = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, c.nperm, c.perm_seed)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
+    posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
+    I, II, III, IV = s.x[posx == 1], s.x[posx == 0], s.xbar[posb == 1], s.xbar[posb == 0]
+    assert got.count == (len(I), len(II), len(III), len(IV))
+    odd = ctx.T(np.vstack([I, IV]), np.vstack([II, III]), c.sigma)
+    even = ctx.T(s.x, s.xbar, c.sigma)
+    obs = got.p_odd.observed
+    for a, b in ((obs, odd), (got.p_even, even)):
+        scale = b.term_scale
+        assert abs(a.T - b.T) <= TOL * scale
+        assert abs(a.T_xx - b.T_xx) <= TOL * scale and abs(a.T_bb - b.T_bb) <= TOL * scale and abs(a.T_xb - b.T_xb) <= TOL * scale
+        assert a.W == b.W and a.Wbar == b.Wbar
+    Tp = got.p_odd.T_perm
+    assert len(Tp) == c.nperm and np.isfinite(Tp).all() and len(np.unique(Tp)) == c.nperm
+    assert got.p_odd.count_gt == int((Tp > obs.T).sum()) and got.p_odd.p_value == got.p_odd.count_gt / c.nperm
+    assert abs(Tp.mean()) <= 5.0 * Tp.std() / math.sqrt(c.nperm)     # pin P6, statistically
+    # the null spread of T scales like 1/N: a wrong normalisation or label count shows up as orders of magnitude
+    assert 1e-9 < Tp.std() < 1e-5 and got.p_odd.n_near <= 5
