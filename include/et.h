@@ -159,6 +159,28 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
                        int dim, et_dtype dtype, et_memspace mem, double sigma,
                        int64_t nperm, uint64_t seed, double *T_perm, et_podd_result *out);
 
+/* Result of et_T_bkg: Eq. 3 and its three normalised brackets, T = T_xx + T_bb - T_xb. */
+typedef struct {
+    double T, T_xx, T_bb, T_xb;
+    double S[10];       /* raw psi sums over unordered pairs (i < j within a sample, all pairs across), in the
+                           order XX, XBx, XXbar, XBxbar, BxBx, BxXbar, BxBxbar, XbarXbar, XbarBxbar, BxbarBxbar */
+    double w, wbar;     /* signal events in the main samples: n - b, nbar - bbar                             */
+    int64_t n_pairs;    /* unordered pairs evaluated                                                         */
+} et_bkg_result;
+
+/* Background-subtracted T of Eq. 3 (readings R8, R9): main
+ * samples x[n][dim], xbar[nbar][dim], background samples bx[bs][dim],
+ * bxbar[bsbar][dim] (all the same dtype and memory space), b and bbar the
+ * numbers of background events IN THE MAIN samples (real, >= 0).  All ten
+ * sample-pair sums come from one all-pairs pass over the four samples.
+ * ET_ERR_INVALID if a sample has < 2 events or b, bbar are negative or not
+ * finite; ET_ERR_DEGENERATE if n - b <= 1 or nbar - bbar <= 1.  With
+ * b = bbar = 0 the result is Eq. 2 of (x, xbar). */
+et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar,
+                   const void *bx, int64_t bs, const void *bxbar, int64_t bsbar,
+                   double b, double bbar, int dim, et_dtype dtype, et_memspace mem,
+                   double sigma, et_bkg_result *out);
+
 /* Test hook: the permutation labels of reading R4, bit-packed,
  * mask[i * ceil(nperm/32) + (p >> 5)] bit (p & 31) = 1 iff pooled event i is in
  * sample X of permutation p.  `mask` lives in `mem`. */

@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+           "et_T_weighted", "et_T_bkg", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
 
 
 class EtError(RuntimeError):
@@ -48,6 +48,11 @@ class _PermResult(C.Structure):
 
 class _PoddResult(C.Structure):
     _fields_ = [("count", C.c_int64 * 4), ("p_even", _Result), ("p_odd", _PermResult)]
+
+
+class _BkgResult(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("T", "T_xx", "T_bb", "T_xb")] + [("S", C.c_double * 10), ("w", C.c_double),
+                                                                        ("wbar", C.c_double), ("n_pairs", C.c_int64)]
 
 
 class _Stats(C.Structure):
@@ -89,6 +94,22 @@ class PoddResult:
     count: tuple
     p_even: Result
     p_odd: PermResult
+
+
+@dataclass
+class BkgResult:
+    T: float
+    T_xx: float
+    T_bb: float
+    T_xb: float
+    S: tuple  # XX, XBx, XXbar, XBxbar, BxBx, BxXbar, BxBxbar, XbarXbar, XbarBxbar, BxbarBxbar
+    w: float
+    wbar: float
+    n_pairs: int
+
+    @property
+    def term_scale(self) -> float:
+        return abs(self.T_xx) + abs(self.T_bb) + abs(self.T_xb)
 
 
 @dataclass
@@ -235,6 +256,18 @@ class Context:
         self._check(lib().et_T_weighted(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
                                         C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
         return _res(out)
+
+    def T_bkg(self, x, xbar, bx, bxbar, b: float, bbar: float, sigma: float) -> BkgResult:
+        """Eq. 3: background-sample-subtracted T (main samples x, xbar; background samples bx, bxbar)."""
+        ax, ab = _coords(x, xbar)
+        abx, abb = _coords(bx, bxbar)
+        if (abx.mem, abx.dtype, abx.shape[1]) != (ax.mem, ax.dtype, ax.shape[1]):
+            raise ValueError("background samples must share memory space, dtype and dim with the main samples")
+        out = _BkgResult()
+        self._check(lib().et_T_bkg(self._h, ax.ptr, C.c_int64(ax.shape[0]), ab.ptr, C.c_int64(ab.shape[0]), abx.ptr,
+                                   C.c_int64(abx.shape[0]), abb.ptr, C.c_int64(abb.shape[0]), C.c_double(b), C.c_double(bbar),
+                                   C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
+        return BkgResult(out.T, out.T_xx, out.T_bb, out.T_xb, tuple(out.S), out.w, out.wbar, out.n_pairs)
 
     # ---------------------------------------------------------------- permutation test
     def permutation_test(self, x, xbar, sigma: float, nperm: int, seed: int, wx=None, wxbar=None) -> PermResult:

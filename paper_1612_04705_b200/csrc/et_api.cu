@@ -538,6 +538,53 @@ __global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q,
 }
 
 // class weights into ctx->clsw (kMaxCls doubles)
+// Eq. 3 from the ten class-pair sums of the layout (X, Bx, Xbar, Bxbar) = classes (0, 1, 2, 3).
+// S[c1*4+c2] holds unordered pairs within a class (the printed sums over i != j are twice that) and all pairs across.
+struct DevBkg {
+    et_bkg_result r;
+    int status;
+};
+__global__ void k_stat_eq3(const double *__restrict__ S, double n, double nbar, double bs, double bsb, double b, double bbar,
+                           long long npairs, DevBkg *out)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    et_bkg_result r;
+    const int order[10] = {0, 1, 2, 3, 5, 6, 7, 10, 11, 15};
+    for (int k = 0; k < 10; ++k) r.S[k] = S[order[k]];
+    r.w = n - b;
+    r.wbar = nbar - bbar;
+    r.n_pairs = npairs;
+    if (!(r.w > 1.0) || !(r.wbar > 1.0)) {
+        r.T = r.T_xx = r.T_bb = r.T_xb = nan("");
+        out->r = r;
+        out->status = ET_ERR_DEGENERATE;
+        return;
+    }
+    const double t1 = 2.0 * S[0] - 2.0 * b / bs * S[1] + b * (b + 1.0) / (bs * (bs - 1.0)) * 2.0 * S[5];
+    const double t2 = 2.0 * S[10] - 2.0 * bbar / bsb * S[11] + bbar * (bbar + 1.0) / (bsb * (bsb - 1.0)) * 2.0 * S[15];
+    const double t3 = S[2] - bbar / bsb * S[3] - b / bs * S[6] + b * bbar / (bs * bsb) * S[7];
+    r.T_xx = t1 / (2.0 * r.w * (r.w - 1.0));
+    r.T_bb = t2 / (2.0 * r.wbar * (r.wbar - 1.0));
+    r.T_xb = t3 / (r.w * r.wbar);
+    r.T = r.T_xx + r.T_bb - r.T_xb;
+    out->r = r;
+    out->status = 0;
+}
+// src[row] for class segments that are consecutive runs of the pooled source index (class c = sources
+// seg_first[c] .. seg_first[c] + seg_count[c] - 1), -1 on padding rows
+__global__ void k_src_runs(PrepParams P, const long long *__restrict__ unused, int *__restrict__ src)
+{
+    for (long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x; row < P.npad; row += (long long)gridDim.x * blockDim.x) {
+        int v = -1;
+        long long first = 0;
+        for (int c = 0; c < P.ncls; ++c) {
+            if (row >= P.seg_pos[c] && row - P.seg_pos[c] < P.seg_count[c]) v = (int)(first + row - P.seg_pos[c]);
+            first += P.seg_count[c];
+        }
+        src[row] = v;
+    }
+}
+
 et_status run_class_weights(et_ctx *ctx, const Layout &L, int dim)
 {
     const int nt = (int)(L.npad / kPad);
@@ -955,6 +1002,53 @@ et_status et_T_weighted(et_ctx *ctx, const void *x, const double *wx, int64_t n,
     ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
     if (!out || !wx || !wxbar) return fail(ctx, ET_ERR_INVALID, "null weights or output");
     return do_T(ctx, x, wx, n, xbar, wxbar, nbar, dim, dtype, mem, sigma, out);
+}
+
+et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,
+                   const void *bxbar, int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem, double sigma,
+                   et_bkg_result *out)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!out || !bx || !bxbar) return fail(ctx, ET_ERR_INVALID, "null background sample or output");
+    if (bs < 2 || bsbar < 2) return fail(ctx, ET_ERR_INVALID, "background samples need >= 2 events (Eq. 3 divides by b_s(b_s-1)); got %lld, %lld", (long long)bs, (long long)bsbar);
+    if (n + nbar + bs + bsbar >= (1ll << 31)) return fail(ctx, ET_ERR_INVALID, "total number of events must be < 2^31");
+    if (!(b >= 0.0) || !(bbar >= 0.0) || !std::isfinite(b) || !std::isfinite(bbar)) return fail(ctx, ET_ERR_INVALID, "b and bbar must be finite and >= 0");
+    ET_TRY(begin_call(ctx));
+    // the x side of the pooled source index is [x ; bx], the xbar side [xbar ; bxbar]
+    const size_t row = (size_t)dim * elem_size(dtype);
+    ET_TRY(ensure(ctx, ctx->in_x, (size_t)(n + bs) * row));
+    ET_TRY(ensure(ctx, ctx->in_xbar, (size_t)(nbar + bsbar) * row));
+    char *sx = static_cast<char *>(ctx->in_x.p), *sb = static_cast<char *>(ctx->in_xbar.p);
+    const cudaMemcpyKind kind = mem == ET_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    CUDA_TRY(cudaMemcpyAsync(sx, x, (size_t)n * row, kind, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(sx + (size_t)n * row, bx, (size_t)bs * row, kind, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(sb, xbar, (size_t)nbar * row, kind, ctx->stream));
+    CUDA_TRY(cudaMemcpyAsync(sb + (size_t)nbar * row, bxbar, (size_t)bsbar * row, kind, ctx->stream));
+    if (mem == ET_HOST) CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // the caller's buffers may be pageable
+    Layout L;
+    const long long cnt[4] = {n, bs, nbar, bsbar};
+    layout_four(L, n + bs, nbar + bsbar, cnt);
+    ET_TRY(upload_tile_classes(ctx, L));
+    ET_TRY(ensure(ctx, ctx->src, (size_t)L.npad * sizeof(int)));
+    PrepParams PP{};
+    PP.npad = L.npad; PP.ncls = 4;
+    for (int c = 0; c <= 4; ++c) PP.seg_pos[c] = L.seg_pos[c];
+    for (int c = 0; c < 4; ++c) PP.seg_count[c] = L.seg_count[c];
+    k_src_runs<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(PP, nullptr, static_cast<int *>(ctx->src.p));
+    LAUNCH_CHECK();
+    ET_TRY(run_prep(ctx, sx, sb, nullptr, nullptr, static_cast<const int *>(ctx->src.p), L, dim, dtype, sigma));
+    ET_TRY(run_pairs_T(ctx, L, dim));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4 + sizeof(DevBkg)));
+    const long long Nall = n + nbar + bs + bsbar;
+    k_stat_eq3<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), (double)n, (double)nbar, (double)bs, (double)bsbar, b, bbar,
+                                          Nall * (Nall - 1) / 2, static_cast<DevBkg *>(ctx->result.p));
+    LAUNCH_CHECK();
+    DevBkg r;
+    ET_TRY(fetch(ctx, ctx->result.p, &r));
+    ET_TRY(end_call(ctx));
+    if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "Eq. 3 normalisation degenerate: w = n - b = %g, wbar = nbar - bbar = %g (need > 1)", r.r.w, r.r.wbar);
+    *out = r.r;
+    return ET_OK;
 }
 
 et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar,

@@ -279,3 +279,23 @@ def make_sample(cfg: Config) -> Sample:
         s.wx = _rng(3000 + cfg.index).uniform(-0.5, 1.5, cfg.n)
         s.wxbar = _rng(4000 + cfg.index).uniform(-0.5, 1.5, cfg.nbar)
     return s
+
+
+def make_bkg_sample(seed: int = 5000, n_sig: int = 4000, n_bkg: int = 1600, asym: float = 0.75, scale: float = 1.0):
+    """Inputs with the structure of the paper's Fig. 3 study for Eq. 3: `n_sig` signal events with a
+    random 50 % flavour, `n_bkg` background events flat over the Dalitz plot contaminating the main samples with a
+    3:1 flavour asymmetry, and `n_bkg` more with the same asymmetry as the background samples.  The paper's signal model
+    (its Ref. [13]) is not available: the stand-in signal is the bumped Dalitz density of the other configs (no CP
+    violation: both flavours are drawn from it).  Returns (x, xbar, bx, bxbar, b, bbar) with b, bbar the numbers of
+    background events that went into the main samples."""
+    rng = _rng(seed)
+    n_sig, n_bkg = max(8, int(n_sig * scale)), max(8, int(n_bkg * scale))
+    sig = dalitz_with_bump(n_sig, rng, 0.3)
+    fl = rng.random(n_sig) < 0.5
+    bkg = dalitz_uniform(n_bkg, rng)
+    flb = rng.random(n_bkg) < asym
+    side = dalitz_uniform(n_bkg, rng)
+    fls = rng.random(n_bkg) < asym
+    x = np.ascontiguousarray(np.vstack([sig[fl], bkg[flb]]))
+    xbar = np.ascontiguousarray(np.vstack([sig[~fl], bkg[~flb]]))
+    return x, xbar, np.ascontiguousarray(side[fls]), np.ascontiguousarray(side[~fls]), float(flb.sum()), float((~flb).sum())

@@ -55,3 +55,12 @@ def test_small_scaled_configs():
     assert s.mom_x.shape == (2000, 3, 3) and s.mom_xbar.shape == (2000, 3, 3)
     ct = np.einsum("ij,ij->i", s.mom_x[:, 0], np.cross(s.mom_x[:, 1], s.mom_x[:, 2]))
     assert 0.4 < (ct > 0).mean() < 0.6
+
+
+def test_bkg_sample_structure():
+    x, xb, bx, bb, b, bbar = dg.make_bkg_sample()
+    assert b + bbar == 1600 and len(bx) + len(bb) == 1600 and len(x) + len(xb) == 5600
+    assert 0.70 < b / 1600 < 0.80 and 0.70 < len(bx) / 1600 < 0.80  # 3:1 flavour asymmetry of the background
+    assert dg.dalitz_inside(x[:, 0], x[:, 1]).all() and dg.dalitz_inside(bb[:, 0], bb[:, 1]).all()
+    again = dg.make_bkg_sample()
+    assert (again[0] == x).all() and again[4] == b

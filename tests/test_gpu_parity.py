@@ -391,3 +391,58 @@ def test_full_size_podd_tc_properties(ctx):
     assert abs(Tp.mean()) <= 5.0 * Tp.std() / math.sqrt(c.nperm)     # pin P6, statistically
     # the null spread of T scales like 1/N: a wrong normalisation or label count shows up as orders of magnitude
     assert 1e-9 < Tp.std() < 1e-5 and got.p_odd.n_near <= 5
+
+
+# ----------------------------------------------------------------------------- Eq. 3 (NEXT-1)
+def assert_bkg_close(got, exp_T, scale):
+    assert abs(got.T - exp_T) <= TOL * scale, (got.T, exp_T)
+
+
+@pytest.mark.parametrize("scale,dtype", [(1.0, np.float64), (0.05, np.float64), (1.0, np.float32)])
+def test_T_bkg_matches_oracle(ctx, scale, dtype):
+    """Eq. 3 on inputs with the structure of the paper's Fig. 3 study (4000 signal, 1600 + 1600 background, 3:1
+    flavour asymmetry of the background, sigma = 0.25) against the oracle's Eq. 3 written out as printed."""
+    x, xb, bx, bb, b, bbar = (a.astype(dtype) if isinstance(a, np.ndarray) else a for a in dg.make_bkg_sample(scale=scale))
+    exp = oracle.T_bkg(x, xb, bx, bb, b, bbar, 0.25)
+    got = ctx.T_bkg(x, xb, bx, bb, b, bbar, 0.25)
+    assert got.w == len(x) - b and got.wbar == len(xb) - bbar
+    assert_bkg_close(got, exp, got.term_scale)
+    # the subtraction does something here: Eq. 2 on the contaminated main samples is far from Eq. 3
+    if scale == 1.0:
+        assert abs(ctx.T(x, xb, 0.25).T - got.T) > 100 * TOL * got.term_scale
+
+
+def test_T_bkg_reductions_and_sums(ctx):
+    rng = np.random.default_rng(77)
+    x, xb = rng.uniform(size=(700, 3)), rng.uniform(size=(1300, 3)) ** 1.1
+    bx, bb = rng.uniform(size=(90, 3)), rng.uniform(size=(2, 3))
+    # b = bbar = 0: Eq. 3 is Eq. 2 of the main samples
+    z = ctx.T_bkg(x, xb, bx, bb, 0.0, 0.0, 0.3)
+    t = ctx.T(x, xb, 0.3)
+    assert abs(z.T - t.T) <= TOL * t.term_scale and abs(z.S[0] - t.S_xx) <= 1e-9 * t.S_xx and abs(z.S[2] - t.S_xb) <= 1e-9 * t.S_xb
+    # the ten raw sums against the oracle's two-sample sums
+    names = {"x": x, "bx": bx, "xb": xb, "bb": bb}
+    order = [("x", "x"), ("x", "bx"), ("x", "xb"), ("x", "bb"), ("bx", "bx"), ("bx", "xb"), ("bx", "bb"), ("xb", "xb"), ("xb", "bb"), ("bb", "bb")]
+    g = ctx.T_bkg(x, xb, bx, bb, 31.5, 0.25, 0.3)
+    for k, (p, q) in enumerate(order):
+        o = oracle.T(names[p], names[q], 0.3)
+        e = o.S_xx if p == q else o.S_xb
+        assert abs(g.S[k] - e) <= 2e-6 * e, (p, q)
+    assert abs(g.T - oracle.T_bkg(x, xb, bx, bb, 31.5, 0.25, 0.3)) <= TOL * g.term_scale
+    # device pointers
+    import torch
+    d = [torch.from_numpy(a).cuda() for a in (x, xb, bx, bb)]
+    assert ctx.T_bkg(*d, 31.5, 0.25, 0.3).T == g.T
+
+
+def test_T_bkg_errors(ctx):
+    a = np.random.default_rng(1).uniform(size=(10, 2))
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_bkg(a, a, a[:1], a, 1.0, 1.0, 0.3)
+    assert e.value.status == -1
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_bkg(a, a, a, a, -1.0, 1.0, 0.3)
+    assert e.value.status == -1
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_bkg(a, a, a, a, 9.5, 1.0, 0.3)
+    assert e.value.status == -4
