@@ -799,7 +799,10 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     }
     ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
 
-    // unit table: 256-row tile I (one CTA pair) against K blocks [4 I, NK) in pieces of <= Lmax, longest first,
+    // unit table: 256-row tile I (one CTA pair) against K blocks [4 I, NK), cut at the GLOBAL boundaries m Lmax so that
+    // units of the same chunk m read the same label rows; full-length units go first, chunk by chunk (the ~74 clusters
+    // then stream one chunk of the label matrix together and it is served from L2: DRAM traffic per launch at config 4
+    // fell from 640 GB to the order of the matrix itself, profiles/r01d), then the shorter ones, longest first.
     // unit u -> cluster u % nclusters
     const int nclusters_max = ctx->num_sms / 2;
     const int nT = (int)(L.npad / tc::kTM2), NK = (int)(L.npad / tc::kKB);
@@ -809,9 +812,10 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     if (Lmax < 8) Lmax = 8;
     if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
     std::vector<tc::Unit> full, tail;
-    for (int I = 0; I < nT; ++I)
-        for (int kb = 4 * I; kb < NK; kb += (int)Lmax) {
-            tc::Unit u{I, kb, (int)std::min<long long>(NK, kb + Lmax), 0};
+    for (long long m = 0; m * Lmax < NK; ++m)
+        for (int I = 0; I < nT && 4ll * I < (m + 1) * Lmax; ++I) {
+            tc::Unit u{I, (int)std::max<long long>(4ll * I, m * Lmax), (int)std::min<long long>(NK, (m + 1) * Lmax), 0};
+            if (u.kb_end <= u.kb_begin) continue;
             (u.kb_end - u.kb_begin == Lmax ? full : tail).push_back(u);
         }
     std::stable_sort(tail.begin(), tail.end(), [](const tc::Unit &a, const tc::Unit &b) { return a.kb_end - a.kb_begin > b.kb_end - b.kb_begin; });
