@@ -446,3 +446,19 @@ def test_T_bkg_errors(ctx):
     with pytest.raises(binding.EtError) as e:
         ctx.T_bkg(a, a, a, a, 9.5, 1.0, 0.3)
     assert e.value.status == -4
+
+
+def test_full_size_config1_permutations_from_scratch(ctx):
+    """BASELINE configs[1] at full size (n = nbar = 100 000, fp32 coordinates, sigma = 0.3), default dispatch (tensor
+    cores): the observed T and the first three permutations against the oracle, each re-evaluated from scratch
+    (4 x 2e10 psi in fp64, about 40 s on 16 host cores); labels of those permutations bit for bit."""
+    c = dg.config(1)
+    s = dg.make_sample(c)
+    assert s.x.dtype == np.float32
+    nperm = 3
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, nperm, c.perm_seed)
+    got = ctx.permutation_test(s.x, s.xbar, 0.3, nperm, c.perm_seed)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    check_perm(got, exp)
+    N = c.n + c.nbar
+    assert (ctx.perm_labels(N, c.n, nperm, c.perm_seed) == oracle.labels(N, c.n, nperm, c.perm_seed)).all()
