@@ -477,71 +477,73 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
                 mbar_wait_a(bar0 + 8 * kStages + 8 * (it & (kStages - 1)), ((it / kStages) & 1) ^ 1);
 
-                // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7 ------------------------------------
-                if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
-                uint32_t fq[R][8];
+                // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7; label tile: j = jj, this CTA's word
+                //      8 qw + 4 rank + l3 -> 32 columns, byte p of a word is label bit beta(p): register t of the lo plane is
+                //      (m >> t) & 0x01010101 (bytes a), of the hi plane (m << (7 - t)) & 0x80808080 (bytes 128 a).
+                //      The four 16-byte label stores are issued between the four j pairs of the psi tile, so that the ALU-pipe
+                //      work of the expansion overlaps the FMA-pipe work of the distances (profiles/r01e).
+                const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
+                auto tile = [&](auto diag_tag) {
+                    constexpr bool DIAG = decltype(diag_tag)::value;
+                    const int x = kb * kKB - dthr;  // DIAG: element (r, t) is dropped when x <= 16 r - t
+                    uint32_t pk[R][4];              // (f_2tp, f_2tp+1) low halves: bytes lo', hi of two j
 #pragma unroll
-                for (int tp = 0; tp < 4; ++tp) {
-                    float2 nu[2 * NLD];
+                    for (int tp = 0; tp < 4; ++tp) {
+                        float2 nu[2 * NLD];
 #pragma unroll
-                    for (int qq = 0; qq < NLD; ++qq) {
-                        const float4 v = lds128(pjJ + (tp * NLD + qq) * 16);
-                        nu[2 * qq] = make_float2(v.x, v.y);
-                        nu[2 * qq + 1] = make_float2(v.z, v.w);
-                    }
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
-                        float2 e = __fmul2_rn(dd, dd);
-#pragma unroll
-                        for (int k = 1; k < D; ++k) {
-                            dd = __fadd2_rn(ui2[r][k], nu[k]);
-                            e = __ffma2_rn(dd, dd, e);
+                        for (int qq = 0; qq < NLD; ++qq) {
+                            const float4 v = lds128(pjJ + (tp * NLD + qq) * 16);
+                            nu[2 * qq] = make_float2(v.x, v.y);
+                            nu[2 * qq + 1] = make_float2(v.z, v.w);
                         }
-                        const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magicA);
-                        fq[r][2 * tp] = __float_as_uint(f2.x);
-                        fq[r][2 * tp + 1] = __float_as_uint(f2.y);
+                        if (ET_TC_DBG != 1 && ET_TC_DBG != 3) {
+                            uint32_t q[4];
+                            if (tp < 2) {
+#pragma unroll
+                                for (int t = 0; t < 4; ++t) q[t] = (mcur >> (4 * tp + t)) & 0x01010101u;
+                                sts128((tp == 0 ? pbB : pbB1) + 8192, make_uint4(q[0], q[1], q[2], q[3]));
+                            } else {
+#pragma unroll
+                                for (int t = 0; t < 4; ++t) q[t] = (mcur << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
+                                sts128(tp == 2 ? pbB : pbB1, make_uint4(q[0], q[1], q[2], q[3]));
+                            }
+                        }
+                        if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
+                                float2 e = __fmul2_rn(dd, dd);
+#pragma unroll
+                                for (int k = 1; k < D; ++k) {
+                                    dd = __fadd2_rn(ui2[r][k], nu[k]);
+                                    e = __ffma2_rn(dd, dd, e);
+                                }
+                                const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magicA);
+                                uint32_t f0 = __float_as_uint(f2.x), f1 = __float_as_uint(f2.y);
+                                if (DIAG) {
+                                    if (x <= 16 * r - 2 * tp) f0 = __float_as_uint(kMagic);
+                                    if (x <= 16 * r - 2 * tp - 1) f1 = __float_as_uint(kMagic);
+                                }
+                                pk[r][tp] = __byte_perm(f0, f1, 0x5140);
+                            }
+                        }
                     }
-                }
-                if (kb < kb_diag) {
-                    const uint32_t zero = __float_as_uint(kMagic);
-                    const int x = kb * kKB - dthr;
+                    if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
 #pragma unroll
-                    for (int r = 0; r < R; ++r)
-#pragma unroll
-                        for (int t = 0; t < 8; ++t)
-                            if (x <= 16 * r - t) fq[r][t] = zero;
-                }
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const uint32_t p01 = __byte_perm(fq[r][0], fq[r][1], 0x5140), p23 = __byte_perm(fq[r][2], fq[r][3], 0x5140);
-                    const uint32_t p45 = __byte_perm(fq[r][4], fq[r][5], 0x5140), p67 = __byte_perm(fq[r][6], fq[r][7], 0x5140);
-                    uint2 lo, hi;
-                    lo.x = (__byte_perm(p01, p23, 0x5410) >> 1) & 0x7f7f7f7fu;
-                    lo.y = (__byte_perm(p45, p67, 0x5410) >> 1) & 0x7f7f7f7fu;
-                    hi.x = __byte_perm(p01, p23, 0x7632);
-                    hi.y = __byte_perm(p45, p67, 0x7632);
-                    sts64(paA + 1024 * r, hi);
-                    sts64(paA + kTM * kKB + 1024 * r, lo);
-                }
-                }
-                // ---- label tile: j = jj, this CTA's word 8 qw + 4 rank + l3 -> 32 columns; byte p of a word
-                //      is label bit beta(p): register t = (m >> t) & 0x01010101 (bytes a), << 7 (bytes 128 a)
-                if (ET_TC_DBG != 1 && ET_TC_DBG != 3) {
-                    uint32_t a[8];
-                    // both planes straight from the word: (m >> t) & 0x01.. and (m << (7 - t)) & 0x80.. (measured faster than
-                    // a << 7 from opaque a, and than SHF.L instead of the compiler's IMAD.SHL: profiles/r01c_README.md)
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) a[t] = (mcur >> t) & 0x01010101u;
-                    uint32_t h[8];
-#pragma unroll
-                    for (int t = 0; t < 8; ++t) h[t] = (mcur << (7 - t)) & 0x80808080u;
-                    const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
-                    sts128(pbB + 8192, make_uint4(a[0], a[1], a[2], a[3]));
-                    sts128(pbB1 + 8192, make_uint4(a[4], a[5], a[6], a[7]));
-                    sts128(pbB, make_uint4(h[0], h[1], h[2], h[3]));
-                    sts128(pbB1, make_uint4(h[4], h[5], h[6], h[7]));
-                }
+                        for (int r = 0; r < R; ++r) {
+                            uint2 lo, hi;
+                            lo.x = (__byte_perm(pk[r][0], pk[r][1], 0x5410) >> 1) & 0x7f7f7f7fu;
+                            lo.y = (__byte_perm(pk[r][2], pk[r][3], 0x5410) >> 1) & 0x7f7f7f7fu;
+                            hi.x = __byte_perm(pk[r][0], pk[r][1], 0x7632);
+                            hi.y = __byte_perm(pk[r][2], pk[r][3], 0x7632);
+                            // row m = mrow0 + 16 r: 8-row group m >> 3 advances by 2 (1024 bytes), the swizzle phase is that of mrow0
+                            sts64(paA + 1024 * r, hi);
+                            sts64(paA + kTM * kKB + 1024 * r, lo);
+                        }
+                    }
+                };
+                if (kb < kb_diag) tile(std::true_type{});   // K block overlaps (or lies below) the rows of this CTA: keep only j > i
+                else tile(std::false_type{});
                 fence_async_smem();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * (it & (kStages - 1)), 0));
