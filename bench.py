@@ -253,6 +253,26 @@ def run_ours(args):
                                       if clocks.get("sm_mhz") else None),
             "peak_model": "min(128/(2D+1),16) pairs/clk/SM x 148 SMs x sm_max_mhz (FP32/SFU pipes)"}
 
+    # sigma scan (configs with several sigma values, BASELINE configs[1] / [3]): one fused pass against separate et_T calls
+    sigma_scan = None
+    if len(getattr(cfg, "sigmas", ()) or ()) > 1:
+        sg = list(cfg.sigmas)
+
+        def ms_of(fn, reps=3):
+            fn()
+            t = 0.0
+            for _ in range(reps):
+                fn()
+                t += ctx.stats().ms_total
+            return t / reps
+
+        fused = ms_of(lambda: ctx.T_sigmas(d["x"], d["xbar"], sg, d["wx"], d["wxbar"]))
+        if cfg.weighted:
+            sep = sum(ms_of(lambda v=v: ctx.T_weighted(d["x"], d["wx"], d["xbar"], d["wxbar"], v)) for v in sg)
+        else:
+            sep = sum(ms_of(lambda v=v: ctx.T(d["x"], d["xbar"], v)) for v in sg)
+        sigma_scan = {"sigmas": sg, "ms_fused": fused, "ms_separate": sep, "pair_sigma_evals_per_s": len(sg) * pairs / (fused * 1e-3)}
+
     # roofline of the dominant kernel of the step (the one with the largest share of ms_pairs)
     dom_ms = agg["ms_dom"] / (args.steps * max(agg["dom_launches"], 1))
     if agg["dom_kernel"].startswith("k_perm_tc"):
@@ -288,6 +308,7 @@ def run_ours(args):
         "effective_pairs_per_s": world * (cfg.nperm + 1) * pairs / (ms_step * 1e-3),  # what one pass per permutation would need
         "p_value": res.p_value, "T_obs": res.observed.T, "n_near": res.n_near,
         "et_T": et_T,
+        "sigma_scan": sigma_scan,
         "share_pairs_kernels": agg["ms_pairs"] / ms, "share_labels": agg["ms_labels"] / ms,
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / args.steps},

@@ -159,6 +159,17 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
                        int dim, et_dtype dtype, et_memspace mem, double sigma,
                        int64_t nperm, uint64_t seed, double *T_perm, et_podd_result *out);
 
+/* Eq. 2 (weighted if wx, wxbar are given; both NULL otherwise) for nsig <= ET_MAX_SIGMAS values of
+ * sigma from ONE pass over the pairs: the sigma scan of Sect. 2.2 (Fig. 2) evaluates the
+ * same samples at several sigma, and d_ij does not depend on sigma.  out[nsig] (host) receives one
+ * et_result per sigma, each within the tolerance of the corresponding et_T / et_T_weighted call.
+ * ET_ERR_SIGMA if a sigma is not finite and > 0 or two of them differ by more than a factor 1e6. */
+#define ET_MAX_SIGMAS 4
+et_status et_T_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n,
+                      const void *xbar, const double *wxbar, int64_t nbar,
+                      int dim, et_dtype dtype, et_memspace mem,
+                      const double *sigmas, int nsig, et_result *out);
+
 /* Result of et_T_bkg: Eq. 3 and its three normalised brackets, T = T_xx + T_bb - T_xb. */
 typedef struct {
     double T, T_xx, T_bb, T_xb;

@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_bkg", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
 
 
 class EtError(RuntimeError):
@@ -256,6 +256,19 @@ class Context:
         self._check(lib().et_T_weighted(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
                                         C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
         return _res(out)
+
+    def T_sigmas(self, x, xbar, sigmas, wx=None, wxbar=None) -> list:
+        """Eq. 2 (weighted if wx, wxbar are given) for up to four sigma values from one pass over the pairs."""
+        ax, ab = _coords(x, xbar)
+        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
+        if wx is not None and (awx.mem != ax.mem or awb.mem != ax.mem):
+            raise ValueError("weights must live where the coordinates live")
+        sg = np.ascontiguousarray(np.asarray(sigmas, dtype=np.float64))
+        out = (_Result * max(len(sg), 1))()
+        self._check(lib().et_T_sigmas(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
+                                      C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), sg.ctypes.data_as(C.c_void_p),
+                                      C.c_int(len(sg)), out))
+        return [_res(out[k]) for k in range(len(sg))]
 
     def T_bkg(self, x, xbar, bx, bxbar, b: float, bbar: float, sigma: float) -> BkgResult:
         """Eq. 3: background-sample-subtracted T (main samples x, xbar; background samples bx, bxbar)."""

@@ -325,6 +325,28 @@ et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim)
     return ET_OK;
 }
 
+// K-T for nsig sigmas in one pass (records scaled for sigmas[0]): class-pair sums into ctx->sums[s * kSumSlots + slot].
+template <int NS>
+et_status run_pairs_T_multi_ns(et_ctx *ctx, const Layout &L, int dim, const float *rho_dev)
+{
+    const int nT = (int)(L.npad / (kThreads * kRT));
+    const long long nunits = (long long)nT * (nT + 1) / 2;
+    DISPATCH_DIM(dim, {
+        int grid = resident_blocks(ctx, k_pairs_T_multi<D, kRT, NS>);
+        if ((long long)grid > nunits) grid = (int)nunits;
+        ET_TRY(ensure(ctx, ctx->partials, (size_t)grid * NS * kSumSlots * sizeof(double)));
+        k_pairs_T_multi<D, kRT, NS><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), nT,
+                                                                       static_cast<const uint8_t *>(ctx->tilecls.p), nunits, rho_dev,
+                                                                       static_cast<double *>(ctx->partials.p));
+        LAUNCH_CHECK();
+        k_reduce_cols<<<(NS * kSumSlots + 31) / 32, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partials.p), grid, NS * kSumSlots,
+                                                                         static_cast<double *>(ctx->sums.p));
+        LAUNCH_CHECK();
+    });
+    ctx->stats.pair_evals += nunits * (long long)(kThreads * kRT) * (kThreads * kRT);
+    return ET_OK;
+}
+
 // K-ROW: rowsum[c][row] for all rows.
 template <int C>
 et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
@@ -1006,6 +1028,60 @@ et_status et_T_weighted(et_ctx *ctx, const void *x, const double *wx, int64_t n,
     ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
     if (!out || !wx || !wxbar) return fail(ctx, ET_ERR_INVALID, "null weights or output");
     return do_T(ctx, x, wx, n, xbar, wxbar, nbar, dim, dtype, mem, sigma, out);
+}
+
+et_status et_T_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar, int64_t nbar,
+                      int dim, et_dtype dtype, et_memspace mem, const double *sigmas, int nsig, et_result *out)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!sigmas || !out) return fail(ctx, ET_ERR_INVALID, "null sigmas or output");
+    if (nsig < 1 || nsig > ET_MAX_SIGMAS) return fail(ctx, ET_ERR_INVALID, "nsig must be in 1..%d; got %d", ET_MAX_SIGMAS, nsig);
+    for (int s = 0; s < nsig; ++s) ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigmas[s]));
+    if ((wx == nullptr) != (wxbar == nullptr)) return fail(ctx, ET_ERR_INVALID, "weights: both NULL or both given");
+    if (nsig == 1) return do_T(ctx, x, wx, n, xbar, wxbar, nbar, dim, dtype, mem, sigmas[0], out);
+    // the exponent scale rho_s = (sigma_0 / sigma_s)^2 multiplies e (< 2^7 where psi matters): keep it within fp32 range
+    for (int s = 1; s < nsig; ++s) {
+        const double r = sigmas[0] / sigmas[s];
+        if (!(r * r < 1e12) || !(r * r > 1e-12)) return fail(ctx, ET_ERR_SIGMA, "sigmas differ by more than a factor 1e6");
+    }
+    ET_TRY(begin_call(ctx));
+    const void *dx, *dxb, *dwx, *dwb;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
+    ET_TRY(stage_in(ctx, wxbar, (size_t)nbar * 8, mem, ctx->in_wxbar, &dwb));
+    Layout L;
+    layout_two(L, n, nbar);
+    ET_TRY(upload_tile_classes(ctx, L));
+    ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigmas[0]));
+    ET_TRY(run_class_weights(ctx, L, dim));
+    ET_TRY(ensure(ctx, ctx->sums, (size_t)ET_MAX_SIGMAS * kSumSlots * sizeof(double) + 64));
+    float *rho_dev = reinterpret_cast<float *>(static_cast<double *>(ctx->sums.p) + ET_MAX_SIGMAS * kSumSlots);
+    ET_TRY(ensure_pinned(ctx, 4096));
+    float *rho_h = static_cast<float *>(ctx->pinned) + 512;
+    for (int s = 0; s < nsig; ++s) rho_h[s] = (float)((sigmas[0] / sigmas[s]) * (sigmas[0] / sigmas[s]));
+    CUDA_TRY(cudaMemcpyAsync(rho_dev, rho_h, nsig * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    ET_TRY(span_begin(ctx, 2));
+    if (nsig == 2) ET_TRY(run_pairs_T_multi_ns<2>(ctx, L, dim, rho_dev));
+    else if (nsig == 3) ET_TRY(run_pairs_T_multi_ns<3>(ctx, L, dim, rho_dev));
+    else ET_TRY(run_pairs_T_multi_ns<4>(ctx, L, dim, rho_dev));
+    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_T, 1, L.N * (L.N - 1) / 2 * (2 * dim + 1 + 2 * (nsig - 1))));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4 + sizeof(DevBkg)));
+    for (int s = 0; s < nsig; ++s) {
+        k_stat_from_sums<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p) + s * kSumSlots, static_cast<const double *>(ctx->clsw.p),
+                                                    2, 0x1u, pairs_two(n, nbar), static_cast<DevT *>(ctx->result.p) + s);
+        LAUNCH_CHECK();
+    }
+    DevT r[ET_MAX_SIGMAS];
+    ET_TRY(ensure_pinned(ctx, 4096));
+    CUDA_TRY(cudaMemcpyAsync(ctx->pinned, ctx->result.p, sizeof(DevT) * nsig, cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    memcpy(r, ctx->pinned, sizeof(DevT) * nsig);
+    ET_TRY(end_call(ctx));
+    for (int s = 0; s < nsig; ++s)
+        if (r[s].status != 0) return fail(ctx, ET_ERR_DEGENERATE, "weighted normalisation degenerate: W = %g, Wbar = %g (need > 1)", r[s].r.W, r[s].r.Wbar);
+    for (int s = 0; s < nsig; ++s) out[s] = r[s].r;
+    return ET_OK;
 }
 
 et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,

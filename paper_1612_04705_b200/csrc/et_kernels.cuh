@@ -259,6 +259,125 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
     if (tid < kSumSlots) partials[(long long)blockIdx.x * kSumSlots + tid] = s_sum[tid];
 }
 
+// K-T for several sigma at once (the sigma scan of PAPER.md:73-81): the records are scaled for
+// sigma_0, e = |u_i - u_j|^2 is evaluated once per pair and psi_s = 2^(-e rho_s), rho_s = (sigma_0 / sigma_s)^2, costs
+// one FMUL2, two MUFU.EX2 and one FFMA2 per extra sigma and pair of j instead of the 2D packed distance instructions.
+// Same tiling, precision rules and reduction order as k_pairs_T; partials[block][s][slot].
+template <int D, int R, int NS>
+__global__ void __launch_bounds__(kThreads) k_pairs_T_multi(const float *__restrict__ rec, int nT,
+                                                           const uint8_t *__restrict__ tile_cls, long long nunits,
+                                                           const float *__restrict__ rho, double *__restrict__ partials)
+{
+    constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
+    constexpr int NP = D + 1, NLD = (NP + 1) / 2;
+    __shared__ float4 sj[kTileJ / 2 * NLD];
+    __shared__ double s_sum[NS][kSumSlots];
+    __shared__ double s_warp[NS][kThreads / 32];
+    const int tid = threadIdx.x;
+    for (int k = tid; k < NS * kSumSlots; k += kThreads) s_sum[k / kSumSlots][k % kSumSlots] = 0.0;
+    float2 nrho[NS];  // -rho_s duplicated (nrho[0] unused: rho_0 = 1)
+#pragma unroll
+    for (int s = 0; s < NS; ++s) nrho[s] = make_float2(-rho[s], -rho[s]);
+
+    for (long long unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+        int I, J;
+        unit_to_pair(unit, nT, I, J);
+        float2 ui[R][D];
+        float wi[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
+            float v[F];
+#pragma unroll
+            for (int q = 0; q < F4; ++q) {
+                const float4 t = __ldg(p + q);
+                v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+            }
+#pragma unroll
+            for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
+            wi[r] = v[D];
+        }
+        double racc[NS][R];
+#pragma unroll
+        for (int s = 0; s < NS; ++s)
+#pragma unroll
+            for (int r = 0; r < R; ++r) racc[s][r] = 0.0;
+
+        for (int sub = 0; sub < TI / kTileJ; ++sub) {
+            __syncthreads();
+            {
+                const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)J * TI + sub * kTileJ + tid) * F);
+                float v[F];
+#pragma unroll
+                for (int q = 0; q < F4; ++q) {
+                    const float4 t = __ldg(p + q);
+                    v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+                }
+                float *o = reinterpret_cast<float *>(sj) + (tid >> 1) * (NLD * 4) + (tid & 1);
+#pragma unroll
+                for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
+                o[2 * D] = v[D];
+                if (NP & 1) o[2 * NP] = 0.f;
+            }
+            __syncthreads();
+            float2 acc[NS][R];
+#pragma unroll
+            for (int s = 0; s < NS; ++s)
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[s][r] = make_float2(0.f, 0.f);
+#pragma unroll 2
+            for (int jp = 0; jp < kTileJ / 2; ++jp) {
+                float2 nu[2 * NLD];
+#pragma unroll
+                for (int q = 0; q < NLD; ++q) {
+                    const float4 t = sj[jp * NLD + q];
+                    nu[2 * q] = make_float2(t.x, t.y);
+                    nu[2 * q + 1] = make_float2(t.z, t.w);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    float2 d = __fadd2_rn(ui[r][0], nu[0]);
+                    float2 e = __fmul2_rn(d, d);
+#pragma unroll
+                    for (int k = 1; k < D; ++k) {
+                        d = __fadd2_rn(ui[r][k], nu[k]);
+                        e = __ffma2_rn(d, d, e);
+                    }
+                    acc[0][r] = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], acc[0][r]);
+#pragma unroll
+                    for (int s = 1; s < NS; ++s) {
+                        const float2 es = __fmul2_rn(e, nrho[s]);
+                        acc[s][r] = __ffma2_rn(make_float2(ex2_approx(es.x), ex2_approx(es.y)), nu[D], acc[s][r]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int s = 0; s < NS; ++s)
+#pragma unroll
+                for (int r = 0; r < R; ++r) racc[s][r] += (double)acc[s][r].x + (double)acc[s][r].y;
+        }
+        const bool diag = I == J;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            double t = 0.0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) t += (double)wi[r] * (diag ? racc[s][r] - (double)wi[r] : racc[s][r]);
+            if (diag) t *= 0.5;
+            t = warp_sum(t);
+            if ((tid & 31) == 0) s_warp[s][tid >> 5] = t;
+        }
+        __syncthreads();
+        if (tid < NS) {
+            double sum = 0.0;
+#pragma unroll
+            for (int w = 0; w < kThreads / 32; ++w) sum += s_warp[tid][w];
+            s_sum[tid][tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad]] += sum;
+        }
+    }
+    __syncthreads();
+    for (int k = tid; k < NS * kSumSlots; k += kThreads) partials[(long long)blockIdx.x * NS * kSumSlots + k] = s_sum[k / kSumSlots][k % kSumSlots];
+}
+
 // K-ROW: full row sums by class of j, rowsum[c][i] = sum_{j in class c, j != i} w_j psi_ij, for every pooled row.
 // Work unit = one i-tile of 256*R rows against all j; units handed out by an atomic counter (each row is summed by
 // one CTA in a fixed j order, so the result does not depend on the schedule).

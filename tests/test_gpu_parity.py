@@ -462,3 +462,38 @@ def test_full_size_config1_permutations_from_scratch(ctx):
     check_perm(got, exp)
     N = c.n + c.nbar
     assert (ctx.perm_labels(N, c.n, nperm, c.perm_seed) == oracle.labels(N, c.n, nperm, c.perm_seed)).all()
+
+
+# ----------------------------------------------------------------------------- sigma scan in one pass (NEXT-3)
+@pytest.mark.parametrize("dim,sigmas", [(2, (0.1, 0.3, 0.5)), (5, (0.2, 0.1)), (3, (0.5, 0.25, 1.0, 0.125)), (2, (0.3,))])
+def test_T_sigmas_matches_oracle(ctx, dim, sigmas):
+    """BASELINE configs[1] evaluates sigma in {0.1, 0.3, 0.5} on the same samples: one pass, one distance per pair."""
+    if dim == 2:
+        s = dg.make_sample(dg.config(1, scale=0.04))  # 4000 + 4000 events, fp32 coordinates
+        x, xb = s.x, s.xbar
+    else:
+        rng = np.random.default_rng(dim)
+        x, xb = rng.uniform(size=(1500, dim)), rng.uniform(size=(2100, dim)) ** 1.2
+    got = ctx.T_sigmas(x, xb, sigmas)
+    assert len(got) == len(sigmas)
+    for g, sg in zip(got, sigmas):
+        assert_T_close(g, oracle.T(x, xb, sg))
+        one = ctx.T(x, xb, sg)
+        assert abs(g.T - one.T) <= TOL * one.term_scale
+
+
+def test_T_sigmas_weighted_and_errors(ctx):
+    c = dg.config(3, scale=0.01)
+    s = dg.make_sample(c)
+    got = ctx.T_sigmas(s.x, s.xbar, (0.3, 0.5, 0.1), s.wx, s.wxbar)
+    for g, sg in zip(got, (0.3, 0.5, 0.1)):
+        assert_T_close(g, oracle.T(s.x, s.xbar, sg, s.wx, s.wxbar))
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_sigmas(s.x, s.xbar, (0.3, -1.0))
+    assert e.value.status == -2
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_sigmas(s.x, s.xbar, (0.3, 0.2, 0.1, 0.4, 0.5))
+    assert e.value.status == -1
+    with pytest.raises(binding.EtError) as e:
+        ctx.T_sigmas(s.x, s.xbar, (1e-9, 1e3))
+    assert e.value.status == -2
