@@ -316,6 +316,16 @@ def run_ours(args):
         "clocks": clocks,
         "roofline": roofline,
     }
+    if world > 1:
+        # the ranks' permutation windows form ONE test of world * nperm permutations (sharding.py; no data-path collective)
+        try:
+            from paper_1612_04705_b200 import sharding
+
+            comb = sharding.all_gather_combine(sharding.Shard(rank * cfg.nperm, float(res.observed.T), np.asarray(res.T_perm),
+                                                              int(res.count_gt), int(res.n_near)))
+            out["combined"] = {"nperm": comb.nperm, "count_gt": comb.count_gt, "p_value": comb.p_value, "n_near": comb.n_near}
+        except Exception as exc:  # the timing line must not depend on the gather
+            out["combined"] = {"error": repr(exc)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(s, cfg, sigma, args.cpu_rows)
     if rank == 0:
