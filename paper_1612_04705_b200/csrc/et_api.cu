@@ -640,7 +640,7 @@ et_status do_T(et_ctx *ctx, const void *x, const double *wx, int64_t n, const vo
                int dim, et_dtype dtype, et_memspace mem, double sigma, et_result *out)
 {
     ET_TRY(begin_call(ctx));
-    const void *dx, *dxb, *dwx, *dwb;
+    const void *dx = nullptr, *dxb = nullptr, *dwx = nullptr, *dwb = nullptr;
     ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
     ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
     ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
@@ -1045,7 +1045,7 @@ et_status et_T_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n, c
         if (!(r * r < 1e12) || !(r * r > 1e-12)) return fail(ctx, ET_ERR_SIGMA, "sigmas differ by more than a factor 1e6");
     }
     ET_TRY(begin_call(ctx));
-    const void *dx, *dxb, *dwx, *dwb;
+    const void *dx = nullptr, *dxb = nullptr, *dwx = nullptr, *dwb = nullptr;
     ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
     ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
     ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
@@ -1140,7 +1140,7 @@ et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int6
     if ((wx == nullptr) != (wxbar == nullptr)) return fail(ctx, ET_ERR_INVALID, "give both weight arrays or neither");
     if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
     ET_TRY(begin_call(ctx));
-    const void *dx, *dxb, *dwx, *dwb;
+    const void *dx = nullptr, *dxb = nullptr, *dwx = nullptr, *dwb = nullptr;
     ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
     ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
     ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
@@ -1198,7 +1198,7 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
     if (!out || !T_perm || !mom_x || !mom_xbar) return fail(ctx, ET_ERR_INVALID, "null pointer");
     if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
     ET_TRY(begin_call(ctx));
-    const void *dx, *dxb, *dmx, *dmb;
+    const void *dx = nullptr, *dxb = nullptr, *dmx = nullptr, *dmb = nullptr;
     ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
     ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
     ET_TRY(stage_in(ctx, mom_x, (size_t)n * 72, mem, ctx->in_mx, &dmx));
@@ -1326,7 +1326,7 @@ et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n, c
     for (int64_t k = 0; k < nrows; ++k)
         if (rows[k] < 0 || rows[k] >= n + nbar) return fail(ctx, ET_ERR_INVALID, "row index out of range");
     ET_TRY(begin_call(ctx));
-    const void *dx, *dxb, *dwx, *dwb;
+    const void *dx = nullptr, *dxb = nullptr, *dwx = nullptr, *dwb = nullptr;
     ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
     ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
     ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
