@@ -751,12 +751,13 @@ __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__
     __syncthreads();
     const double Tobs = obs.r.T;
     // guard band (reading R5): 1e-9 of the term scale plus 8 sigma of the quantisation noise of T_p - T_obs; every
-    // pair carries an independent rounding error of variance qstep^2 / 12, so
-    // var(T) = qstep^2/12 [ pairs_xx / (W(W-1))^2 + pairs_bb / (Wb(Wb-1))^2 + pairs_xb / (W Wb)^2 ].
+    // pair carries an independent rounding error of variance (7/48) qstep^2 (round to 16 bits: 1/48; the dithered halving
+    // v = (u + k) >> 1 adds +-1/2 for odd u: 1/8), so
+    // var(T) = (7/48) qstep^2 [ pairs_xx / (W(W-1))^2 + pairs_bb / (Wb(Wb-1))^2 + pairs_xb / (W Wb)^2 ].
     const double Wo = obs.r.W, Wb = obs.r.Wbar;
     const double var = 0.5 * nA * (nA - 1.0) / ((Wo * (Wo - 1.0)) * (Wo * (Wo - 1.0))) + 0.5 * nB * (nB - 1.0) / ((Wb * (Wb - 1.0)) * (Wb * (Wb - 1.0))) +
                        nA * nB / ((Wo * Wb) * (Wo * Wb));
-    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb)) + 8.0 * 1.4142135623730951 * qstep * sqrt(var / 12.0);
+    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb)) + 8.0 * 1.4142135623730951 * qstep * sqrt(var * (7.0 / 48.0));
     unsigned long long cnt = 0, near = 0;
     for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
         const int k = (p / tc::kPermsPerChunk) * tc::kCols + tc::kSpecial + p % tc::kPermsPerChunk;

@@ -497,3 +497,23 @@ def test_T_sigmas_weighted_and_errors(ctx):
     with pytest.raises(binding.EtError) as e:
         ctx.T_sigmas(s.x, s.xbar, (1e-9, 1e3))
     assert e.value.status == -2
+
+
+@pytest.mark.parametrize("n,nbar,nperm", [(2, 3, 7), (300, 340, 1), (300, 340, 509), (300, 340, 510), (257, 1023, 1019)])
+def test_perm_tc_chunk_and_size_edges(ctx, n, nbar, nperm):
+    """Tensor-core path forced at its edges: the smallest samples, one permutation, and permutation counts on both
+    sides of the 509-per-launch boundary (1, 2 and 3 launches of 512 label columns).  Below the default dispatch
+    threshold (16384 rows) the 15-bit quantisation noise of psi does not average out: the bound used here is 8 sigma of
+    DESIGN.md section 6, var(T) = (7/48) q^2 [1/(2n(n-1)) + 1/(2nbar(nbar-1)) + 1/(n nbar)] with q = 1 / 32767, or the
+    north-star tolerance if that is larger."""
+    rng = np.random.default_rng(n * 1000 + nperm)
+    x, xb = rng.normal(size=(n, 4)), rng.normal(size=(nbar, 4)) * 1.1 + 0.05
+    exp = oracle.perm_test(x, xb, 0.8, nperm, 99)
+    with force_kernel(ctx, 2):
+        got = ctx.permutation_test(x, xb, 0.8, nperm, 99)
+        assert ctx.stats().dominant_kernel == "k_perm_tc"
+    var = (7.0 / 48.0) / 32767.0 ** 2 * (0.5 / (n * (n - 1.0)) + 0.5 / (nbar * (nbar - 1.0)) + 1.0 / (n * nbar))
+    bound = max(TOL * exp.observed.term_scale, 8.0 * math.sqrt(var))
+    assert abs(got.observed.T - exp.observed.T) <= bound
+    assert np.abs(got.T_perm - exp.T_perm).max() <= bound and got.nperm == nperm
+    assert abs(got.count_gt - exp.count_gt) <= got.n_near
