@@ -517,3 +517,16 @@ def test_perm_tc_chunk_and_size_edges(ctx, n, nbar, nperm):
     assert abs(got.observed.T - exp.observed.T) <= bound
     assert np.abs(got.T_perm - exp.T_perm).max() <= bound and got.nperm == nperm
     assert abs(got.count_gt - exp.count_gt) <= got.n_near
+
+
+@pytest.mark.parametrize("dim", [1, 4, 6, 7])
+def test_perm_tc_remaining_dims(ctx, dim):
+    """Every pair-record width of K-PERM-TC (1 to 5 float4 per j pair): dims not covered by test_perm_tc_matches_oracle."""
+    rng = np.random.default_rng(40 + dim)
+    x, xb = rng.uniform(size=(1100, dim)), rng.uniform(size=(1300, dim)) ** 1.3
+    sigma = 0.2 * math.sqrt(dim)
+    exp = oracle.perm_test(x, xb, sigma, 20, 5)
+    with force_kernel(ctx, 2):
+        got = ctx.permutation_test(x, xb, sigma, 20, 5)
+        assert ctx.stats().dominant_kernel == "k_perm_tc"
+    check_perm(got, exp)
