@@ -28,7 +28,7 @@
 #include "et_kernels.cuh"
 
 #ifndef ET_TC_DBG
-#define ET_TC_DBG 0  // timing experiments only (_work probes): 1 no tile generation, 2 no MMAs, 3 no label tile, 4 no psi tile
+#define ET_TC_DBG 0  // timing experiments only (_work probes): 1 no tile generation, 2 no MMAs, 3 no label tile, 4 no psi tile, 5 half of the psi tile
 #endif
 
 namespace et {
@@ -511,6 +511,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                         if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
+                                if (ET_TC_DBG == 5 && r > 0) { pk[r][tp] = pk[0][tp]; continue; }  // experiment: half the psi work
                                 float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
                                 float2 e = __fmul2_rn(dd, dd);
 #pragma unroll
