@@ -530,3 +530,18 @@ def test_perm_tc_remaining_dims(ctx, dim):
         got = ctx.permutation_test(x, xb, sigma, 20, 5)
         assert ctx.stats().dominant_kernel == "k_perm_tc"
     check_perm(got, exp)
+
+
+def test_perm_tc_bit_reproducible_many_units(ctx):
+    """N = 60 000 pooled events through the default dispatch: hundreds of work units over all 74 clusters, two launches.
+    Integer accumulation and fixed-order reductions: two calls agree bit for bit, and a second context does too."""
+    c = dg.config(2, scale=0.1)
+    s = dg.make_sample(c)
+    a = ctx.permutation_test(s.x, s.xbar, c.sigma, 600, 11)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    b = ctx.permutation_test(s.x, s.xbar, c.sigma, 600, 11)
+    assert (a.T_perm == b.T_perm).all() and a.observed.T == b.observed.T and a.count_gt == b.count_gt
+    with binding.Context(0) as other:
+        d = other.permutation_test(s.x, s.xbar, c.sigma, 600, 11)
+    assert (a.T_perm == d.T_perm).all() and a.observed.T == d.observed.T
+    assert abs(a.observed.T - ctx.T(s.x, s.xbar, c.sigma).T) <= TOL * a.observed.term_scale
