@@ -273,6 +273,13 @@ def run_ours(args):
             sep = sum(ms_of(lambda v=v: ctx.T(d["x"], d["xbar"], v)) for v in sg)
         sigma_scan = {"sigmas": sg, "ms_fused": fused, "ms_separate": sep, "pair_sigma_evals_per_s": len(sg) * pairs / (fused * 1e-3)}
 
+    # GEV fit of this step's permutation T values: the p-value where counting gives 0 (host-only, ~ms)
+    try:
+        g = binding.gev_pvalue(res.T_perm, res.observed.T, np.random.default_rng(12345).standard_normal((2000, 3)))
+        gev = {"p_value": g.p_value, "p_lo": g.p_lo, "p_hi": g.p_hi, "mu": g.mu, "sigma": g.sigma, "xi": g.xi, "converged": g.converged}
+    except binding.EtError as exc:
+        gev = {"error": str(exc)}
+
     # roofline of the dominant kernel of the step (the one with the largest share of ms_pairs)
     dom_ms = agg["ms_dom"] / (args.steps * max(agg["dom_launches"], 1))
     if agg["dom_kernel"].startswith("k_perm_tc"):
@@ -307,6 +314,7 @@ def run_ours(args):
         "pair_perm_updates_per_s": world * cfg.nperm * pairs / (ms_step * 1e-3),
         "effective_pairs_per_s": world * (cfg.nperm + 1) * pairs / (ms_step * 1e-3),  # what one pass per permutation would need
         "p_value": res.p_value, "T_obs": res.observed.T, "n_near": res.n_near,
+        "gev": gev,
         "et_T": et_T,
         "sigma_scan": sigma_scan,
         "share_pairs_kernels": agg["ms_pairs"] / ms, "share_labels": agg["ms_labels"] / ms,

@@ -192,6 +192,32 @@ et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int6
                    double b, double bbar, int dim, et_dtype dtype, et_memspace mem,
                    double sigma, et_bkg_result *out);
 
+/* GEV fit of the permutation T values ("the permutation T distribution can be fitted with a
+ * generalised-extreme-value (GEV) function ... The p-value from the fitted T distribution can be calculated as
+ * the fraction of the integral of the function above the observed T value"; its uncertainty "by
+ * randomly resampling the fit parameters within their uncertainties, taking into account their correlations").
+ * F(x) = exp(-t^(-1/xi)), t = 1 + xi (x - mu) / sigma  (xi -> 0: Gumbel; xi > 0 is the heavy upper tail). */
+typedef struct {
+    double mu, sigma, xi;     /* maximum-likelihood location, scale, shape                                    */
+    double cov[9];            /* covariance of (mu, sigma, xi), row-major: inverse observed information; NaN if
+                                 it is not positive definite                                                   */
+    double nll;               /* negative log-likelihood at the optimum                                        */
+    double p_value;           /* 1 - F(T_obs) of the fitted function                                           */
+    double p_lo, p_med, p_hi; /* 15.9 %, 50 %, 84.1 % quantiles of the p-values of the resampled parameter sets
+                                 (NaN if nresample == 0 or no covariance)                                      */
+    int64_t n_used;           /* finite T_perm values that entered the fit                                     */
+    int64_t converged;        /* 1: simplex restarts agree and the covariance is positive definite             */
+    int64_t n_resampled;      /* parameter sets with sigma > 0 that entered the quantiles                      */
+} et_gev_result;
+
+/* Host-only post-processing, O(nperm): all pointers are host memory, no context and no GPU work.  T_perm[nperm]
+ * as returned by et_permutation_test / et_podd_test (non-finite entries are skipped; >= 10 finite values with
+ * non-zero spread are required, else ET_ERR_DEGENERATE).  z[nresample][3] are the caller's standard normal
+ * draws for the parameter resampling theta = theta_hat + L z, cov = L L^T (nresample may be 0, z NULL): the
+ * library draws no random numbers here, so the result is a pure function of its inputs. */
+et_status et_gev_pvalue(const double *T_perm, int64_t nperm, double T_obs,
+                        const double *z, int64_t nresample, et_gev_result *out);
+
 /* Test hook: the permutation labels of reading R4, bit-packed,
  * mask[i * ceil(nperm/32) + (p >> 5)] bit (p & 31) = 1 iff pooled event i is in
  * sample X of permutation p.  `mask` lives in `mem`. */

@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
 
 
 class EtError(RuntimeError):
@@ -53,6 +53,12 @@ class _PoddResult(C.Structure):
 class _BkgResult(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("T", "T_xx", "T_bb", "T_xb")] + [("S", C.c_double * 10), ("w", C.c_double),
                                                                         ("wbar", C.c_double), ("n_pairs", C.c_int64)]
+
+
+class _GevResult(C.Structure):
+    _fields_ = ([(k, C.c_double) for k in ("mu", "sigma", "xi")] + [("cov", C.c_double * 9)] +
+                [(k, C.c_double) for k in ("nll", "p_value", "p_lo", "p_med", "p_hi")] +
+                [(k, C.c_int64) for k in ("n_used", "converged", "n_resampled")])
 
 
 class _Stats(C.Structure):
@@ -110,6 +116,38 @@ class BkgResult:
     @property
     def term_scale(self) -> float:
         return abs(self.T_xx) + abs(self.T_bb) + abs(self.T_xb)
+
+
+@dataclass
+class GevResult:
+    mu: float
+    sigma: float
+    xi: float
+    cov: np.ndarray
+    nll: float
+    p_value: float
+    p_lo: float
+    p_med: float
+    p_hi: float
+    n_used: int
+    converged: bool
+    n_resampled: int
+
+
+def gev_pvalue(T_perm, T_obs: float, z=None) -> GevResult:
+    """GEV fit of the permutation T values and the fitted p-value of T_obs (host-only; z: [nresample, 3] standard
+    normal draws for the parameter resampling, or None)."""
+    tp = np.ascontiguousarray(np.asarray(T_perm, dtype=np.float64))
+    zz = None if z is None else np.ascontiguousarray(np.asarray(z, dtype=np.float64).reshape(-1, 3))
+    out = _GevResult()
+    L = lib()
+    L.et_gev_pvalue.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_int64, C.c_void_p]
+    st = L.et_gev_pvalue(tp.ctypes.data_as(C.c_void_p), len(tp), float(T_obs), None if zz is None else zz.ctypes.data_as(C.c_void_p),
+                         0 if zz is None else len(zz), C.byref(out))
+    if st != ET_OK:
+        raise EtError(st, "et_gev_pvalue: needs >= 10 finite permutation T values with non-zero spread and a finite T_obs")
+    return GevResult(out.mu, out.sigma, out.xi, np.array(out.cov).reshape(3, 3), out.nll, out.p_value, out.p_lo, out.p_med,
+                     out.p_hi, out.n_used, bool(out.converged), out.n_resampled)
 
 
 @dataclass
