@@ -199,3 +199,27 @@ def T_bkg(x, xbar, bx, bxbar, b: float, bbar: float, sigma: float) -> float:
                             C.c_double(sigma), C.byref(out))
     _check(rc, "oracle_T_bkg")
     return float(out.value)
+
+
+BKG_SEED_XOR = 0x9E3779B97F4A7C15  # reading R18: the background pool draws from the stream of seed ^ this constant
+
+
+def bkg_perm_test(x, xbar, bx, bxbar, b: float, bbar: float, sigma: float, nperm: int, seed: int):
+    """Permutation test with Eq. 3 as the statistic ("using the same method to remove background from the
+    randomly permuted samples"; reading R18).  Permutation p reassigns the pooled main events to main samples of sizes
+    (n, nbar) with the labels of reading R4 from `seed`, and the pooled background-sample events to samples of sizes
+    (bs, bsbar) with the labels from `seed ^ BKG_SEED_XOR`; a random flavour gives both main samples the same purity, so
+    the permuted samples are evaluated with b' = (b + bbar) n / (n + nbar), bbar' = (b + bbar) nbar / (n + nbar).
+    Every T_p is Eq. 3 from scratch (`T_bkg`).  Returns (T_obs, T_perm, count_gt, p_value)."""
+    x, xbar, bx, bxbar = (np.atleast_2d(_f64(a)) for a in (x, xbar, bx, bxbar))
+    n, nbar, bs, bsbar = len(x), len(xbar), len(bx), len(bxbar)
+    t_obs = T_bkg(x, xbar, bx, bxbar, b, bbar, sigma)
+    main, side = np.vstack([x, xbar]), np.vstack([bx, bxbar])
+    am = labels_range(n + nbar, n, 0, nperm, seed)
+    ab = labels_range(bs + bsbar, bs, 0, nperm, seed ^ BKG_SEED_XOR)
+    bp, bbp = (b + bbar) * n / (n + nbar), (b + bbar) * nbar / (n + nbar)
+    t_perm = np.empty(nperm)
+    for p in range(nperm):
+        t_perm[p] = T_bkg(main[am[p] == 1], main[am[p] == 0], side[ab[p] == 1], side[ab[p] == 0], bp, bbp, sigma)
+    count = int((t_perm > t_obs).sum())
+    return t_obs, t_perm, count, count / nperm

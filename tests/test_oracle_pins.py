@@ -417,3 +417,29 @@ def test_oracle_rejects_bad_arguments():
         oracle.T(x, x, float("nan"))
     with pytest.raises(ValueError):
         oracle.T(x, x, 0.3, np.array([0.2, 0.2, 0.2]), np.ones(3))  # W <= 1
+
+
+def test_eq3_permutations_without_background_are_eq2_permutations():
+    """Reading R18 pinned to the Eq. 2 permutation oracle: with b = bbar = 0 the background samples drop out of Eq. 3
+    and every permutation T equals the one of `perm_test` on the main samples (same label stream, same order)."""
+    rng = np.random.default_rng(31)
+    x, xb = rng.uniform(size=(14, 2)), rng.uniform(size=(11, 2))
+    bx, bb = rng.uniform(size=(5, 2)), rng.uniform(size=(4, 2))
+    t_obs, t_perm, count, p = oracle.bkg_perm_test(x, xb, bx, bb, 0.0, 0.0, 0.3, 12, 77)
+    ref = oracle.perm_test(x, xb, 0.3, 12, 77)
+    assert t_obs == pytest.approx(ref.observed.T, abs=1e-15)
+    assert np.allclose(t_perm, ref.T_perm, rtol=0, atol=1e-15) and count == ref.count_gt
+
+
+def test_eq3_permutations_keep_sizes_and_equalise_the_purity():
+    """Flat signal and flat background with a 3:1 flavour asymmetry of the background only: Eq. 2 on the main samples
+    is blind to it (same density), and under permutation the expected background counts are proportional to the
+    sample sizes: the mean of the permutation T of Eq. 3 is compatible with zero."""
+    rng = np.random.default_rng(32)
+    sig, bkg, side = rng.uniform(size=(60, 2)), rng.uniform(size=(40, 2)), rng.uniform(size=(40, 2))
+    fl, flb, fls = rng.random(60) < 0.5, rng.random(40) < 0.75, rng.random(40) < 0.75
+    x, xb = np.vstack([sig[fl], bkg[flb]]), np.vstack([sig[~fl], bkg[~flb]])
+    t_obs, t_perm, count, p = oracle.bkg_perm_test(x, xb, side[fls], side[~fls], float(flb.sum()), float((~flb).sum()), 0.25, 60, 5)
+    assert np.isfinite(t_perm).all() and len(np.unique(t_perm)) == 60
+    assert abs(t_perm.mean()) < 4 * t_perm.std() / np.sqrt(60)
+    assert 0 <= p <= 1 and count == int((t_perm > t_obs).sum())
