@@ -192,6 +192,26 @@ et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int6
                    double b, double bbar, int dim, et_dtype dtype, et_memspace mem,
                    double sigma, et_bkg_result *out);
 
+/* Permutation test with Eq. 3 as the statistic (the permutation method is used "using the same
+ * method to remove background from the randomly permuted samples"; reading R18 of DESIGN.md).  Permutation p
+ * reassigns the pooled main events to main samples of sizes (n, nbar) with the labels of reading R4 drawn from
+ * `seed`, and the pooled background-sample events to samples of sizes (bs, bsbar) with the labels drawn from
+ * seed ^ 0x9E3779B97F4A7C15; a random flavour gives both main samples the same purity, so the permuted samples
+ * are evaluated with b' = (b + bbar) n / (n + nbar) and bbar' = (b + bbar) nbar / (n + nbar).  One four-class
+ * all-pairs pass per permutation (the paper's cost model; meant for background studies of modest size).
+ * T_perm[nperm] is host memory; ET_OPT_PERM_OFFSET applies. */
+typedef struct {
+    et_bkg_result observed;
+    double p_value;                  /* count_gt / nperm                                              */
+    int64_t count_gt, n_near, nperm; /* as et_perm_result                                             */
+} et_bkg_perm_result;
+
+et_status et_bkg_permutation_test(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar,
+                                  const void *bx, int64_t bs, const void *bxbar, int64_t bsbar,
+                                  double b, double bbar, int dim, et_dtype dtype, et_memspace mem,
+                                  double sigma, int64_t nperm, uint64_t seed,
+                                  double *T_perm, et_bkg_perm_result *out);
+
 /* GEV fit of the permutation T values ("the permutation T distribution can be fitted with a
  * generalised-extreme-value (GEV) function ... The p-value from the fitted T distribution can be calculated as
  * the fraction of the integral of the function above the observed T value"; its uncertainty "by

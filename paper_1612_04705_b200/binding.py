@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
 
 
 class EtError(RuntimeError):
@@ -53,6 +53,11 @@ class _PoddResult(C.Structure):
 class _BkgResult(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("T", "T_xx", "T_bb", "T_xb")] + [("S", C.c_double * 10), ("w", C.c_double),
                                                                         ("wbar", C.c_double), ("n_pairs", C.c_int64)]
+
+
+class _BkgPermResult(C.Structure):
+    _fields_ = [("observed", _BkgResult), ("p_value", C.c_double), ("count_gt", C.c_int64), ("n_near", C.c_int64),
+                ("nperm", C.c_int64)]
 
 
 class _GevResult(C.Structure):
@@ -116,6 +121,16 @@ class BkgResult:
     @property
     def term_scale(self) -> float:
         return abs(self.T_xx) + abs(self.T_bb) + abs(self.T_xb)
+
+
+@dataclass
+class BkgPermResult:
+    observed: BkgResult
+    p_value: float
+    count_gt: int
+    n_near: int
+    nperm: int
+    T_perm: np.ndarray
 
 
 @dataclass
@@ -319,6 +334,22 @@ class Context:
                                    C.c_int64(abx.shape[0]), abb.ptr, C.c_int64(abb.shape[0]), C.c_double(b), C.c_double(bbar),
                                    C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
         return BkgResult(out.T, out.T_xx, out.T_bb, out.T_xb, tuple(out.S), out.w, out.wbar, out.n_pairs)
+
+    def bkg_permutation_test(self, x, xbar, bx, bxbar, b: float, bbar: float, sigma: float, nperm: int, seed: int) -> BkgPermResult:
+        """Permutation test with Eq. 3 as the statistic (main and background pools permuted independently)."""
+        ax, ab = _coords(x, xbar)
+        abx, abb = _coords(bx, bxbar)
+        if (abx.mem, abx.dtype, abx.shape[1]) != (ax.mem, ax.dtype, ax.shape[1]):
+            raise ValueError("background samples must share memory space, dtype and dim with the main samples")
+        Tp = np.zeros(max(int(nperm), 1), dtype=np.float64)
+        out = _BkgPermResult()
+        self._check(lib().et_bkg_permutation_test(
+            self._h, ax.ptr, C.c_int64(ax.shape[0]), ab.ptr, C.c_int64(ab.shape[0]), abx.ptr, C.c_int64(abx.shape[0]), abb.ptr,
+            C.c_int64(abb.shape[0]), C.c_double(b), C.c_double(bbar), C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem),
+            C.c_double(sigma), C.c_int64(nperm), C.c_uint64(seed), Tp.ctypes.data_as(C.c_void_p), C.byref(out)))
+        o = out.observed
+        return BkgPermResult(BkgResult(o.T, o.T_xx, o.T_bb, o.T_xb, tuple(o.S), o.w, o.wbar, o.n_pairs), out.p_value,
+                             out.count_gt, out.n_near, out.nperm, Tp)
 
     # ---------------------------------------------------------------- permutation test
     def permutation_test(self, x, xbar, sigma: float, nperm: int, seed: int, wx=None, wxbar=None) -> PermResult:

@@ -567,9 +567,10 @@ struct DevBkg {
     int status;
 };
 __global__ void k_stat_eq3(const double *__restrict__ S, double n, double nbar, double bs, double bsb, double b, double bbar,
-                           long long npairs, DevBkg *out)
+                           long long npairs, DevBkg *out, double *T_out)
 {
     if (threadIdx.x || blockIdx.x) return;
+    if (T_out) *T_out = nan("");
     et_bkg_result r;
     const int order[10] = {0, 1, 2, 3, 5, 6, 7, 10, 11, 15};
     for (int k = 0; k < 10; ++k) r.S[k] = S[order[k]];
@@ -591,6 +592,7 @@ __global__ void k_stat_eq3(const double *__restrict__ S, double n, double nbar, 
     r.T = r.T_xx + r.T_bb - r.T_xb;
     out->r = r;
     out->status = 0;
+    if (T_out) *T_out = r.T;
 }
 // src[row] for class segments that are consecutive runs of the pooled source index (class c = sources
 // seg_first[c] .. seg_first[c] + seg_count[c] - 1), -1 on padding rows
@@ -1085,16 +1087,15 @@ et_status et_T_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n, c
     return ET_OK;
 }
 
-et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,
-                   const void *bxbar, int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem, double sigma,
-                   et_bkg_result *out)
+}  // extern "C" (helpers of the Eq. 3 entry points follow)
+namespace {
+
+// Validation, staging, identity four-class layout (X, Bx, Xbar, Bxbar), records, one K-T pass and Eq. 3 of the observed
+// samples.  Leaves the records in ctx->rec and the layout in L.
+et_status bkg_observed(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,
+                       const void *bxbar, int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem, double sigma,
+                       Layout &L, DevBkg &r)
 {
-    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
-    if (!out || !bx || !bxbar) return fail(ctx, ET_ERR_INVALID, "null background sample or output");
-    if (bs < 2 || bsbar < 2) return fail(ctx, ET_ERR_INVALID, "background samples need >= 2 events (Eq. 3 divides by b_s(b_s-1)); got %lld, %lld", (long long)bs, (long long)bsbar);
-    if (n + nbar + bs + bsbar >= (1ll << 31)) return fail(ctx, ET_ERR_INVALID, "total number of events must be < 2^31");
-    if (!(b >= 0.0) || !(bbar >= 0.0) || !std::isfinite(b) || !std::isfinite(bbar)) return fail(ctx, ET_ERR_INVALID, "b and bbar must be finite and >= 0");
-    ET_TRY(begin_call(ctx));
     // the x side of the pooled source index is [x ; bx], the xbar side [xbar ; bxbar]
     const size_t row = (size_t)dim * elem_size(dtype);
     ET_TRY(ensure(ctx, ctx->in_x, (size_t)(n + bs) * row));
@@ -1106,7 +1107,6 @@ et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int6
     CUDA_TRY(cudaMemcpyAsync(sb, xbar, (size_t)nbar * row, kind, ctx->stream));
     CUDA_TRY(cudaMemcpyAsync(sb + (size_t)nbar * row, bxbar, (size_t)bsbar * row, kind, ctx->stream));
     if (mem == ET_HOST) CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // the caller's buffers may be pageable
-    Layout L;
     const long long cnt[4] = {n, bs, nbar, bsbar};
     layout_four(L, n + bs, nbar + bsbar, cnt);
     ET_TRY(upload_tile_classes(ctx, L));
@@ -1122,13 +1122,110 @@ et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int6
     ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4 + sizeof(DevBkg)));
     const long long Nall = n + nbar + bs + bsbar;
     k_stat_eq3<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), (double)n, (double)nbar, (double)bs, (double)bsbar, b, bbar,
-                                          Nall * (Nall - 1) / 2, static_cast<DevBkg *>(ctx->result.p));
+                                          Nall * (Nall - 1) / 2, static_cast<DevBkg *>(ctx->result.p), nullptr);
     LAUNCH_CHECK();
-    DevBkg r;
     ET_TRY(fetch(ctx, ctx->result.p, &r));
+    return ET_OK;
+}
+
+et_status bkg_check(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs, const void *bxbar,
+                    int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem, double sigma)
+{
+    ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigma));
+    if (!bx || !bxbar) return fail(ctx, ET_ERR_INVALID, "null background sample");
+    if (bs < 2 || bsbar < 2) return fail(ctx, ET_ERR_INVALID, "background samples need >= 2 events (Eq. 3 divides by b_s(b_s-1)); got %lld, %lld", (long long)bs, (long long)bsbar);
+    if (n + nbar + bs + bsbar >= (1ll << 31)) return fail(ctx, ET_ERR_INVALID, "total number of events must be < 2^31");
+    if (!(b >= 0.0) || !(bbar >= 0.0) || !std::isfinite(b) || !std::isfinite(bbar)) return fail(ctx, ET_ERR_INVALID, "b and bbar must be finite and >= 0");
+    return ET_OK;
+}
+
+}  // namespace
+extern "C" {
+
+et_status et_T_bkg(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,
+                   const void *bxbar, int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem, double sigma,
+                   et_bkg_result *out)
+{
+    ET_TRY(bkg_check(ctx, x, n, xbar, nbar, bx, bs, bxbar, bsbar, b, bbar, dim, dtype, mem, sigma));
+    if (!out) return fail(ctx, ET_ERR_INVALID, "null output");
+    ET_TRY(begin_call(ctx));
+    Layout L;
+    DevBkg r;
+    ET_TRY(bkg_observed(ctx, x, n, xbar, nbar, bx, bs, bxbar, bsbar, b, bbar, dim, dtype, mem, sigma, L, r));
     ET_TRY(end_call(ctx));
     if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "Eq. 3 normalisation degenerate: w = n - b = %g, wbar = nbar - bbar = %g (need > 1)", r.r.w, r.r.wbar);
     *out = r.r;
+    return ET_OK;
+}
+
+et_status et_bkg_permutation_test(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, const void *bx, int64_t bs,
+                                  const void *bxbar, int64_t bsbar, double b, double bbar, int dim, et_dtype dtype, et_memspace mem,
+                                  double sigma, int64_t nperm, uint64_t seed, double *T_perm, et_bkg_perm_result *out)
+{
+    ET_TRY(bkg_check(ctx, x, n, xbar, nbar, bx, bs, bxbar, bsbar, b, bbar, dim, dtype, mem, sigma));
+    if (!out || !T_perm) return fail(ctx, ET_ERR_INVALID, "null output");
+    if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
+    ET_TRY(begin_call(ctx));
+    Layout L;
+    DevBkg obs;
+    ET_TRY(bkg_observed(ctx, x, n, xbar, nbar, bx, bs, bxbar, bsbar, b, bbar, dim, dtype, mem, sigma, L, obs));
+    if (obs.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "Eq. 3 normalisation degenerate: w = n - b = %g, wbar = nbar - bbar = %g (need > 1)", obs.r.w, obs.r.wbar);
+    // purity of the permuted samples (reading R18): a random flavour spreads the b + bbar background events over the
+    // two main samples in proportion to their sizes
+    const double bp = (b + bbar) * (double)n / (double)(n + nbar), bbp = (b + bbar) * (double)nbar / (double)(n + nbar);
+    if (!((double)n - bp > 1.0) || !((double)nbar - bbp > 1.0)) return fail(ctx, ET_ERR_DEGENERATE, "Eq. 3 normalisation of the permuted samples degenerate");
+
+    // labels of both pools: select states of the n-th (bs-th) smallest composite of every permutation
+    ET_TRY(span_begin(ctx, 4));
+    const uint64_t seed_b = seed ^ 0x9E3779B97F4A7C15ull;
+    ET_TRY(run_label_select(ctx, n + nbar, n, (int)nperm, seed));
+    ET_TRY(ensure(ctx, ctx->mask, 2 * (size_t)nperm * sizeof(SelState)));
+    SelState *sel_m = static_cast<SelState *>(ctx->mask.p), *sel_b = sel_m + nperm;
+    CUDA_TRY(cudaMemcpyAsync(sel_m, ctx->sel.p, (size_t)nperm * sizeof(SelState), cudaMemcpyDeviceToDevice, ctx->stream));
+    ET_TRY(run_label_select(ctx, bs + bsbar, bs, (int)nperm, seed_b));
+    CUDA_TRY(cudaMemcpyAsync(sel_b, ctx->sel.p, (size_t)nperm * sizeof(SelState), cudaMemcpyDeviceToDevice, ctx->stream));
+    ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
+
+    // the identity-layout records are kept aside; every permutation gathers its own order from them
+    const int F = rec_floats(dim);
+    const size_t rec_bytes = (size_t)L.npad * F * sizeof(float);
+    ET_TRY(ensure(ctx, ctx->recP, rec_bytes));
+    CUDA_TRY(cudaMemcpyAsync(ctx->recP.p, ctx->rec.p, rec_bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    k_fill_int<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<int *>(ctx->src.p), L.npad, -1);
+    LAUNCH_CHECK();
+    ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
+    BkgPermParams BP{};
+    BP.n = n; BP.nbar = nbar; BP.bs = bs; BP.bsbar = bsbar;
+    for (int c = 0; c < 4; ++c) BP.pos0[c] = L.seg_pos[c];
+    BP.seedm_lo = (uint32_t)(seed & 0xffffffffu); BP.seedm_hi = (uint32_t)(seed >> 32);
+    BP.seedb_lo = (uint32_t)(seed_b & 0xffffffffu); BP.seedb_hi = (uint32_t)(seed_b >> 32);
+    DevBkg *scratch = reinterpret_cast<DevBkg *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm) + sizeof(DevT) * 4);
+    const long long Nall = n + nbar + bs + bsbar;
+    for (int64_t p = 0; p < nperm; ++p) {
+        k_bkg_perm_map<<<1, 1024, 0, ctx->stream>>>(BP, ctx->opt_perm_offset + p, sel_m + p, sel_b + p, static_cast<int *>(ctx->src.p));
+        LAUNCH_CHECK();
+        k_gather_rec<<<ctx->num_sms * 2, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->recP.p), static_cast<const int *>(ctx->src.p),
+                                                               L.npad, F / 4, static_cast<float4 *>(ctx->rec.p));
+        LAUNCH_CHECK();
+        ET_TRY(run_pairs_T(ctx, L, dim));
+        k_stat_eq3<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), (double)n, (double)nbar, (double)bs, (double)bsbar, bp, bbp,
+                                              Nall * (Nall - 1) / 2, scratch, static_cast<double *>(ctx->tperm.p) + p);
+        LAUNCH_CHECK();
+    }
+    const double guard = 1e-9 * (std::fabs(obs.r.T_xx) + std::fabs(obs.r.T_bb) + std::fabs(obs.r.T_xb));
+    ET_TRY(ensure(ctx, ctx->count64, 16));
+    k_count_gt<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->tperm.p), (int)nperm, obs.r.T, guard, static_cast<long long *>(ctx->count64.p));
+    LAUNCH_CHECK();
+    long long cnt2[2];
+    ET_TRY(fetch(ctx, ctx->count64.p, &cnt2));
+    CUDA_TRY(cudaMemcpyAsync(T_perm, ctx->tperm.p, (size_t)nperm * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    ET_TRY(end_call(ctx));
+    out->observed = obs.r;
+    out->count_gt = cnt2[0];
+    out->n_near = cnt2[1];
+    out->nperm = nperm;
+    out->p_value = (double)cnt2[0] / (double)nperm;
     return ET_OK;
 }
 

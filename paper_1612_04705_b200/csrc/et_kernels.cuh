@@ -856,6 +856,96 @@ __global__ void k_fill_int(int *p, long long n, int v)
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
 }
 
+// ---- Eq. 3 permutation test (one all-pairs pass per permutation over re-ordered records) ---------------------
+// Sources: the pooled source index s of et_T_bkg's staging, x side = [x (n) ; bx (bs)], xbar side = [xbar (nbar) ;
+// bxbar (bsbar)].  Main pool index: x[k] -> k, xbar[k] -> n + k; background pool index: bx[k] -> k, bxbar[k] -> bs + k.
+struct BkgPermParams {
+    long long n, nbar, bs, bsbar;
+    long long pos0[4];   // first record row of the identity layout's class segments (X, Bx, Xbar, Bxbar)
+    uint32_t seedm_lo, seedm_hi, seedb_lo, seedb_hi;
+};
+// rowmap[row] = row of the identity-layout records that permutation pg (global index; `sm`, `sb` its select states for
+// the main and the background pool) puts into layout row `row`: classes (X', Bx', Xbar', Bxbar'), each in source order
+// (stable), padding rows untouched (-1 from the caller's fill).  One CTA of 1024 threads, chunked block scan: the
+// statistic is for background-subtraction studies of modest size (PAPER.md:105 uses 7 200 events).
+__global__ void __launch_bounds__(1024) k_bkg_perm_map(BkgPermParams P, long long pg, const SelState *__restrict__ sm,
+                                                      const SelState *__restrict__ sb, int *__restrict__ rowmap)
+{
+    __shared__ int warp_cnt[32][4];
+    __shared__ long long run[4];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid < 4) run[tid] = 0;
+    __syncthreads();
+    const long long Nx = P.n + P.bs, Ntot = Nx + P.nbar + P.bsbar;
+    const unsigned long long pre_m = sm->prefix, pre_b = sb->prefix;
+    for (long long base = 0; base < Ntot; base += 1024) {
+        const long long s = base + tid;
+        int c = -1;
+        long long row0 = 0;
+        if (s < Ntot) {
+            bool bkg;
+            long long idx;  // index in its pool
+            if (s < Nx) { bkg = s >= P.n; idx = bkg ? s - P.n : s; row0 = bkg ? P.pos0[1] + idx : P.pos0[0] + idx; }
+            else {
+                const long long t = s - Nx;
+                bkg = t >= P.nbar;
+                idx = bkg ? P.bs + (t - P.nbar) : P.n + t;
+                row0 = bkg ? P.pos0[3] + (t - P.nbar) : P.pos0[2] + t;
+            }
+            uint64_t K[4];
+            label_keys4((uint32_t)idx, (uint32_t)(pg >> 2), bkg ? P.seedb_lo : P.seedm_lo, bkg ? P.seedb_hi : P.seedm_hi, K);
+            const bool in_x = K[pg & 3] <= (bkg ? pre_b : pre_m);
+            c = (in_x ? 0 : 2) + (bkg ? 1 : 0);
+        }
+        unsigned bal[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) bal[k] = __ballot_sync(0xffffffffu, c == k);
+        if (lane == 0)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) warp_cnt[warp][k] = __popc(bal[k]);
+        __syncthreads();
+        if (c >= 0) {
+            long long r = run[c] + __popc(bal[c] & ((1u << lane) - 1u));
+            for (int w = 0; w < warp; ++w) r += warp_cnt[w][c];
+            rowmap[P.pos0[c] + r] = (int)row0;   // class segments of the permuted layout start where the identity ones do
+        }
+        __syncthreads();
+        if (tid < 4) {
+            long long t = 0;
+            for (int w = 0; w < 32; ++w) t += warp_cnt[w][tid];
+            run[tid] += t;
+        }
+        __syncthreads();
+    }
+}
+// rec[row] = rec0[rowmap[row]] (zero record on padding rows), F floats per row
+__global__ void k_gather_rec(const float4 *__restrict__ rec0, const int *__restrict__ rowmap, long long npad, int F4, float4 *__restrict__ rec)
+{
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < npad * F4; k += (long long)gridDim.x * blockDim.x) {
+        const long long row = k / F4;
+        const int q = (int)(k % F4), src = rowmap[row];
+        rec[k] = src >= 0 ? rec0[(long long)src * F4 + q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+// count = #{T_p > T_obs}, near = #{|T_p - T_obs| <= guard or T_p not finite}; one block
+__global__ void __launch_bounds__(256) k_count_gt(const double *__restrict__ T, int nperm, double Tobs, double guard, long long *__restrict__ out)
+{
+    __shared__ unsigned long long s_cnt, s_near;
+    if (threadIdx.x == 0) { s_cnt = 0ull; s_near = 0ull; }
+    __syncthreads();
+    unsigned long long c = 0, nr = 0;
+    for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
+        const double t = T[p];
+        if (!isfinite(t)) { nr += 1; continue; }
+        if (t > Tobs) c += 1;
+        if (fabs(t - Tobs) <= guard) nr += 1;
+    }
+    atomicAdd(&s_cnt, c);
+    atomicAdd(&s_near, nr);
+    __syncthreads();
+    if (threadIdx.x == 0) { out[0] = (long long)s_cnt; out[1] = (long long)s_near; }
+}
+
 // gather of the listed rows of rowsum (test hook et_row_sums)
 __global__ void k_gather_rows(const double *__restrict__ rowsum, long long npad, const long long *__restrict__ pos, long long nrows,
                               int C, double *__restrict__ out)

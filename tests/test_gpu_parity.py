@@ -545,3 +545,43 @@ def test_perm_tc_bit_reproducible_many_units(ctx):
         d = other.permutation_test(s.x, s.xbar, c.sigma, 600, 11)
     assert (a.T_perm == d.T_perm).all() and a.observed.T == d.observed.T
     assert abs(a.observed.T - ctx.T(s.x, s.xbar, c.sigma).T) <= TOL * a.observed.term_scale
+
+
+# ----------------------------------------------------------------------------- Eq. 3 permutation test (NEXT-1, R18)
+def test_bkg_permutation_test_matches_oracle(ctx):
+    """Fig. 3-structured inputs at a tenth of the paper's size: every permutation T of Eq. 3 against the oracle's
+    from-scratch re-evaluation (both pools permuted with the shared Philox label rule)."""
+    x, xb, bx, bb, b, bbar = dg.make_bkg_sample(scale=0.1)
+    nperm = 40
+    t_obs, t_perm, count, p = oracle.bkg_perm_test(x, xb, bx, bb, b, bbar, 0.25, nperm, 4711)
+    got = ctx.bkg_permutation_test(x, xb, bx, bb, b, bbar, 0.25, nperm, 4711)
+    scale = got.observed.term_scale
+    assert abs(got.observed.T - t_obs) <= TOL * scale
+    assert np.abs(got.T_perm - t_perm).max() <= TOL * scale
+    assert abs(got.count_gt - count) <= got.n_near and got.nperm == nperm
+    if got.n_near == 0:
+        assert got.p_value == p
+    # same permutation order of the T values
+    assert (np.argsort(got.T_perm) == np.argsort(t_perm)).all()
+
+
+def test_bkg_permutation_test_reduces_to_eq2_and_windows(ctx):
+    rng = np.random.default_rng(90)
+    x, xb = rng.uniform(size=(900, 3)), rng.uniform(size=(1200, 3)) ** 1.1
+    bx, bb = rng.uniform(size=(1030, 3)), rng.uniform(size=(17, 3))
+    # b = bbar = 0: the permutation T values of Eq. 3 are those of Eq. 2 on the main samples (same label stream)
+    z = ctx.bkg_permutation_test(x, xb, bx, bb, 0.0, 0.0, 0.3, 24, 5)
+    with force_kernel(ctx, 1):
+        ref = ctx.permutation_test(x, xb, 0.3, 24, 5)
+    assert np.abs(z.T_perm - ref.T_perm).max() <= TOL * ref.observed.term_scale and z.count_gt == ref.count_gt
+    # ET_OPT_PERM_OFFSET: a window of the same stream
+    full = ctx.bkg_permutation_test(x, xb, bx, bb, 40.0, 10.0, 0.3, 12, 5)
+    try:
+        ctx.set_option(binding.ET_OPT_PERM_OFFSET, 5)
+        win = ctx.bkg_permutation_test(x, xb, bx, bb, 40.0, 10.0, 0.3, 7, 5)
+    finally:
+        ctx.set_option(binding.ET_OPT_PERM_OFFSET, 0)
+    assert (win.T_perm == full.T_perm[5:12]).all() and win.observed.T == full.observed.T
+    with pytest.raises(binding.EtError) as e:
+        ctx.bkg_permutation_test(x, xb, bx, bb, 899.5, 0.0, 0.3, 4, 5)
+    assert e.value.status == -4
