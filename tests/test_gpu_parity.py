@@ -585,3 +585,23 @@ def test_bkg_permutation_test_reduces_to_eq2_and_windows(ctx):
     with pytest.raises(binding.EtError) as e:
         ctx.bkg_permutation_test(x, xb, bx, bb, 899.5, 0.0, 0.3, 4, 5)
     assert e.value.status == -4
+
+
+def test_full_size_config3_weighted_tc_properties(ctx):
+    """BASELINE configs[3] at full size (n = nbar = 200 000, signed per-event weights, 1000 permutations): the weighted
+    tensor-core path (signed hi digit, fp64 epilogue) against the weighted all-pairs kernel for the observed statistic,
+    and the permutation distribution through properties (count consistency, distinct values, W_p recomputed)."""
+    c = dg.config(3)
+    s = dg.make_sample(c)
+    got = ctx.permutation_test(s.x, s.xbar, c.sigma, c.nperm, c.perm_seed, s.wx, s.wxbar)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    ref = ctx.T_weighted(s.x, s.wx, s.xbar, s.wxbar, c.sigma)
+    scale = ref.term_scale
+    o = got.observed
+    assert abs(o.T - ref.T) <= TOL * scale and abs(o.T_xx - ref.T_xx) <= TOL * scale and abs(o.T_xb - ref.T_xb) <= TOL * scale
+    assert o.W == pytest.approx(ref.W, rel=1e-12) and o.Wbar == pytest.approx(ref.Wbar, rel=1e-12)
+    assert o.W == pytest.approx(float(np.float32(s.wx).astype(np.float64).sum()), rel=1e-9)   # weights enter as fp32
+    Tp = got.T_perm
+    assert np.isfinite(Tp).all() and len(np.unique(Tp)) == c.nperm
+    assert got.count_gt == int((Tp > o.T).sum()) and got.p_value == got.count_gt / c.nperm
+    assert 1e-8 < Tp.std() < 1e-4
