@@ -605,3 +605,16 @@ def test_full_size_config3_weighted_tc_properties(ctx):
     assert np.isfinite(Tp).all() and len(np.unique(Tp)) == c.nperm
     assert got.count_gt == int((Tp > o.T).sum()) and got.p_value == got.count_gt / c.nperm
     assert 1e-8 < Tp.std() < 1e-4
+
+
+def test_perm_tc_accumulator_headroom_coincident_points(ctx):
+    """The largest values the int32 TMEM accumulators can see: 80 000 coincident events, psi = 1 for every pair, so the
+    first row tile's units sum 1000 K blocks x 64 j x 32767.  Pin P1 at scale: T = 1/2 + 1/2 - 1 = 0 for the observed
+    and for every permutation; the raw sums are the pair counts."""
+    n = nbar = 40000
+    x, xb = np.full((n, 2), 0.25), np.full((nbar, 2), 0.25)
+    got = ctx.permutation_test(x, xb, 0.3, 20, 3)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    o = got.observed
+    assert o.S_xx == pytest.approx(n * (n - 1) / 2, rel=1e-12) and o.S_xb == pytest.approx(n * nbar, rel=1e-12)
+    assert abs(o.T) <= 1e-12 and np.abs(got.T_perm).max() <= 1e-12
