@@ -41,7 +41,10 @@ constexpr int kCols = 512;               // label columns per launch (2 accumula
 constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
-constexpr int kProducerWarps = 16;          // four per scheduler: the tile generation is latency-bound with two (profiles/r01b)
+#ifndef ET_TC_PW
+#define ET_TC_PW 16
+#endif
+constexpr int kProducerWarps = ET_TC_PW;          // four per scheduler: the tile generation is latency-bound with two (profiles/r01b)
 constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // a thread evaluates 8 j x this many rows (2)
 constexpr int kEpiGroups = 16 / (kProducerWarps / 4);                 // 32-column groups per warp in the epilogue (4)
 constexpr int kProducers = kProducerWarps * 32;
@@ -432,7 +435,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
         magicA.x = keep(magicA.x);
         magicA.y = keep(magicA.y);
-        const int jw = warp & 7, qw = warp >> 3;        // label task: 8 j of the K block, column half q
+        constexpr int NQ = 16 / kProducerWarps;          // label words (column halves) per thread: 1 with 16 warps, 2 with 8
+        const int jw = warp & 7, qw = NQ == 1 ? warp >> 3 : 0;  // label task: 8 j of the K block, column half q (first of NQ)
         const int jj = 8 * jw + (lane >> 2);            // j (local) of this thread's label word
         const int l3 = lane & 3;
         // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct; SWIZZLE_64B; row
@@ -469,12 +473,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             const int dthr = row0 + mrow0 - 8 * oct;
             // this thread's label word of K block kb (element index < 2^32), prefetched one block ahead into a register
             uint32_t im = (uint32_t)(U.kb_begin * kKB + jj) * (uint32_t)P.words_total + (uint32_t)(P.word0 + 8 * qw + 4 * (int)rank + l3);
-            uint32_t mw = __ldg(P.maskT + im);
+            uint32_t mw = __ldg(P.maskT + im), mw2 = NQ == 2 ? __ldg(P.maskT + im + 8) : 0u;
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                const uint32_t mcur = mw;
+                const uint32_t mcur = mw, mcur2 = mw2;
                 if (kb + 1 < U.kb_end) {
                     im += (uint32_t)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
+                    if (NQ == 2) mw2 = __ldg(P.maskT + im + 8);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
                 mbar_wait_a(bar0 + 8 * kStages + 8 * (it & (kStages - 1)), ((it / kStages) & 1) ^ 1);
@@ -504,10 +509,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur >> (4 * tp + t)) & 0x01010101u;
                                 sts128((tp == 0 ? pbB : pbB1) + 8192, make_uint4(q[0], q[1], q[2], q[3]));
+                                if (NQ == 2) {
+#pragma unroll
+                                    for (int t = 0; t < 4; ++t) q[t] = (mcur2 >> (4 * tp + t)) & 0x01010101u;
+                                    sts128((tp == 0 ? pbB : pbB1) + 16384 + 8192, make_uint4(q[0], q[1], q[2], q[3]));
+                                }
                             } else {
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
                                 sts128(tp == 2 ? pbB : pbB1, make_uint4(q[0], q[1], q[2], q[3]));
+                                if (NQ == 2) {
+#pragma unroll
+                                    for (int t = 0; t < 4; ++t) q[t] = (mcur2 << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
+                                    sts128((tp == 2 ? pbB : pbB1) + 16384, make_uint4(q[0], q[1], q[2], q[3]));
+                                }
                             }
                         }
                         if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
