@@ -789,11 +789,11 @@ template <int D>
 et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted)
 {
     if (weighted) {
-        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemTC));
-        tc::k_perm_tc<D, true><<<grid, tc::kThreadsTC, tc::kSmemTC, ctx->stream>>>(P);
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_tc(D)));
+        tc::k_perm_tc<D, true><<<grid, tc::kThreadsTC, tc::smem_tc(D), ctx->stream>>>(P);
     } else {
-        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemTC));
-        tc::k_perm_tc<D, false><<<grid, tc::kThreadsTC, tc::kSmemTC, ctx->stream>>>(P);
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_tc(D)));
+        tc::k_perm_tc<D, false><<<grid, tc::kThreadsTC, tc::smem_tc(D), ctx->stream>>>(P);
     }
     LAUNCH_CHECK();
     return ET_OK;
@@ -809,8 +809,10 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // labels
     ET_TRY(span_begin(ctx, 4));
     ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
-    ET_TRY(ensure(ctx, ctx->maskT, (size_t)L.npad * words_total * sizeof(uint32_t)));
-    CUDA_TRY(cudaMemsetAsync(ctx->maskT.p, 0, (size_t)L.npad * words_total * sizeof(uint32_t), ctx->stream));
+    // the j range of the contraction is padded to whole K blocks: rows npad .. npadK - 1 carry zero labels and zero records
+    const long long npadK = (L.npad + tc::kKB - 1) / tc::kKB * tc::kKB;
+    ET_TRY(ensure(ctx, ctx->maskT, (size_t)npadK * words_total * sizeof(uint32_t)));
+    CUDA_TRY(cudaMemsetAsync(ctx->maskT.p, 0, (size_t)npadK * words_total * sizeof(uint32_t), ctx->stream));
     LabelOut lo{};
     lo.nseg = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
@@ -830,16 +832,17 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // fell from 640 GB to the order of the matrix itself, profiles/r01d), then the shorter ones, longest first.
     // unit u -> cluster u % nclusters
     const int nclusters_max = ctx->num_sms / 2;
-    const int nT = (int)(L.npad / tc::kTM2), NK = (int)(L.npad / tc::kKB);
+    const int nT = (int)(L.npad / tc::kTM2), NK = (int)(npadK / tc::kKB);
+    auto first_kb = [](int I) { return (long long)I * tc::kTM2 / tc::kKB; };  // K block that holds the tile's first row
     long long total_kb = 0;
-    for (int I = 0; I < nT; ++I) total_kb += NK - 4 * I;
+    for (int I = 0; I < nT; ++I) total_kb += NK - first_kb(I);
     long long Lmax = (total_kb + (long long)nclusters_max * 24 - 1) / ((long long)nclusters_max * 24);
     if (Lmax < 8) Lmax = 8;
     if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
     std::vector<tc::Unit> full, tail;
     for (long long m = 0; m * Lmax < NK; ++m)
-        for (int I = 0; I < nT && 4ll * I < (m + 1) * Lmax; ++I) {
-            tc::Unit u{I, (int)std::max<long long>(4ll * I, m * Lmax), (int)std::min<long long>(NK, (m + 1) * Lmax), 0};
+        for (int I = 0; I < nT && first_kb(I) < (m + 1) * Lmax; ++I) {
+            tc::Unit u{I, (int)std::max<long long>(first_kb(I), m * Lmax), (int)std::min<long long>(NK, (m + 1) * Lmax), 0};
             if (u.kb_end <= u.kb_begin) continue;
             (u.kb_end - u.kb_begin == Lmax ? full : tail).push_back(u);
         }
@@ -864,7 +867,8 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(span_begin(ctx, 2));
     const float sc2 = (float)(2.0 * sc);
-    ET_TRY(ensure(ctx, ctx->recP, (size_t)(L.npad / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
+    ET_TRY(ensure(ctx, ctx->recP, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
+    CUDA_TRY(cudaMemsetAsync(ctx->recP.p, 0, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4), ctx->stream));
     DISPATCH_DIM(dim, (tc::k_pair_records<D><<<(unsigned)((L.npad / 2 + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
                           static_cast<const float *>(ctx->rec.p), L.npad / 2, sc2, static_cast<float4 *>(ctx->recP.p))));
     LAUNCH_CHECK();

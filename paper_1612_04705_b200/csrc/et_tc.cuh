@@ -36,26 +36,37 @@ namespace tc {
 
 constexpr int kTM = 128;                 // rows (i) per CTA = UMMA M / 2
 constexpr int kTM2 = 2 * kTM;            // rows per cluster (work unit)
-constexpr int kKB = 64;                  // j per K block
+#ifndef ET_TC_KB
+#define ET_TC_KB 96
+#endif
+constexpr int kKB = ET_TC_KB;            // j per K block: 64 (16 producer warps x 2 rows) or 96 (12 warps x 4 rows, needs ET_TC_A32)
 constexpr int kCols = 512;               // label columns per launch (2 accumulators of N = 256)
 constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
+#ifndef ET_TC_A32
+#define ET_TC_A32 1  // A digit tiles as K chunks of 32 bytes, each a SWIZZLE_32B [128 rows x 32 B] sub-tile; 0: one SWIZZLE_64B tile (K blocks of 64 j only)
+#endif
 #ifndef ET_TC_PW
-#define ET_TC_PW 16
+#define ET_TC_PW (ET_TC_KB == 96 ? 12 : 16)
 #endif
 constexpr int kProducerWarps = ET_TC_PW;          // four per scheduler: the tile generation is latency-bound with two (profiles/r01b)
 constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // a thread evaluates 8 j x this many rows (2)
-constexpr int kEpiGroups = 16 / (kProducerWarps / 4);                 // 32-column groups per warp in the epilogue (4)
+constexpr int kEpiWarps = kProducerWarps / 4;                         // warps per TMEM lane quarter
+constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;          // most 32-column groups a warp reads in the epilogue
+__host__ __device__ constexpr int epi_first(int e) { return 16 * e / kEpiWarps; }  // groups [epi_first(e), epi_first(e + 1)) of warp row e
 constexpr int kProducers = kProducerWarps * 32;
 constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
-constexpr int kStages = 4;
+constexpr int kStages = kKB == 96 ? 3 : 4;
 constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (16 KB)
-constexpr int kBBytes = 2 * 2 * 8192;        // this CTA's half of B: [q 2][digit 2][64 j x 128 columns] (32 KB)
+constexpr int kBPlane = kKB * 128;           // one plane of this CTA's half of B: kKB j x 128 columns
+constexpr int kBBytes = 2 * 2 * kBPlane;     // [q 2][digit 2][plane]
 constexpr int kStageBytes = kABytes + kBBytes;
-constexpr int kRecSlots = 8;                 // ring of j pair-record blocks (32 pairs each), filled by bulk copies
-constexpr int kRecSlotBytesMax = (kKB / 2) * 5 * 16;
-constexpr int kSmemTC = kStages * kStageBytes + kRecSlots * kRecSlotBytesMax + 1024 /*alignment slack*/;
+// ring of j pair-record blocks (kKB / 2 pairs each), filled by bulk copies; slots <= 2 kStages (see the loader)
+__host__ __device__ constexpr int rec_slots(int dim) { return kKB == 96 ? ((dim + 2) / 2 <= 3 ? 4 : 2) : 8; }
+__host__ __device__ constexpr int rec_slot_bytes(int dim) { return (kKB / 2) * ((dim + 2) / 2) * 16; }
+__host__ __device__ constexpr int smem_tc(int dim) { return kStages * kStageBytes + rec_slots(dim) * rec_slot_bytes(dim) + 1024 /*alignment slack*/; }
+constexpr int kMaxRecSlots = 8;
 // 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
 // complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
 // of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
@@ -63,7 +74,7 @@ constexpr int kSmemTC = kStages * kStageBytes + kRecSlots * kRecSlotBytesMax + 1
 constexpr float kMagic = 12582912.0f;
 // K blocks per unit: |Y| <= 32767 * 64 * 1000 = 2 097 088 000 < 2^31.  Longer units mean fewer epilogues and pipeline drains:
 // 512 -> 1000 measured -1.2 % (config 2) and -0.9 % (config 4) per step, identical integer sums.
-constexpr int kMaxUnitKB = 1000;
+constexpr int kMaxUnitKB = kKB == 96 ? 660 : 1000;   // 32767 * 96 * 660 = 2 076 117 120 < 2^31
 
 // label bit held by byte / TMEM column p of a 32-column word
 __host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
@@ -340,7 +351,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
     // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // one array, so that the hot loop addresses every barrier as bar0 + constant + 8 * index
-    __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + kRecSlots];
+    constexpr int kRecSlots = rec_slots(D);
+    __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + kMaxRecSlots];
     uint64_t *const bar_full = bars_s, *const bar_empty = bars_s + kStages, *const bar_rec = bars_s + 2 * kStages + 2;
     uint64_t &bar_accfull = bars_s[2 * kStages], &bar_accempty = bars_s[2 * kStages + 1];
     constexpr uint32_t kRecSlotBytes = (kKB / 2) * NLD * 16;
@@ -390,9 +402,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 #pragma unroll
                         for (int d = 0; d < 2; ++d)
 #pragma unroll
-                            for (int ks = 0; ks < 2; ++ks) {
-                                const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
-                                const uint64_t db = umma_desc(b_base + (q * 2 + d) * 8192 + ks * 4 * 1024, 8192, 1024, 2);
+                            for (int ks = 0; ks < kKB / 32; ++ks) {
+                                const uint64_t da = ET_TC_A32 ? umma_desc(a_base + d * (kTM * kKB) + ks * (kTM * 32), 16, 256, 6)
+                                                               : umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
+                                const uint64_t db = umma_desc(b_base + (q * 2 + d) * kBPlane + ks * 4 * 1024, kBPlane, 1024, 2);
                                 const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
                                 if (ET_TC_DBG != 2) umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
                             }
@@ -410,7 +423,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             for (int u = cluster_id; u < P.nunits; u += nclusters) {
                 const Unit U = P.units[u];
                 for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                    if (it >= kRecSlots) mbar_wait(&bar_empty[(it - kRecSlots) & (kStages - 1)], ((it - kRecSlots) / kStages) & 1);
+                    // kRecSlots <= 2 kStages: the awaited phase of bar_empty can be at most one phase old, never aliased
+                    if (it >= kRecSlots) mbar_wait(&bar_empty[(it - kRecSlots) % kStages], ((it - kRecSlots) / kStages) & 1);
                     const uint32_t slot = it & (kRecSlots - 1);
                     bulk_g2s(smem_u32(recs + slot * kRecSlotBytes), P.recP + (long long)kb * (kKB / 2) * NLD, kRecSlotBytes, &bar_rec[slot]);
                 }
@@ -422,9 +436,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         // 8 rows x 2 octets, so its 8-byte A-tile stores fall into 16 different bank pairs (no conflicts).
         constexpr int R = kRowsPerThread, G = kEpiGroups;
         const int og = (lane >> 3) & 1, l8 = lane & 7;
-        const int oct = 2 * (warp & 3) + og;
-        const int mrow0 = 16 * R * (warp >> 2) + 8 * (lane >> 4) + l8;
-        const int grp0 = G * (warp >> 2);            // first of the 16 column groups (32 columns each) of this warp's epilogue
+        constexpr int OW = kKB / 16;                 // warps along j (two octets each)
+        const int oct = 2 * (warp % OW) + og;
+        const int mrow0 = 16 * R * (warp / OW) + 8 * (lane >> 4) + l8;
+        const int grp0 = epi_first(warp >> 2), ngrp = epi_first((warp >> 2) + 1) - grp0;  // this warp's column groups in the epilogue
         const int lane_base = 32 * (warp & 3);       // TMEM lanes this warp may access
         Acc accQ[G], accR[G];
 #pragma unroll
@@ -435,20 +450,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
         magicA.x = keep(magicA.x);
         magicA.y = keep(magicA.y);
-        constexpr int NQ = 16 / kProducerWarps;          // label words (column halves) per thread: 1 with 16 warps, 2 with 8
-        const int jw = warp & 7, qw = NQ == 1 ? warp >> 3 : 0;  // label task: 8 j of the K block, column half q (first of NQ)
+        constexpr int NQ = kKB * 8 / kProducers;         // label words (column halves) per thread: 1 (64 j, 16 warps) or 2
+        const int jw = NQ == 1 ? warp & 7 : warp, qw = NQ == 1 ? warp >> 3 : 0;  // label task: 8 j of the K block, column half q (first of NQ)
         const int jj = 8 * jw + (lane >> 2);            // j (local) of this thread's label word
         const int l3 = lane & 3;
         // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct; SWIZZLE_64B; row
         // mrow0 + 16 r is 1024 r further) and B tile (j = jj, hi plane of column half qw, 16-byte chunk 2 l3 of the
         // 128-column row; SWIZZLE_128B; chunk 2 l3 + 1 is at address ^ 16, the lo plane 8192 further)
-        const int offA = (mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3);
-        const int offB = kABytes + qw * 16384 + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
+        // ET_TC_A32: the digit tile as K chunks of 32 bytes, each a [128 rows x 32 B] SWIZZLE_32B sub-tile (4 KB)
+        const int offA = ET_TC_A32 ? (oct >> 2) * (kTM * 32) + (mrow0 >> 3) * 256 + (mrow0 & 7) * 32 + (((((oct & 3) >> 1) ^ ((mrow0 >> 2) & 1))) << 4) + ((oct & 1) << 3)
+                                   : (mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3);
+        const int offB = kABytes + qw * (2 * kBPlane) + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
         const int offJ = kStages * kStageBytes + 4 * oct * NLD * 16;  // its four j pairs inside a record slot
         // running shared-memory addresses of the current stage / record slot (advanced and wrapped every K block)
         const uint32_t bar0 = smem_u32(bars_s);
         uint32_t paA = smem_u32(smem) + offA, pbB = smem_u32(smem) + offB, pjJ = smem_u32(smem) + offJ;
-        uint32_t it = 0, un = 0;
+        uint32_t it = 0, un = 0, st = 0, pe = 0;   // K blocks done, units done, stage index it % kStages, its phase (it / kStages) & 1
         for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
             const Unit U = P.units[u];
             const int row0 = U.I * kTM2 + (int)rank * kTM;   // npad < 2^31
@@ -482,7 +499,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     if (NQ == 2) mw2 = __ldg(P.maskT + im + 8);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
-                mbar_wait_a(bar0 + 8 * kStages + 8 * (it & (kStages - 1)), ((it / kStages) & 1) ^ 1);
+                mbar_wait_a(bar0 + 8 * kStages + 8 * st, pe ^ 1);
 
                 // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7; label tile: j = jj, this CTA's word
                 //      8 qw + 4 rank + l3 -> 32 columns, byte p of a word is label bit beta(p): register t of the lo plane is
@@ -508,11 +525,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             if (tp < 2) {
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur >> (4 * tp + t)) & 0x01010101u;
-                                sts128((tp == 0 ? pbB : pbB1) + 8192, make_uint4(q[0], q[1], q[2], q[3]));
+                                sts128((tp == 0 ? pbB : pbB1) + kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
                                 if (NQ == 2) {
 #pragma unroll
                                     for (int t = 0; t < 4; ++t) q[t] = (mcur2 >> (4 * tp + t)) & 0x01010101u;
-                                    sts128((tp == 0 ? pbB : pbB1) + 16384 + 8192, make_uint4(q[0], q[1], q[2], q[3]));
+                                    sts128((tp == 0 ? pbB : pbB1) + 3 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
                                 }
                             } else {
 #pragma unroll
@@ -521,7 +538,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                                 if (NQ == 2) {
 #pragma unroll
                                     for (int t = 0; t < 4; ++t) q[t] = (mcur2 << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
-                                    sts128((tp == 2 ? pbB : pbB1) + 16384, make_uint4(q[0], q[1], q[2], q[3]));
+                                    sts128((tp == 2 ? pbB : pbB1) + 2 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
                                 }
                             }
                         }
@@ -555,8 +572,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             hi.x = __byte_perm(pk[r][0], pk[r][1], 0x7632);
                             hi.y = __byte_perm(pk[r][2], pk[r][3], 0x7632);
                             // row m = mrow0 + 16 r: 8-row group m >> 3 advances by 2 (1024 bytes), the swizzle phase is that of mrow0
-                            sts64(paA + 1024 * r, hi);
-                            sts64(paA + kTM * kKB + 1024 * r, lo);
+                            sts64(paA + (ET_TC_A32 ? 512 : 1024) * r, hi);
+                            sts64(paA + kTM * kKB + (ET_TC_A32 ? 512 : 1024) * r, lo);
                         }
                     }
                 };
@@ -564,8 +581,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 else tile(std::false_type{});
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * (it & (kStages - 1)), 0));
-                const bool wrapS = ((it + 1) & (kStages - 1)) == 0, wrapJ = ((it + 1) & (kRecSlots - 1)) == 0;
+                if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * st, 0));
+                const bool wrapS = st == kStages - 1, wrapJ = ((it + 1) & (kRecSlots - 1)) == 0;
+                st = wrapS ? 0 : st + 1;
+                pe ^= wrapS ? 1u : 0u;
                 paA += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
                 pbB += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
                 pjJ += wrapJ ? kRecSlotBytes - kRecSlots * kRecSlotBytes : kRecSlotBytes;
@@ -585,7 +604,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 if (WEIGHTED) { wi = (Acc)wf; zi = wi * (Acc)yones; }
                 else { wi = 1; zi = (Acc)yones; }
 #pragma unroll 1
-                for (int g = 0; g < G; ++g) {
+                for (int g = 0; g < ngrp; ++g) {
                     const uint32_t mword = __ldg(mp + grp0 + g);
                     uint32_t v[32];
                     tmem_ld32(taddr + 32 * (grp0 + g), v);
@@ -629,11 +648,14 @@ __global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= kCols) return;
     constexpr int G = kEpiGroups;
-    const int gc = c >> 5, g = gc % G, lane = c & 31;
+    const int gc = c >> 5, lane = c & 31;
+    int e = 0;  // warp row that reads column group gc in the epilogue
+    while (e + 1 < kEpiWarps && epi_first(e + 1) <= gc) ++e;
+    const int g = gc - epi_first(e);
     const Acc *p = reinterpret_cast<const Acc *>(partial);
     Acc sq = 0, sr = 0;
     for (int b = 0; b < ncta; ++b)
-        for (int w = 4 * (gc / G); w < 4 * (gc / G) + 4; ++w) {
+        for (int w = 4 * e; w < 4 * e + 4; ++w) {
             const Acc *e = p + (((long long)b * kProducerWarps + w) * G * 32 + g * 32 + lane) * 2;
             sq += e[0];
             sr += e[1];
