@@ -108,8 +108,8 @@ class ClockSampler:
 
 def ncu_traffic(kernel: str, cfg_index: int, default_nperm: bool):
     """DRAM bytes per launch (read + write) of `kernel` from the committed ncu capture of this workload, or None.
-    Only the default configs[4] workload has one (profiles/r01f_README.md names the command)."""
-    path = os.path.join(ROOT, "profiles", "r01f_traffic_k_perm_tc_cfg4.csv")
+    Only the default configs[4] workload has one (profiles/r01g_README.md names the command)."""
+    path = os.path.join(ROOT, "profiles", "r01g_traffic_k_perm_tc_cfg4.csv")
     if kernel != "k_perm_tc" or cfg_index != 4 or not default_nperm or not os.path.exists(path):
         return None, None
     import csv
@@ -121,7 +121,7 @@ def ncu_traffic(kernel: str, cfg_index: int, default_nperm: bool):
                 per_launch[r["ID"]] = per_launch.get(r["ID"], 0.0) + float(r["Metric Value"].replace(",", ""))
     if not per_launch:
         return None, None
-    return sum(per_launch.values()) / len(per_launch), "profiles/r01f_traffic_k_perm_tc_cfg4.csv (ncu, bytes per launch)"
+    return sum(per_launch.values()) / len(per_launch), "profiles/r01g_traffic_k_perm_tc_cfg4.csv (ncu, bytes per launch)"
 
 
 def pinned(a: np.ndarray):

@@ -7,17 +7,18 @@
 //   R_c = sum_{i<j} w_i w_j psi_ij (a_ic + a_jc)       = sum_i real_i w_i Y_ic + sum_i a_ic w_i Y_i,ones
 //   S   = sum_{i<j} w_i w_j psi_ij                     = Q of the all-ones column
 // and S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q.  Y = Psi A is a GEMM whose left operand is
-// never stored.  A cluster of two CTAs (one SM pair) works on a 256-row tile; per block of 64 j each CTA evaluates its
-// 128 x 64 tile of psi in fp32 (packed FFMA2 + MUFU.EX2; the j side comes as pre-formatted pair records that a loader
-// warp bulk-copies into a shared-memory ring), quantises Psi_ij = w_j psi_ij to a 15-bit fixed-point integer
-// v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7) into its shared memory in the UMMA K-major SWIZZLE_64B
-// layout, and expands ITS HALF of the label columns from the bit masks into the B tile (bytes 128 a and a, MN-major
-// SWIZZLE_128B).  One thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M = 256, N = 256, K = 32):
-// the pair's tensor cores read A from their own SM and each half of B from one SM of the pair, so a label byte is
-// written and read once per 256 rows instead of once per 128.  The kernel is bound by the CUDA-core tile generation
-// (16 producer warps per CTA), not by the tensor pipe: profiles/r01c_README.md.  Accumulation is ONE int32 per column
-// in TMEM (all 512 columns of each SM).  Integer accumulation is exact, so S, R and Q are sums of the SAME quantised
-// Psi whatever the schedule (hard part 3 "consistency"), and the unweighted result is bit-reproducible.
+// never stored.  A cluster of two CTAs (one SM pair) works on a 256-row tile; per K block of 96 j each CTA evaluates its
+// 128 x 96 tile of psi in fp32 (packed FFMA2 + MUFU.EX2, 12 producer warps, 4 rows x 8 j per thread; the j side comes
+// as pre-formatted pair records that a loader warp bulk-copies into a shared-memory ring), quantises
+// Psi_ij = w_j psi_ij to a 15-bit fixed-point integer v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7) into
+// its shared memory as K chunks of 32 bytes in the UMMA K-major SWIZZLE_32B layout, and expands ITS HALF of the label
+// columns from the bit masks into the B tile (bytes 128 a and a, MN-major SWIZZLE_128B).  One thread of the leader CTA
+// issues tcgen05.mma.cta_group::2.kind::i8 (M = 256, N = 256, K = 32): the pair's tensor cores read A from their own
+// SM and each half of B from one SM of the pair, so a label byte is written and read once per 256 rows instead of
+// once per 128.  The kernel is bound by the CUDA-core tile generation, not by the tensor pipe
+// (profiles/r01g_README.md).  Accumulation is ONE int32 per column in TMEM (all 512 columns of each SM).  Integer
+// accumulation is exact, so S, R and Q are sums of the SAME quantised Psi whatever the schedule (hard part 3
+// "consistency"), and the unweighted result is bit-reproducible.
 //
 // Columns of one launch (512): 0 = observed labelling, 1 = second labelling (P-even grouping of Sect. 5, else a copy
 // of column 0), 2 = all ones, 3.. = 509 permutations.  Inside a 32-column mask word the B tile / TMEM column p holds
