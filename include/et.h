@@ -69,9 +69,13 @@ typedef struct {
     et_result observed;
     double p_value;   /* count_gt / nperm  (strict >; reading R3)                   */
     int64_t count_gt; /* #{p : T_p > T_obs}                                                       */
-    int64_t n_near;   /* #{p : |T_p - T_obs| <= guard} or T_p NaN (R5, R10); guard = 1e-9 (|T_xx|+
-                         |T_bb|+|T_xb|), plus, on the tensor-core path, 8 sigma of the 15-bit
-                         quantisation noise of T_p - T_obs.  count_gt is exact when 0 */
+    int64_t n_near;   /* permutations whose side of T_obs the arithmetic cannot certify (R5, R10):
+                         #{p : |T_p - T_obs| <= guard} or T_p NaN, guard = 8 sigma of the error model
+                         of T_p - T_obs (fp32 psi; on the tensor-core path
+                         also the 15-bit rounding).  With ET_OPT_EXACT_P (default on) the
+                         tensor-core path re-evaluates the permutations inside its band in the
+                         fp32-pair / fp64-sum arithmetic of et_T and n_near is what is left after
+                         that.  count_gt equals the oracle's count when n_near = 0             */
     int64_t nperm;
 } et_perm_result;
 
@@ -95,6 +99,12 @@ typedef struct {
                                   (CUDA-core kernels: unique pairs x (2 dim + 1), per mask word
                                   unique pairs x (2 dim + 32)) or 2 x MACs (tensor-core kernel)     */
     char dominant_kernel[32];  /* "k_pairs_T", "k_pairs_rows", "k_perm32", "k_perm_tc" or ""       */
+    int64_t dominant_ops_executed; /* k_perm_tc: the same count over the label columns the launches
+                                  carried (256 or 512 per launch, the three special columns in every
+                                  launch); 0 for the other kernels                                  */
+    double ms_escalation;      /* device time of the guard-band escalation (ET_OPT_EXACT_P)         */
+    int64_t n_near_before;     /* n_near of the tensor-core pass, before the escalation             */
+    int64_t n_escalated;       /* permutations re-evaluated by the escalation                       */
 } et_stats;
 
 /* Options for et_set_option. */
@@ -102,12 +112,19 @@ typedef enum {
     ET_OPT_PERM_KERNEL = 0, /* permutation sums: 0 (default) = tensor-core contraction (tcgen05
                                kind::i8, psi quantised to 15 bits, exact integer sums) when the
                                padded pooled size is >= 16384 rows, else the fp32 CUDA-core
-                               kernel; 1 = always CUDA cores; 2 = always tensor cores            */
-    ET_OPT_PERM_OFFSET = 1  /* first permutation index p0 (default 0): the calls evaluate
+                               kernel; 1 = always CUDA cores; 2 = always tensor cores (below
+                               16384 rows the 15-bit rounding noise can exceed the 1e-6 tolerance
+                               of T: a test hook)                       */
+    ET_OPT_PERM_OFFSET = 1, /* first permutation index p0 (default 0): the calls evaluate
                                permutations p0 .. p0+nperm-1 of the seed's stream, T_perm[k] is
                                permutation p0+k.  Permutation p depends only on (seed, p), so
                                disjoint ranges on several GPUs / calls form one test
-                               (PAPER.md:219 farms permutations out the same way)                 */
+                               (PAPER.md:219 farms permutations out the same way).
+                               p0 + nperm must stay below 2^34                                    */
+    ET_OPT_EXACT_P = 2      /* guard-band escalation of the tensor-core path: re-evaluate up to this
+                               many permutations (default 16, at most 64; 0 = off) whose T_p lies
+                               inside the guard band of T_obs, one 5/8 all-pairs pass each on the
+                               CUDA cores (a full pass when weighted); skipped when more are inside  */
 } et_option;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t to
@@ -117,6 +134,18 @@ void et_destroy(et_ctx *ctx);
 /* Context-owned explanation of the last non-OK status; never freed by the caller. */
 const char *et_last_error(const et_ctx *ctx);
 et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value);
+
+/* Unit-range shard over `world` contexts (one per GPU / process): the context evaluates
+ * every world-th work unit of the O(N^2) kernels (the tile-pair list of et_T, the unit table of the tensor-core
+ * permutation sums) and completes its partial sums -- exact int64 column sums when unweighted, doubles otherwise --
+ * through `fn`: buf is HOST memory [world][bytes_per_rank] with slice `rank` filled in; fn must return 0 with every
+ * slice filled with that rank's bytes (an all-gather, e.g. over NCCL or gloo; the binding supplies one on
+ * torch.distributed).  The slices are summed in rank order on the device, so all ranks return identical results;
+ * unweighted results do not depend on `world` at all (integer sums).  Labels, prep and the O(N) kernels are
+ * replicated; every rank must make the same calls with the same arguments.  world = 1 (fn may be NULL) switches the
+ * shard off.  The small-N CUDA-core permutation kernels are not sharded (every rank evaluates them in full). */
+typedef int (*et_allgather_fn)(void *user, void *buf, int64_t bytes_per_rank);
+et_status et_set_shard(et_ctx *ctx, int rank, int world, et_allgather_fn fn, void *user);
 et_status et_get_stats(const et_ctx *ctx, et_stats *out);
 const char *et_version(void);
 

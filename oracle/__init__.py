@@ -204,6 +204,16 @@ def T_bkg(x, xbar, bx, bxbar, b: float, bbar: float, sigma: float) -> float:
 BKG_SEED_XOR = 0x9E3779B97F4A7C15  # reading R18: the background pool draws from the stream of seed ^ this constant
 
 
+def bkg_perm_purity(b: float, bbar: float, n: int, nbar: int):
+    """Reading R18: the numbers of background events (b', bbar') that Eq. 3 subtracts from the PERMUTED main samples.
+    A random reassignment of the n + nbar pooled main events, b + bbar of which are background, to samples of sizes n
+    and nbar puts (b + bbar) n / (n + nbar) background events into X' and (b + bbar) nbar / (n + nbar) into Xbar' on
+    average (the purities are consistent for the permuted samples).  Pinned in tests/test_oracle_pins.py by
+    enumerating every split of a tagged pool (n != nbar, so that a swapped formula fails)."""
+    tot = b + bbar
+    return tot * n / (n + nbar), tot * nbar / (n + nbar)
+
+
 def bkg_perm_test(x, xbar, bx, bxbar, b: float, bbar: float, sigma: float, nperm: int, seed: int):
     """Permutation test with Eq. 3 as the statistic ("using the same method to remove background from the
     randomly permuted samples"; reading R18).  Permutation p reassigns the pooled main events to main samples of sizes
@@ -217,7 +227,7 @@ def bkg_perm_test(x, xbar, bx, bxbar, b: float, bbar: float, sigma: float, nperm
     main, side = np.vstack([x, xbar]), np.vstack([bx, bxbar])
     am = labels_range(n + nbar, n, 0, nperm, seed)
     ab = labels_range(bs + bsbar, bs, 0, nperm, seed ^ BKG_SEED_XOR)
-    bp, bbp = (b + bbar) * n / (n + nbar), (b + bbar) * nbar / (n + nbar)
+    bp, bbp = bkg_perm_purity(b, bbar, n, nbar)
     t_perm = np.empty(nperm)
     for p in range(nperm):
         t_perm[p] = T_bkg(main[am[p] == 1], main[am[p] == 0], side[ab[p] == 1], side[ab[p] == 0], bp, bbp, sigma)

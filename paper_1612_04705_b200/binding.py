@@ -22,11 +22,12 @@ ET_F32, ET_F64 = 0, 1
 ET_HOST, ET_DEVICE = 0, 1
 ET_OPT_PERM_KERNEL = 0
 ET_OPT_PERM_OFFSET = 1
+ET_OPT_EXACT_P = 2
 STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ERR_NONFINITE", -4: "ET_ERR_DEGENERATE",
                 -5: "ET_ERR_NOMEM", -6: "ET_ERR_CUDA"}
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
-SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_get_stats", "et_version", "et_T",
+SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_set_shard", "et_get_stats", "et_version", "et_T",
            "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
 
 
@@ -69,7 +70,8 @@ class _GevResult(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [("ms_total", C.c_double), ("ms_pairs", C.c_double), ("ms_labels", C.c_double), ("launches", C.c_int64),
                 ("pair_evals", C.c_int64), ("ms_dominant", C.c_double), ("dominant_launches", C.c_int64),
-                ("dominant_ops", C.c_int64), ("dominant_kernel", C.c_char * 32)]
+                ("dominant_ops", C.c_int64), ("dominant_kernel", C.c_char * 32), ("dominant_ops_executed", C.c_int64),
+                ("ms_escalation", C.c_double), ("n_near_before", C.c_int64), ("n_escalated", C.c_int64)]
 
 
 @dataclass
@@ -156,7 +158,6 @@ def gev_pvalue(T_perm, T_obs: float, z=None) -> GevResult:
     zz = None if z is None else np.ascontiguousarray(np.asarray(z, dtype=np.float64).reshape(-1, 3))
     out = _GevResult()
     L = lib()
-    L.et_gev_pvalue.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_int64, C.c_void_p]
     st = L.et_gev_pvalue(tp.ctypes.data_as(C.c_void_p), len(tp), float(T_obs), None if zz is None else zz.ctypes.data_as(C.c_void_p),
                          0 if zz is None else len(zz), C.byref(out))
     if st != ET_OK:
@@ -176,6 +177,10 @@ class Stats:
     dominant_launches: int = 0
     dominant_ops: int = 0
     dominant_kernel: str = ""
+    dominant_ops_executed: int = 0
+    ms_escalation: float = 0.0
+    n_near_before: int = 0
+    n_escalated: int = 0
 
 
 _lib = None
@@ -189,12 +194,33 @@ def lib():
             raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1612_04705_b200.build` "
                               "(there is no CPU fallback)")
         L = C.CDLL(LIB_PATH)
+        vp, i64, u64, dbl, ci = C.c_void_p, C.c_int64, C.c_uint64, C.c_double, C.c_int
         L.et_last_error.restype = C.c_char_p
-        L.et_last_error.argtypes = [C.c_void_p]
         L.et_version.restype = C.c_char_p
-        L.et_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
-        L.et_destroy.argtypes = [C.c_void_p]
         L.et_destroy.restype = None
+        # the argument types of EVERY entry point of include/et.h, in its order (a missing one would let ctypes pass a
+        # Python int as a 32-bit C int and truncate an int64 silently)
+        sample = [vp, i64, vp, i64]                       # x, n, xbar, nbar
+        wsample = [vp, vp, i64, vp, vp, i64]              # x, wx, n, xbar, wxbar, nbar
+        tail = [ci, ci, ci, dbl]                          # dim, dtype, mem, sigma
+        bkg = [vp] + sample + [vp, i64, vp, i64, dbl, dbl] + tail
+        for name, args in {
+            "et_create": [C.POINTER(vp), ci, vp], "et_destroy": [vp], "et_last_error": [vp], "et_version": [],
+            "et_set_option": [vp, ci, i64], "et_set_shard": [vp, ci, ci, vp, vp], "et_get_stats": [vp, vp],
+            "et_T": [vp] + sample + tail + [vp],
+            "et_T_weighted": [vp] + wsample + tail + [vp],
+            "et_T_sigmas": [vp] + wsample + [ci, ci, ci, vp, ci, vp],
+            "et_T_bkg": bkg + [vp],
+            "et_bkg_permutation_test": bkg + [i64, u64, vp, vp],
+            "et_gev_pvalue": [vp, i64, dbl, vp, i64, vp],
+            "et_permutation_test": [vp] + wsample + tail + [i64, u64, vp, vp],
+            "et_podd_split": [vp, vp, vp, vp, i64, ci, ci, vp, vp],
+            "et_podd_test": [vp] + wsample + tail + [i64, u64, vp, vp],
+            "et_perm_labels": [vp, i64, i64, i64, u64, ci, vp],
+            "et_row_sums": [vp] + wsample + tail + [vp, i64, vp, vp],
+        }.items():
+            getattr(L, name).argtypes = args
+        assert all(getattr(L, n).argtypes is not None for n in SYMBOLS)
         _lib = L
     return _lib
 
@@ -237,6 +263,21 @@ def _marshal(a, want=None) -> _Arr:
     return _Arr(C.c_void_p(a.ctypes.data), dt, ET_HOST, a.shape, a)
 
 
+def _aux(a, shape, mem, what, device=None) -> _Arr:
+    """A double-precision companion array (weights, momenta): must have exactly `shape` and live where the coordinates
+    live, or the library would read past its end."""
+    r = _marshal(a, "f64")
+    if r.ptr is None:
+        return r
+    if tuple(r.shape) != tuple(shape):
+        raise ValueError(f"{what} must have shape {tuple(shape)}, got {tuple(r.shape)}")
+    if r.mem != mem:
+        raise ValueError(f"{what} must live where the coordinates live")
+    if device is not None and r.mem == ET_DEVICE and r.keep.device.index != device:
+        raise ValueError(f"{what} is on cuda:{r.keep.device.index}, the coordinates on cuda:{device}")
+    return r
+
+
 def _coords(x, xbar):
     ax, ab = _marshal(x), _marshal(xbar)
     if ax.mem != ab.mem or ax.dtype != ab.dtype:
@@ -245,7 +286,49 @@ def _coords(x, xbar):
         ax.shape, ab.shape = (ax.shape[0], 1), (ab.shape[0], 1)
     if len(ax.shape) != 2 or len(ab.shape) != 2 or ax.shape[1] != ab.shape[1]:
         raise ValueError("x and xbar must be [n, dim] and [nbar, dim]")
+    if ax.mem == ET_DEVICE and ax.keep.device != ab.keep.device:
+        raise ValueError("x and xbar must be on the same CUDA device")
     return ax, ab
+
+
+def _weights(ax, ab, wx, wxbar):
+    if (wx is None) != (wxbar is None):
+        raise ValueError("give both weight arrays or neither")
+    dev = ax.keep.device.index if ax.mem == ET_DEVICE else None
+    return _aux(wx, (ax.shape[0],), ax.mem, "wx", dev), _aux(wxbar, (ab.shape[0],), ax.mem, "wxbar", dev)
+
+
+_ALLGATHER = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64)
+
+
+def make_allgather(rank: int, world: int, group=None):
+    """The et_allgather_fn of include/et.h on torch.distributed: buf is host memory [world][nbytes] with slice `rank`
+    filled in; on return every slice holds that rank's bytes.  Pure data movement (no arithmetic): the library sums the
+    slices on the device.  NCCL moves device tensors, so there the slices travel through a small CUDA staging tensor."""
+    def fn(_user, buf, nbytes):
+        try:
+            import torch
+            import torch.distributed as dist
+
+            raw = (C.c_uint8 * (world * nbytes)).from_address(buf)
+            host = torch.frombuffer(raw, dtype=torch.uint8).view(world, nbytes)
+            if dist.get_backend(group) == "nccl":
+                mine = host[rank].cuda()
+                parts = torch.empty(world, nbytes, dtype=torch.uint8, device=mine.device)
+                dist.all_gather_into_tensor(parts, mine, group=group)
+                host.copy_(parts.cpu())
+            else:
+                parts = [torch.empty(nbytes, dtype=torch.uint8) for _ in range(world)]
+                dist.all_gather(parts, host[rank].clone(), group=group)
+                for r in range(world):
+                    host[r].copy_(parts[r])
+            return 0
+        except Exception:  # an exception must not unwind through the C caller
+            import traceback
+
+            traceback.print_exc()
+            return 1
+    return fn
 
 
 class Context:
@@ -286,11 +369,23 @@ class Context:
     def set_option(self, opt: int, value: int):
         self._check(lib().et_set_option(self._h, C.c_int(opt), C.c_int64(value)))
 
+    def set_shard(self, rank: int, world: int, group=None):
+        """Unit-range shard over the ranks of a torch.distributed process group (et_set_shard): this context evaluates
+        every world-th work unit of the O(N^2) kernels, and the library's partial sums are completed by an all-gather on
+        `group` (NCCL or gloo).  world = 1 switches the shard off."""
+        if world <= 1:
+            self._shard_cb = None
+            self._check(lib().et_set_shard(self._h, 0, 1, None, None))
+            return
+        self._shard_cb = _ALLGATHER(make_allgather(rank, world, group))
+        self._check(lib().et_set_shard(self._h, rank, world, C.cast(self._shard_cb, C.c_void_p), None))
+
     def stats(self) -> Stats:
         s = _Stats()
         self._check(lib().et_get_stats(self._h, C.byref(s)))
         return Stats(s.ms_total, s.ms_pairs, s.ms_labels, s.launches, s.pair_evals, s.ms_dominant, s.dominant_launches,
-                     s.dominant_ops, s.dominant_kernel.decode())
+                     s.dominant_ops, s.dominant_kernel.decode(), s.dominant_ops_executed, s.ms_escalation, s.n_near_before,
+                     s.n_escalated)
 
     # ---------------------------------------------------------------- Eq. 2
     def T(self, x, xbar, sigma: float) -> Result:
@@ -302,9 +397,9 @@ class Context:
 
     def T_weighted(self, x, wx, xbar, wxbar, sigma: float) -> Result:
         ax, ab = _coords(x, xbar)
-        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
-        if awx.mem != ax.mem or awb.mem != ax.mem:
-            raise ValueError("weights must live where the coordinates live")
+        if wx is None or wxbar is None:
+            raise ValueError("T_weighted needs both weight arrays")
+        awx, awb = _weights(ax, ab, wx, wxbar)
         out = _Result()
         self._check(lib().et_T_weighted(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
                                         C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_int(ax.mem), C.c_double(sigma), C.byref(out)))
@@ -313,9 +408,7 @@ class Context:
     def T_sigmas(self, x, xbar, sigmas, wx=None, wxbar=None) -> list:
         """Eq. 2 (weighted if wx, wxbar are given) for up to four sigma values from one pass over the pairs."""
         ax, ab = _coords(x, xbar)
-        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
-        if wx is not None and (awx.mem != ax.mem or awb.mem != ax.mem):
-            raise ValueError("weights must live where the coordinates live")
+        awx, awb = _weights(ax, ab, wx, wxbar)
         sg = np.ascontiguousarray(np.asarray(sigmas, dtype=np.float64))
         out = (_Result * max(len(sg), 1))()
         self._check(lib().et_T_sigmas(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),
@@ -354,9 +447,7 @@ class Context:
     # ---------------------------------------------------------------- permutation test
     def permutation_test(self, x, xbar, sigma: float, nperm: int, seed: int, wx=None, wxbar=None) -> PermResult:
         ax, ab = _coords(x, xbar)
-        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
-        if wx is not None and (awx.mem != ax.mem or awb.mem != ax.mem):
-            raise ValueError("weights must live where the coordinates live")
+        awx, awb = _weights(ax, ab, wx, wxbar)
         Tp = np.zeros(max(int(nperm), 1), dtype=np.float64)
         out = _PermResult()
         self._check(lib().et_permutation_test(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr,
@@ -369,6 +460,8 @@ class Context:
     def podd_split(self, pB, pC, pD, is_conjugate: bool):
         aB, aC, aD = _marshal(pB, "f64"), _marshal(pC, "f64"), _marshal(pD, "f64")
         n = aB.shape[0]
+        if not (tuple(aB.shape) == tuple(aC.shape) == tuple(aD.shape) == (n, 3)) or not (aB.mem == aC.mem == aD.mem):
+            raise ValueError("pB, pC, pD must be [n, 3] arrays in the same memory space")
         cnt = C.c_int64(0)
         if aB.mem == ET_DEVICE:
             import torch
@@ -384,9 +477,11 @@ class Context:
 
     def podd_test(self, x, mom_x, xbar, mom_xbar, sigma: float, nperm: int, seed: int) -> PoddResult:
         ax, ab = _coords(x, xbar)
-        amx, amb = _marshal(mom_x, "f64"), _marshal(mom_xbar, "f64")
-        if amx.mem != ax.mem or amb.mem != ax.mem:
-            raise ValueError("momenta must live where the coordinates live")
+        dev = ax.keep.device.index if ax.mem == ET_DEVICE else None
+        amx = _aux(mom_x, (ax.shape[0], 3, 3), ax.mem, "mom_x", dev)
+        amb = _aux(mom_xbar, (ab.shape[0], 3, 3), ax.mem, "mom_xbar", dev)
+        if amx.ptr is None or amb.ptr is None:
+            raise ValueError("podd_test needs the momenta of both samples")
         Tp = np.zeros(max(int(nperm), 1), dtype=np.float64)
         out = _PoddResult()
         self._check(lib().et_podd_test(self._h, ax.ptr, amx.ptr, C.c_int64(ax.shape[0]), ab.ptr, amb.ptr, C.c_int64(ab.shape[0]),
@@ -405,7 +500,7 @@ class Context:
 
     def row_sums(self, x, xbar, sigma: float, rows, wx=None, wxbar=None):
         ax, ab = _coords(x, xbar)
-        awx, awb = _marshal(wx, "f64"), _marshal(wxbar, "f64")
+        awx, awb = _weights(ax, ab, wx, wxbar)
         rows = np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
         rx, rb = np.zeros(len(rows)), np.zeros(len(rows))
         self._check(lib().et_row_sums(self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]),

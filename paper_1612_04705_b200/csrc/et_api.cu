@@ -57,8 +57,16 @@ struct et_ctx {
     int64_t kc_ops[4] = {0, 0, 0, 0};
     int64_t opt_perm_kernel = 0;
     int64_t opt_perm_offset = 0;
+    int64_t opt_exact_p = 16;       // guard-band escalation: re-evaluate up to this many near permutations (0 = off)
+    // unit-range shard (et_set_shard): this context evaluates work units u = shard_rank (mod shard_world) of the O(N^2)
+    // kernels and completes the partial sums through the caller's all-gather
+    int shard_rank = 0, shard_world = 1;
+    et_allgather_fn shard_fn = nullptr;
+    void *shard_user = nullptr;
+    Buf shardbuf;
+    Buf rec2, tilecls2, esccls, escD, nearbuf, escw;
     double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
-    Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP;
+    Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     bool tc_attr_set = false;
 };
 
@@ -174,14 +182,15 @@ void layout_four(Layout &L, long long n, long long nbar, const long long cnt[4])
     L.n_a = cnt[0] + cnt[1];
 }
 
-et_status upload_tile_classes(et_ctx *ctx, const Layout &L)
+et_status upload_tile_classes(et_ctx *ctx, const Layout &L, Buf *dst = nullptr)
 {
+    Buf &b = dst ? *dst : ctx->tilecls;
     const long long nt = L.npad / kPad;
     std::vector<uint8_t> cls((size_t)nt);
     for (int c = 0; c < L.ncls; ++c)
         for (long long t = L.seg_pos[c] / kPad; t < L.seg_pos[c + 1] / kPad; ++t) cls[(size_t)t] = (uint8_t)c;
-    ET_TRY(ensure(ctx, ctx->tilecls, (size_t)nt));
-    CUDA_TRY(cudaMemcpyAsync(ctx->tilecls.p, cls.data(), (size_t)nt, cudaMemcpyHostToDevice, ctx->stream));
+    ET_TRY(ensure(ctx, b, (size_t)nt));
+    CUDA_TRY(cudaMemcpyAsync(b.p, cls.data(), (size_t)nt, cudaMemcpyHostToDevice, ctx->stream));
     CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // cls goes out of scope
     return ET_OK;
 }
@@ -301,27 +310,35 @@ int resident_blocks(et_ctx *ctx, K kernel)
 constexpr int kRT = 4;    // rows per thread in K-T (i-tile = 1024 rows = kPad)
 constexpr int kRRow = 2;  // rows per thread in K-ROW (i-tile = 512 rows)
 
-// K-T: class-pair sums into ctx->sums (device, kSumSlots doubles).
-et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim)
+et_status shard_sum(et_ctx *ctx, void *dev, int count, bool is_f64);
+
+// K-T: class-pair sums into ctx->sums (device, kSumSlots doubles).  rec / tilecls default to the call's own layout;
+// skip_mask drops class pairs (k_pairs_T); `booked` = false keeps the pass out of the per-kernel-class statistics (the
+// escalation books its own time).
+et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim, const float *rec = nullptr, const uint8_t *tilecls = nullptr,
+                      unsigned skip_mask = 0u, bool booked = true)
 {
+    if (!rec) rec = static_cast<const float *>(ctx->rec.p);
+    if (!tilecls) tilecls = static_cast<const uint8_t *>(ctx->tilecls.p);
     const int nT = (int)(L.npad / (kThreads * kRT));
     const long long nunits = (long long)nT * (nT + 1) / 2;
     ET_TRY(ensure(ctx, ctx->sums, kSumSlots * sizeof(double)));
-    ET_TRY(span_begin(ctx, 2));
+    if (booked) ET_TRY(span_begin(ctx, 2));
     DISPATCH_DIM(dim, {
         int grid = resident_blocks(ctx, k_pairs_T<D, kRT>);
-        if ((long long)grid > nunits) grid = (int)nunits;
+        const long long mine = (nunits - ctx->shard_rank + ctx->shard_world - 1) / ctx->shard_world;  // units of this rank
+        if ((long long)grid > mine) grid = (int)std::max<long long>(mine, 1);
         ET_TRY(ensure(ctx, ctx->partials, (size_t)grid * kSumSlots * sizeof(double)));
-        k_pairs_T<D, kRT><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), nT,
-                                                             static_cast<const uint8_t *>(ctx->tilecls.p), nunits,
+        k_pairs_T<D, kRT><<<grid, kThreads, 0, ctx->stream>>>(rec, nT, tilecls, nunits, skip_mask, ctx->shard_rank, ctx->shard_world,
                                                              static_cast<double *>(ctx->partials.p));
         LAUNCH_CHECK();
         k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partials.p), grid, kSumSlots,
                                                  static_cast<double *>(ctx->sums.p));
         LAUNCH_CHECK();
     });
-    ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_T, 1, L.N * (L.N - 1) / 2 * (2 * dim + 1)));
-    ctx->stats.pair_evals += nunits * (long long)(kThreads * kRT) * (kThreads * kRT);
+    if (booked) ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_T, 1, L.N * (L.N - 1) / 2 * (2 * dim + 1)));
+    ctx->stats.pair_evals += nunits * (long long)(kThreads * kRT) * (kThreads * kRT) / ctx->shard_world;
+    if (ctx->shard_world > 1) ET_TRY(shard_sum(ctx, ctx->sums.p, kSumSlots, true));
     return ET_OK;
 }
 
@@ -510,15 +527,39 @@ __global__ void k_sym_class_sums(const double *__restrict__ M, int ncls, double 
             S[c1 * 4 + c2] = c1 == c2 ? 0.5 * M[c1 * 4 + c1] : 0.5 * (M[c1 * 4 + c2] + M[c2 * 4 + c1]);
 }
 
+// Guard band of the decision T_p > T_obs (reading R5 of DESIGN.md): 8 sigma of the noise of T_p - T_obs under the error
+// model of the arithmetic.  Every pair's Psi_ij = w_i w_j psi_ij carries an independent absolute error of standard
+// deviation `pair_err` (fp32 path: 2^-22 wabs^2 -- ex2.approx is good to 2 ulp and psi <= 1; tensor-core path: that and
+// the 15-bit rounding), so var(T) = pair_err^2 [ pairs_xx / (W(W-1))^2 + pairs_bb / (Wb(Wb-1))^2 + pairs_xb / (W Wb)^2 ]
+// and the difference of two labellings that share the psi values has twice that.  1e-13 of the term scale covers the
+// fp64 summation order.  The achieved errors are asserted against this band in tests/test_gpu_parity.py.
+constexpr double kPairErrF32 = 2.384185791015625e-07;  // 2^-22
+__device__ double guard_band(double pair_err, double nA, double nB, double Wo, double Wb, double scale)
+{
+    const double var = 0.5 * nA * (nA - 1.0) / ((Wo * (Wo - 1.0)) * (Wo * (Wo - 1.0))) + 0.5 * nB * (nB - 1.0) / ((Wb * (Wb - 1.0)) * (Wb * (Wb - 1.0))) +
+                       nA * nB / ((Wo * Wb) * (Wo * Wb));
+    return 1e-13 * scale + 8.0 * 1.4142135623730951 * pair_err * sqrt(var);
+}
+
+// Permutations inside the guard band, for the escalation (finite T_p only; NaN permutations cannot be decided).
+constexpr int kMaxNear = 64;
+struct DevNear {
+    int n_finite;          // near permutations with a finite T_p (all of them, also beyond kMaxNear)
+    int n_nan;             // degenerate weighted splits (T_p = NaN)
+    int idx[kMaxNear];     // local permutation indices of the first kMaxNear (unordered)
+    double guard;          // the band used
+    double guard_f32;      // the band of the fp32-pair / fp64-sum arithmetic (what the escalation certifies)
+};
+
 // Permutation statistic (H6): columns c = 0 (observed) and c = p + 1.  From Q_c, R_c, W_c, S = RW_all / 2, Wtot:
 //   S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q  (SURVEY 8(a) identity), Eq. 2 with W = W_c, Wbar = Wtot - W_c.
-// Then count = #{T_p > T_obs}, n_near = #{|T_p - T_obs| <= 1e-9 * term scale, or T_p NaN}.
+// Then count = #{T_p > T_obs}, n_near = #{|T_p - T_obs| <= guard, or T_p NaN}.
 struct DevPerm {
     et_perm_result r;
     int status;
 };
 __global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q, const double *__restrict__ RW, int nwords, int nperm,
-                                                  long long npairs, double *__restrict__ T_perm, DevPerm *out)
+                                                  long long npairs, double nA, double nB, double wabs, double *__restrict__ T_perm, DevPerm *out)
 {
     // RW layout: [g][which][kRWCols]
     __shared__ DevT obs;
@@ -533,7 +574,7 @@ __global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q,
     }
     __syncthreads();
     const double Tobs = obs.r.T;
-    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb));
+    const double guard = guard_band(kPairErrF32 * wabs * wabs, nA, nB, obs.r.W, obs.r.Wbar, fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb));
     unsigned long long cnt = 0, near = 0;
     for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
         const int c = p + 1, g = c >> 5, b = c & 31;
@@ -609,16 +650,16 @@ __global__ void k_src_runs(PrepParams P, const long long *__restrict__ unused, i
     }
 }
 
-et_status run_class_weights(et_ctx *ctx, const Layout &L, int dim)
+et_status run_class_weights(et_ctx *ctx, const Layout &L, int dim, const float *rec = nullptr, const uint8_t *tilecls = nullptr)
 {
+    if (!rec) rec = static_cast<const float *>(ctx->rec.p);
+    if (!tilecls) tilecls = static_cast<const uint8_t *>(ctx->tilecls.p);
     const int nt = (int)(L.npad / kPad);
     ET_TRY(ensure(ctx, ctx->clssum, (size_t)nt * 4 * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->clsw, kMaxCls * sizeof(double)));
-    k_tile_weights<<<nt, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
-                                                    static_cast<double *>(ctx->clssum.p));
+    k_tile_weights<<<nt, kThreads, 0, ctx->stream>>>(rec, rec_floats(dim), dim, static_cast<double *>(ctx->clssum.p));
     LAUNCH_CHECK();
-    k_reduce_by_class<<<1, kMaxCls, 0, ctx->stream>>>(static_cast<const double *>(ctx->clssum.p),
-                                                     static_cast<const uint8_t *>(ctx->tilecls.p), nt, 1,
+    k_reduce_by_class<<<1, kMaxCls, 0, ctx->stream>>>(static_cast<const double *>(ctx->clssum.p), tilecls, nt, 1,
                                                      static_cast<double *>(ctx->clsw.p));
     LAUNCH_CHECK();
     return ET_OK;
@@ -634,6 +675,40 @@ et_status fetch(et_ctx *ctx, const void *dev, T *host)
     CUDA_TRY(cudaMemcpyAsync(ctx->pinned, dev, sizeof(T), cudaMemcpyDeviceToHost, ctx->stream));
     CUDA_TRY(cudaStreamSynchronize(ctx->stream));
     memcpy(host, ctx->pinned, sizeof(T));
+    return ET_OK;
+}
+
+// ---- unit-range shard: completing partial sums over ranks --------------------------------------------------
+// buf[r * count + k] (r < world) -> dev[k] = sum over r in rank order; T = long long (exact) or double (fixed order).
+template <typename T>
+__global__ void k_sum_slices(const T *__restrict__ buf, int world, int count, T *__restrict__ dev)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= count) return;
+    T s = 0;
+    for (int r = 0; r < world; ++r) s += buf[(long long)r * count + k];
+    dev[k] = s;
+}
+// dev[count] holds this rank's partial sums (8-byte values); on return it holds the sums over all ranks, identical on
+// every rank: the caller's all-gather (et_set_shard) fills a host buffer [world][count], summed on the device in rank order.
+et_status shard_sum(et_ctx *ctx, void *dev, int count, bool is_f64)
+{
+    if (ctx->shard_world <= 1) return ET_OK;
+    const size_t slice = (size_t)count * 8, total = slice * ctx->shard_world;
+    ET_TRY(ensure_pinned(ctx, 4096 + total));
+    char *h = static_cast<char *>(ctx->pinned) + 4096;  // the first 4 KB are the scratch of fetch() and prep
+    memset(h, 0, total);
+    CUDA_TRY(cudaMemcpyAsync(h + slice * ctx->shard_rank, dev, slice, cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    if (ctx->shard_fn(ctx->shard_user, h, (int64_t)slice) != 0) return fail(ctx, ET_ERR_INVALID, "the all-gather callback of et_set_shard failed");
+    ET_TRY(ensure(ctx, ctx->shardbuf, total));
+    CUDA_TRY(cudaMemcpyAsync(ctx->shardbuf.p, h, total, cudaMemcpyHostToDevice, ctx->stream));
+    if (is_f64)
+        k_sum_slices<double><<<(count + 255) / 256, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->shardbuf.p), ctx->shard_world, count, static_cast<double *>(dev));
+    else
+        k_sum_slices<long long><<<(count + 255) / 256, 256, 0, ctx->stream>>>(static_cast<const long long *>(ctx->shardbuf.p), ctx->shard_world, count, static_cast<long long *>(dev));
+    LAUNCH_CHECK();
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // the pinned buffer is reused by the next call
     return ET_OK;
 }
 
@@ -715,13 +790,13 @@ et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
     return ET_OK;
 }
 
-et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, double *T_perm, et_perm_result *out)
+et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, double nA, double nB, double *T_perm, et_perm_result *out)
 {
     ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
     k_perm_stat<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->Q.p), static_cast<const double *>(ctx->RW.p), nwords,
-                                            (int)nperm, npairs, static_cast<double *>(ctx->tperm.p),
-                                            static_cast<DevPerm *>(ctx->result.p));
+                                            (int)nperm, npairs, nA, nB, std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin)),
+                                            static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p));
     LAUNCH_CHECK();
     DevPerm r;
     ET_TRY(fetch(ctx, ctx->result.p, &r));
@@ -736,11 +811,12 @@ et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, 
 // ---- tensor-core permutation sums (K-PERM-TC) -------------------------------------------------------------
 // T for every label column of the TC layout (et_tc.cuh): chunk ch, column c at index ch * 512 + c.
 __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__ Q, const double *__restrict__ R, const double *__restrict__ W,
-                                                     int nperm, long long npairs_obs, long long npairs_second, double qstep,
-                                                     double nA, double nB, double *__restrict__ T_perm, DevPerm *out, DevT *second)
+                                                     int nperm, long long npairs_obs, long long npairs_second, double qstep, double wabs,
+                                                     double nA, double nB, double *__restrict__ T_perm, DevPerm *out, DevT *second, DevNear *nearout)
 {
     __shared__ DevT obs;
     __shared__ unsigned long long s_cnt, s_near;
+    __shared__ int s_nfin, s_nnan;
     const double S = Q[2], Wtot = W[2];  // the all-ones column
     if (threadIdx.x == 0) {
         form_result(Q[0], S - R[0] + Q[0], R[0] - 2.0 * Q[0], W[0], Wtot - W[0], npairs_obs, &obs);
@@ -749,17 +825,17 @@ __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__
         *second = sec;
         s_cnt = 0ull;
         s_near = 0ull;
+        s_nfin = 0;
+        s_nnan = 0;
     }
     __syncthreads();
     const double Tobs = obs.r.T;
-    // guard band (reading R5): 1e-9 of the term scale plus 8 sigma of the quantisation noise of T_p - T_obs; every
-    // pair carries an independent rounding error of variance (7/48) qstep^2 (round to 16 bits: 1/48; the dithered halving
-    // v = (u + k) >> 1 adds +-1/2 for odd u: 1/8), so
-    // var(T) = (7/48) qstep^2 [ pairs_xx / (W(W-1))^2 + pairs_bb / (Wb(Wb-1))^2 + pairs_xb / (W Wb)^2 ].
-    const double Wo = obs.r.W, Wb = obs.r.Wbar;
-    const double var = 0.5 * nA * (nA - 1.0) / ((Wo * (Wo - 1.0)) * (Wo * (Wo - 1.0))) + 0.5 * nB * (nB - 1.0) / ((Wb * (Wb - 1.0)) * (Wb * (Wb - 1.0))) +
-                       nA * nB / ((Wo * Wb) * (Wo * Wb));
-    const double guard = 1e-9 * (fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb)) + 8.0 * 1.4142135623730951 * qstep * sqrt(var * (7.0 / 48.0));
+    // guard band (reading R5, guard_band above): on top of the fp32 error of psi every pair carries the rounding of
+    // w_j psi_ij to the 15-bit grid of step qstep / |w_i|, an independent error of variance kQuantVar qstep^2
+    const double scale = fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb);
+    const double e32 = kPairErrF32 * wabs * wabs;
+    const double guard = guard_band(sqrt(tc::kQuantVar * qstep * qstep + e32 * e32), nA, nB, obs.r.W, obs.r.Wbar, scale);
+    if (threadIdx.x == 0) { nearout->guard = guard; nearout->guard_f32 = guard_band(e32, nA, nB, obs.r.W, obs.r.Wbar, scale); }
     unsigned long long cnt = 0, near = 0;
     for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
         const int k = (p / tc::kPermsPerChunk) * tc::kCols + tc::kSpecial + p % tc::kPermsPerChunk;
@@ -768,9 +844,13 @@ __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__
         DevT t;
         form_result(q, S - r + q, r - 2.0 * q, w, Wtot - w, npairs_obs, &t);
         T_perm[p] = t.r.T;
-        if (t.status != 0) { near += 1; continue; }
+        if (t.status != 0) { near += 1; atomicAdd(&s_nnan, 1); continue; }
         if (t.r.T > Tobs) cnt += 1;
-        if (fabs(t.r.T - Tobs) <= guard) near += 1;
+        if (fabs(t.r.T - Tobs) <= guard) {
+            near += 1;
+            const int k = atomicAdd(&s_nfin, 1);
+            if (k < kMaxNear) nearout->idx[k] = p;
+        }
     }
     atomicAdd(&s_cnt, cnt);
     atomicAdd(&s_near, near);
@@ -782,6 +862,60 @@ __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__
         out->r.nperm = nperm;
         out->r.p_value = (double)s_cnt / (double)nperm;
         out->status = obs.status;
+        nearout->n_finite = s_nfin;
+        nearout->n_nan = s_nnan;
+    }
+}
+
+// Escalation, statistic of one re-evaluated permutation: D = T_p - T_obs in the fp32-pair / fp64-sum arithmetic from the
+// class-pair sums S[c1 * 4 + c2] of the four classes (a_obs, a_perm) = A (1,1), B (1,0), C (0,1), D (0,0) (k_esc_class):
+//   T_obs = c_xx (AA + AB + BB) + c_bb (CC + CD + DD) - c_xb (AC + AD + BC + BD),   X = A + B observed,
+//   T_p   = c_xx (AA + AC + CC) + c_bb (BB + BD + DD) - c_xb (AB + AD + BC + CD),   X = A + C permuted.
+// Unweighted, the sample sizes and hence c_xx = 1/(n(n-1)), c_bb, c_xb are those of both labellings, AA, DD, AD, BC cancel
+// and were not evaluated (skip mask): D = (c_xx + c_xb)(AC - AB) + (c_bb + c_xb)(BD - CD) + (c_xx - c_bb)(CC - BB).
+// Weighted, W_p differs from W_obs: both T from all ten sums and the class weights.
+constexpr unsigned kEscSkipMask = (1u << 0) | (1u << 3) | (1u << 6) | (1u << 15);  // AA, AD, BC, DD
+__global__ void k_esc_stat(const double *__restrict__ S, const double *__restrict__ clsw, int weighted, double nA, double nB, double *out)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    if (!weighted) {
+        const double cxx = 1.0 / (nA * (nA - 1.0)), cbb = 1.0 / (nB * (nB - 1.0)), cxb = 1.0 / (nA * nB);
+        *out = (cxx + cxb) * (S[2] - S[1]) + (cbb + cxb) * (S[7] - S[11]) + (cxx - cbb) * (S[10] - S[5]);
+        return;
+    }
+    DevT o, p;
+    form_result(S[0] + S[1] + S[5], S[10] + S[11] + S[15], S[2] + S[3] + S[6] + S[7], clsw[0] + clsw[1], clsw[2] + clsw[3], 0, &o);
+    form_result(S[0] + S[2] + S[10], S[5] + S[7] + S[15], S[1] + S[3] + S[6] + S[11], clsw[0] + clsw[2], clsw[1] + clsw[3], 0, &p);
+    *out = (o.status == 0 && p.status == 0) ? p.r.T - o.r.T : nan("");
+}
+// Applies the escalated differences: T_perm[p] = T_obs + D_p (the reported T_obs stays that of the tensor-core pass, so
+// that count_gt = #{T_perm > T_obs} holds for what the caller sees), recounts, n_near = undecidable permutations.
+__global__ void __launch_bounds__(256) k_esc_apply(const DevNear *__restrict__ nr, const double *__restrict__ D, int nesc, int nperm,
+                                                  double *__restrict__ T_perm, DevPerm *out)
+{
+    __shared__ unsigned long long s_cnt;
+    __shared__ int s_near;
+    const double Tobs = out->r.observed.T;
+    if (threadIdx.x == 0) { s_cnt = 0ull; s_near = nr->n_nan + (nr->n_finite - nesc); }
+    __syncthreads();
+    if ((int)threadIdx.x < nesc) {
+        const double d = D[threadIdx.x];
+        double t = Tobs + d;
+        if (d > 0.0 && !(t > Tobs)) t = nextafter(Tobs, Tobs + 1.0);
+        if (d < 0.0 && !(t < Tobs)) t = nextafter(Tobs, Tobs - 1.0);
+        T_perm[nr->idx[threadIdx.x]] = t;
+        if (!(fabs(d) > nr->guard_f32)) atomicAdd(&s_near, 1);
+    }
+    __syncthreads();
+    unsigned long long cnt = 0;
+    for (int p = threadIdx.x; p < nperm; p += blockDim.x)
+        if (T_perm[p] > Tobs) cnt += 1;
+    atomicAdd(&s_cnt, cnt);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        out->r.count_gt = (long long)s_cnt;
+        out->r.n_near = s_near;
+        out->r.p_value = (double)s_cnt / (double)nperm;
     }
 }
 
@@ -796,6 +930,76 @@ et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weig
         tc::k_perm_tc<D, false><<<grid, tc::kThreadsTC, tc::smem_tc(D), ctx->stream>>>(P);
     }
     LAUNCH_CHECK();
+    return ET_OK;
+}
+
+// Guard-band escalation (SURVEY 7 hard part 3; PAPER.md:67 defines p as the fraction of permutation T values greater
+// than the observed one): the permutations whose tensor-core T_p lies within the guard band of T_obs are re-evaluated in
+// the fp32-pair / fp64-sum arithmetic of k_pairs_T, one pass each.  The records of the call's layout are regrouped into
+// the four classes (a_obs, a_perm) of that permutation (k_esc_class, stable partition, k_esc_gather -- the psi values are
+// those of et_T bit for bit), k_pairs_T evaluates the class-pair sums that do not cancel in T_p - T_obs (six of ten when
+// unweighted: 5/8 of the pairs), k_esc_stat forms the difference and k_esc_apply recounts.  Needs ctx->sel (the select
+// states of the labels), ctx->rec, ctx->tperm and the DevPerm / DevNear of k_perm_stat_tc.
+et_status run_escalation(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted)
+{
+    DevNear nr;
+    ET_TRY(fetch(ctx, ctx->nearbuf.p, &nr));
+    if (nr.n_finite == 0 || nr.n_finite > kMaxNear || nr.n_finite > ctx->opt_exact_p) return ET_OK;
+    ET_TRY(span_begin(ctx, 6));
+    const int F = rec_floats(dim);
+    const long long N = L.N;
+    const int nblk = (int)((N + kPartBlock - 1) / kPartBlock);
+    ET_TRY(ensure(ctx, ctx->esccls, (size_t)N));
+    ET_TRY(ensure(ctx, ctx->blkcnt, (size_t)nblk * 4 * sizeof(int)));
+    ET_TRY(ensure(ctx, ctx->totals, 16 * sizeof(long long)));
+    ET_TRY(ensure(ctx, ctx->escD, kMaxNear * sizeof(double)));
+    LabelOut lo{};
+    lo.nseg = L.ncls;
+    for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
+    for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
+    for (int k = 0; k < nr.n_finite; ++k) {
+        const int p = nr.idx[k];
+        k_esc_class<<<(unsigned)((N + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
+            N, L.n_a, ctx->opt_perm_offset + p, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+            static_cast<const SelState *>(ctx->sel.p) + p, static_cast<uint8_t *>(ctx->esccls.p));
+        LAUNCH_CHECK();
+        k_part_count<<<nblk, kPartBlock, 0, ctx->stream>>>(N, static_cast<const uint8_t *>(ctx->esccls.p), static_cast<int *>(ctx->blkcnt.p));
+        LAUNCH_CHECK();
+        k_part_scan<<<1, 32, 0, ctx->stream>>>(nblk, static_cast<int *>(ctx->blkcnt.p), static_cast<long long *>(ctx->totals.p));
+        LAUNCH_CHECK();
+        long long cnt[4];
+        ET_TRY(fetch(ctx, ctx->totals.p, &cnt));
+        Layout L4;
+        layout_four(L4, L.n_a, N - L.n_a, cnt);
+        ET_TRY(upload_tile_classes(ctx, L4, &ctx->tilecls2));
+        ET_TRY(ensure(ctx, ctx->src, (size_t)L4.npad * sizeof(int)));
+        ET_TRY(ensure(ctx, ctx->rec2, (size_t)L4.npad * F * sizeof(float)));
+        k_fill_int<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<int *>(ctx->src.p), L4.npad, -1);
+        LAUNCH_CHECK();
+        CUDA_TRY(cudaMemcpyAsync(static_cast<long long *>(ctx->totals.p) + 8, L4.seg_pos, 4 * sizeof(long long), cudaMemcpyHostToDevice, ctx->stream));
+        CUDA_TRY(cudaStreamSynchronize(ctx->stream));  // L4 is a local
+        k_part_scatter<<<nblk, kPartBlock, 0, ctx->stream>>>(N, static_cast<const uint8_t *>(ctx->esccls.p), static_cast<const int *>(ctx->blkcnt.p),
+                                                            static_cast<const long long *>(ctx->totals.p) + 8, static_cast<int *>(ctx->src.p));
+        LAUNCH_CHECK();
+        k_esc_gather<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->rec.p), static_cast<const int *>(ctx->src.p), L4.npad,
+                                                               F / 4, lo, static_cast<float4 *>(ctx->rec2.p));
+        LAUNCH_CHECK();
+        const float *rec2 = static_cast<const float *>(ctx->rec2.p);
+        const uint8_t *tc2 = static_cast<const uint8_t *>(ctx->tilecls2.p);
+        if (weighted) ET_TRY(run_class_weights(ctx, L4, dim, rec2, tc2));
+        else ET_TRY(ensure(ctx, ctx->clsw, kMaxCls * sizeof(double)));
+        ET_TRY(run_pairs_T(ctx, L4, dim, rec2, tc2, weighted ? 0u : kEscSkipMask, false));
+        k_esc_stat<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), static_cast<const double *>(ctx->clsw.p), weighted ? 1 : 0,
+                                              (double)L.n_a, (double)(N - L.n_a), static_cast<double *>(ctx->escD.p) + k);
+        LAUNCH_CHECK();
+    }
+    k_esc_apply<<<1, 256, 0, ctx->stream>>>(static_cast<const DevNear *>(ctx->nearbuf.p), static_cast<const double *>(ctx->escD.p), nr.n_finite, nperm,
+                                            static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p));
+    LAUNCH_CHECK();
+    double ms = 0;
+    ET_TRY(span_end(ctx, 6, &ms));
+    ctx->stats.ms_escalation += ms;
+    ctx->stats.n_escalated += nr.n_finite;
     return ET_OK;
 }
 
@@ -836,7 +1040,9 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     auto first_kb = [](int I) { return (long long)I * tc::kTM2 / tc::kKB; };  // K block that holds the tile's first row
     long long total_kb = 0;
     for (int I = 0; I < nT; ++I) total_kb += NK - first_kb(I);
-    long long Lmax = (total_kb + (long long)nclusters_max * 24 - 1) / ((long long)nclusters_max * 24);
+    // about 24 units per cluster and rank (ranks of a unit-range shard take every world-th unit of the same table)
+    const long long nshare = (long long)nclusters_max * 24 * ctx->shard_world;
+    long long Lmax = (total_kb + nshare - 1) / nshare;
     if (Lmax < 8) Lmax = 8;
     if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
     std::vector<tc::Unit> full, tail;
@@ -848,6 +1054,14 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         }
     std::stable_sort(tail.begin(), tail.end(), [](const tc::Unit &a, const tc::Unit &b) { return a.kb_end - a.kb_begin > b.kb_end - b.kb_begin; });
     full.insert(full.end(), tail.begin(), tail.end());
+    if (ctx->shard_world > 1) {  // this rank's share: every world-th unit, so that all ranks stream the same label chunks
+        std::vector<tc::Unit> mine;
+        for (size_t k = (size_t)ctx->shard_rank; k < full.size(); k += (size_t)ctx->shard_world) mine.push_back(full[k]);
+        full.swap(mine);
+        total_kb = 0;
+        for (const tc::Unit &u : full) total_kb += u.kb_end - u.kb_begin;
+        if (full.empty()) full.push_back(tc::Unit{0, 0, 0, 0});  // an empty unit: the kernel's epilogue still writes zero partials
+    }
     const int nunits = (int)full.size();
     ET_TRY(ensure(ctx, ctx->units, full.size() * sizeof(tc::Unit)));
     CUDA_TRY(cudaMemcpyAsync(ctx->units.p, full.data(), full.size() * sizeof(tc::Unit), cudaMemcpyHostToDevice, ctx->stream));
@@ -865,13 +1079,15 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     ET_TRY(ensure(ctx, ctx->tcpart, part_bytes));
     ET_TRY(ensure(ctx, ctx->tcQ, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->tcraw, 2 * tc::kCols * 8));
     ET_TRY(span_begin(ctx, 2));
-    const float sc2 = (float)(2.0 * sc);
+    const float scf = (float)sc;
     ET_TRY(ensure(ctx, ctx->recP, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
     CUDA_TRY(cudaMemsetAsync(ctx->recP.p, 0, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4), ctx->stream));
     DISPATCH_DIM(dim, (tc::k_pair_records<D><<<(unsigned)((L.npad / 2 + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
-                          static_cast<const float *>(ctx->rec.p), L.npad / 2, sc2, static_cast<float4 *>(ctx->recP.p))));
+                          static_cast<const float *>(ctx->rec.p), L.npad / 2, scf, static_cast<float4 *>(ctx->recP.p))));
     LAUNCH_CHECK();
+    long long cols_algo = 0, cols_exec = 0;
     for (int ch = 0; ch < nchunks; ++ch) {
         tc::TCParams P{};
         P.rec = static_cast<const float *>(ctx->rec.p);
@@ -880,24 +1096,37 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         P.word0 = ch * tc::kWordsPerChunk;
         P.units = static_cast<const tc::Unit *>(ctx->units.p);
         P.nunits = nunits;
-        P.sc2 = sc2;
+        P.sc = scf;
         P.recP = static_cast<const float4 *>(ctx->recP.p);
         P.idesc_hi = tc::umma_idesc_i8(hi_signed);
+        // label columns of this launch: the three special ones and up to 509 permutations; 256 or fewer need one accumulator
+        const int cols_used = tc::kSpecial + std::min(tc::kPermsPerChunk, nperm - ch * tc::kPermsPerChunk);
+        P.nq = cols_used <= 256 ? 1 : 2;
+        cols_algo += ch == 0 ? cols_used : cols_used - tc::kSpecial;  // the special columns are algorithmic work once
+        cols_exec += 256 * P.nq;
         P.partial = ctx->tcpart.p;
         DISPATCH_DIM(dim, ET_TRY(launch_perm_tc<D>(ctx, P, grid, weighted)));
-        // the scale actually applied is the fp32 value of 2 sc
-        const double inv_sc = 2.0 / (double)P.sc2;
+        // the scale actually applied is the fp32 value of sc
+        const double inv_sc = 1.0 / (double)P.sc;
+        if (weighted) tc::k_tc_reduce<true><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
+        else tc::k_tc_reduce<false><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
+        LAUNCH_CHECK();
+        ET_TRY(shard_sum(ctx, ctx->tcraw.p, 2 * tc::kCols, weighted));  // exact int64 (or fp64) column sums over the ranks
         if (weighted)
-            tc::k_tc_reduce<true><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
-                                                            static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
+            tc::k_tc_scale<true><<<2, 256, 0, ctx->stream>>>(ctx->tcraw.p, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
+                                                           static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
         else
-            tc::k_tc_reduce<false><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
-                                                             static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
+            tc::k_tc_scale<false><<<2, 256, 0, ctx->stream>>>(ctx->tcraw.p, inv_sc, static_cast<double *>(ctx->tcQ.p) + ch * tc::kCols,
+                                                            static_cast<double *>(ctx->tcR.p) + ch * tc::kCols);
         LAUNCH_CHECK();
     }
     {
         const long long pairs = L.N * (L.N - 1) / 2;
-        ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * tc::kCols * nchunks));
+        // algorithmic work (et.h): 2 digits x 2 ops per (pair, label column) over the columns the test needs -- the
+        // permutations plus observed / second labelling / ones once; the executed count (padded accumulators, the
+        // special columns repeated in every chunk) is kept beside it
+        ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * cols_algo));
+        ctx->stats.dominant_ops_executed = 2ll * 2 * pairs * cols_exec;
         ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM2 * tc::kKB;
     }
 
@@ -923,14 +1152,21 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
     DevT *dev_second = reinterpret_cast<DevT *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm));
+    ET_TRY(ensure(ctx, ctx->nearbuf, sizeof(DevNear)));
     k_perm_stat_tc<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->tcQ.p), static_cast<const double *>(ctx->tcR.p),
-                                               static_cast<const double *>(ctx->tcW.p), nperm, npairs_obs, npairs_second, qstep,
+                                               static_cast<const double *>(ctx->tcW.p), nperm, npairs_obs, npairs_second, qstep, wabs,
                                                (double)L.n_a, (double)(L.N - L.n_a),
-                                               static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p), dev_second);
+                                               static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p), dev_second,
+                                               static_cast<DevNear *>(ctx->nearbuf.p));
     LAUNCH_CHECK();
     DevPerm r;
     ET_TRY(fetch(ctx, ctx->result.p, &r));
     if (r.status != 0) return fail(ctx, ET_ERR_DEGENERATE, "weighted normalisation degenerate: W = %g, Wbar = %g (need > 1)", r.r.observed.W, r.r.observed.Wbar);
+    ctx->stats.n_near_before = r.r.n_near;
+    if (r.r.n_near > 0 && ctx->opt_exact_p > 0) {
+        ET_TRY(run_escalation(ctx, L, dim, nperm, seed, weighted));
+        ET_TRY(fetch(ctx, ctx->result.p, &r));
+    }
     DevT sec;
     ET_TRY(fetch(ctx, dev_second, &sec));
     CUDA_TRY(cudaMemcpyAsync(T_perm, ctx->tperm.p, (size_t)nperm * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -986,7 +1222,8 @@ void et_destroy(et_ctx *ctx)
                    &ctx->tilecls, &ctx->partials, &ctx->sums, &ctx->rowsum, &ctx->mask, &ctx->sel, &ctx->hist, &ctx->partQ,
                    &ctx->Q, &ctx->partRW, &ctx->RW, &ctx->mm, &ctx->flag, &ctx->counter, &ctx->src, &ctx->posx, &ctx->posb,
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
-                   &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP};
+                   &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
+                   &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
@@ -1007,11 +1244,29 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
         return ET_OK;
     }
     if (opt == ET_OPT_PERM_OFFSET) {
-        if (value < 0 || value > (1ll << 40)) return fail(ctx, ET_ERR_INVALID, "permutation offset out of range");
+        // the Philox counter word of reading R4 is (uint32)(p >> 2): permutation indices stay below 2^34
+        if (value < 0 || value > (1ll << 34) - ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "permutation offset out of range (p0 + nperm must stay below 2^34)");
         ctx->opt_perm_offset = value;
         return ET_OK;
     }
+    if (opt == ET_OPT_EXACT_P) {
+        if (value < 0 || value > kMaxNear) return fail(ctx, ET_ERR_INVALID, "ET_OPT_EXACT_P must be in 0..%d", kMaxNear);
+        ctx->opt_exact_p = value;
+        return ET_OK;
+    }
     return fail(ctx, ET_ERR_INVALID, "unknown option %d", (int)opt);
+}
+
+et_status et_set_shard(et_ctx *ctx, int rank, int world, et_allgather_fn fn, void *user)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (world < 1 || world > 4096 || rank < 0 || rank >= world) return fail(ctx, ET_ERR_INVALID, "bad shard: rank %d of %d", rank, world);
+    if (world > 1 && !fn) return fail(ctx, ET_ERR_INVALID, "a shard over %d ranks needs the all-gather callback", world);
+    ctx->shard_rank = rank;
+    ctx->shard_world = world;
+    ctx->shard_fn = fn;
+    ctx->shard_user = user;
+    return ET_OK;
 }
 
 et_status et_get_stats(const et_ctx *ctx, et_stats *out)
@@ -1259,7 +1514,7 @@ et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int6
         ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
         ET_TRY(run_pairs_rows(ctx, L, dim));
         ET_TRY(run_perm_sums(ctx, L, dim, nwords));
-        ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), T_perm, &r));
+        ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), (double)n, (double)nbar, T_perm, &r));
     }
     ET_TRY(end_call(ctx));
     *out = r;
@@ -1333,13 +1588,17 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
     ET_TRY(ensure(ctx, ctx->src, (size_t)L.npad * sizeof(int)));
     k_fill_int<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<int *>(ctx->src.p), L.npad, -1);
     LAUNCH_CHECK();
-    k_part_count<<<nblk, kPartBlock, 0, ctx->stream>>>(N, n, static_cast<const uint8_t *>(ctx->posx.p), static_cast<const uint8_t *>(ctx->posb.p),
-                                                      static_cast<int *>(ctx->blkcnt.p));
+    ET_TRY(ensure(ctx, ctx->esccls, (size_t)N));
+    k_podd_classes<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, n, static_cast<const uint8_t *>(ctx->posx.p),
+                                                                      static_cast<const uint8_t *>(ctx->posb.p),
+                                                                      static_cast<uint8_t *>(ctx->esccls.p));
+    LAUNCH_CHECK();
+    k_part_count<<<nblk, kPartBlock, 0, ctx->stream>>>(N, static_cast<const uint8_t *>(ctx->esccls.p), static_cast<int *>(ctx->blkcnt.p));
     LAUNCH_CHECK();
     k_part_scan<<<1, 32, 0, ctx->stream>>>(nblk, static_cast<int *>(ctx->blkcnt.p), static_cast<long long *>(ctx->totals.p));
     LAUNCH_CHECK();
     CUDA_TRY(cudaMemcpyAsync(static_cast<long long *>(ctx->totals.p) + 8, L.seg_pos, 4 * sizeof(long long), cudaMemcpyHostToDevice, ctx->stream));
-    k_part_scatter<<<nblk, kPartBlock, 0, ctx->stream>>>(N, n, static_cast<const uint8_t *>(ctx->posx.p), static_cast<const uint8_t *>(ctx->posb.p),
+    k_part_scatter<<<nblk, kPartBlock, 0, ctx->stream>>>(N, static_cast<const uint8_t *>(ctx->esccls.p),
                                                         static_cast<const int *>(ctx->blkcnt.p), static_cast<const long long *>(ctx->totals.p) + 8,
                                                         static_cast<int *>(ctx->src.p));
     LAUNCH_CHECK();
@@ -1382,7 +1641,7 @@ et_status et_podd_test(et_ctx *ctx, const void *x, const double *mom_x, int64_t 
 
     ET_TRY(run_perm_sums(ctx, L, dim, nwords));
     et_perm_result pr;
-    ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(nI + nIV, nII + nIII), T_perm, &pr));
+    ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(nI + nIV, nII + nIII), (double)(nI + nIV), (double)(nII + nIII), T_perm, &pr));
     DevT even;
     ET_TRY(fetch(ctx, dev_even, &even));
     ET_TRY(end_call(ctx));

@@ -160,9 +160,13 @@ __device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int 
 // scalar one (u_i + (-u_j) == u_i - u_j exactly), so psi is bit-identical to psi_pair<D>.  The packed instructions
 // halve the issue slots per pair (2D+1 FP32 lane-ops and one MUFU.EX2 per pair stay): measured 2.3 -> 2.8e12 pairs/s
 // at D = 5 (profiles/r01_pipe_probes.md).
+// skip_mask: bit c1 * 4 + c2 (c1 <= c2) set = tile pairs of that class pair are not evaluated (their slot stays 0);
+// the guard-band escalation needs six of the ten class-pair sums only.  Units unit0 + k * unit_step (k = 0, 1, ...) are
+// this launch's share: (0, 1) on one GPU, (rank, world) when the unit range is sharded over ranks.
 template <int D, int R>
 __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ rec, int nT,
                                                      const uint8_t *__restrict__ tile_cls, long long nunits,
+                                                     unsigned skip_mask, int unit0, int unit_step,
                                                      double *__restrict__ partials)
 {
     constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
@@ -173,9 +177,11 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
     const int tid = threadIdx.x;
     if (tid < kSumSlots) s_sum[tid] = 0.0;
 
-    for (long long unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
+    for (long long unit = unit0 + (long long)unit_step * blockIdx.x; unit < nunits; unit += (long long)unit_step * gridDim.x) {
         int I, J;
         unit_to_pair(unit, nT, I, J);
+        const int slot = tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad];
+        if (skip_mask >> slot & 1u) continue;
         float2 ui[R][D];
         float wi[R];
 #pragma unroll
@@ -252,7 +258,7 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
             double s = 0.0;
 #pragma unroll
             for (int w = 0; w < kThreads / 32; ++w) s += s_warp[w];
-            s_sum[tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad]] += s;
+            s_sum[slot] += s;
         }
     }
     __syncthreads();
@@ -801,20 +807,22 @@ __global__ void k_podd_flags(const double *pB, const double *pC, const double *p
 
 // Stable partition of the pooled source events into the four class segments of the P-odd layout:
 // layout class 0 = I (D, C_T > 0), 1 = IV (Dbar, -Cbar_T <= 0), 2 = II, 3 = III; A = {0, 1}, B = {2, 3}.
-__device__ __forceinline__ int podd_layout_class(long long s, long long n, const uint8_t *posx, const uint8_t *posb)
+__global__ void k_podd_classes(long long N, long long n, const uint8_t *__restrict__ posx, const uint8_t *__restrict__ posb,
+                               uint8_t *__restrict__ cls)
 {
-    if (s < n) return posx[s] ? 0 : 2;
-    return posb[s - n] ? 3 : 1;
+    const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    cls[s] = s < n ? (posx[s] ? 0 : 2) : (posb[s - n] ? 3 : 1);
 }
+// Stable four-way partition of the indices 0 .. N-1 by cls[s] (k_part_count, k_part_scan, k_part_scatter).
 constexpr int kPartBlock = 1024;
-__global__ void __launch_bounds__(kPartBlock) k_part_count(long long N, long long n, const uint8_t *posx, const uint8_t *posb,
-                                                          int *__restrict__ blk_cnt)
+__global__ void __launch_bounds__(kPartBlock) k_part_count(long long N, const uint8_t *__restrict__ cls, int *__restrict__ blk_cnt)
 {
     __shared__ int cnt[4];
     if (threadIdx.x < 4) cnt[threadIdx.x] = 0;
     __syncthreads();
     const long long s = blockIdx.x * (long long)kPartBlock + threadIdx.x;
-    if (s < N) atomicAdd(&cnt[podd_layout_class(s, n, posx, posb)], 1);
+    if (s < N) atomicAdd(&cnt[cls[s]], 1);
     __syncthreads();
     if (threadIdx.x < 4) blk_cnt[blockIdx.x * 4 + threadIdx.x] = cnt[threadIdx.x];
 }
@@ -832,14 +840,14 @@ __global__ void k_part_scan(int nblk, int *__restrict__ blk_cnt, long long *__re
     }
 }
 // src[seg_pos[c] + rank] = s, ranks in increasing s (stable)
-__global__ void __launch_bounds__(kPartBlock) k_part_scatter(long long N, long long n, const uint8_t *posx, const uint8_t *posb,
+__global__ void __launch_bounds__(kPartBlock) k_part_scatter(long long N, const uint8_t *__restrict__ cls,
                                                             const int *__restrict__ blk_off, const long long *__restrict__ seg_pos,
                                                             int *__restrict__ src)
 {
     __shared__ int warp_cnt[kPartBlock / 32][4];
     const long long s = blockIdx.x * (long long)kPartBlock + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int c = s < N ? podd_layout_class(s, n, posx, posb) : -1;
+    const int c = s < N ? (int)cls[s] : -1;
     unsigned int bal[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) bal[k] = __ballot_sync(0xffffffffu, c == k);
@@ -927,6 +935,40 @@ __global__ void k_gather_rec(const float4 *__restrict__ rec0, const int *__restr
         rec[k] = src >= 0 ? rec0[(long long)src * F4 + q] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
+// ---- guard-band escalation (exact p-value) ------------------------------------------------
+// Class of pooled (label) index i for the re-evaluation of permutation p: 2 (1 - a_obs) + (1 - a_perm), i.e.
+// 0 = in X of both labellings, 1 = X observed / Xbar permuted, 2 = Xbar observed / X permuted, 3 = Xbar of both.
+// a_perm by the rule of reading R4 from the select state of p (K_ip <= K*_p).
+__global__ void __launch_bounds__(kThreads) k_esc_class(long long N, long long n_x, long long pg, uint32_t seed_lo, uint32_t seed_hi,
+                                                       const SelState *__restrict__ st, uint8_t *__restrict__ cls)
+{
+    const long long i = blockIdx.x * (long long)kThreads + threadIdx.x;
+    if (i >= N) return;
+    uint64_t K[4];
+    label_keys4((uint32_t)i, (uint32_t)(pg >> 2), seed_lo, seed_hi, K);
+    const int a_perm = K[pg & 3] <= st->prefix, a_obs = i < n_x;
+    cls[i] = (uint8_t)(2 * (1 - a_obs) + (1 - a_perm));
+}
+// rec2[row] = rec[pos(src[row])]: src[row] is the pooled (label) index that the escalation layout puts into `row`
+// (-1: padding, zero record), pos() its row in the records of the call's own layout (class segments of L).
+__global__ void k_esc_gather(const float4 *__restrict__ rec, const int *__restrict__ src, long long npad2, int F4, LabelOut L,
+                             float4 *__restrict__ rec2)
+{
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < npad2 * F4; k += (long long)gridDim.x * blockDim.x) {
+        const long long row = k / F4;
+        const int q = (int)(k % F4);
+        const long long i = src[row];
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i >= 0) {
+            long long pos = i;
+            for (int s = 0; s < L.nseg; ++s)
+                if (i >= L.seg_first[s] && i < L.seg_first[s + 1]) pos = L.seg_pos[s] + (i - L.seg_first[s]);
+            v = rec[pos * F4 + q];
+        }
+        rec2[k] = v;
+    }
+}
+
 // count = #{T_p > T_obs}, near = #{|T_p - T_obs| <= guard or T_p not finite}; one block
 __global__ void __launch_bounds__(256) k_count_gt(const double *__restrict__ T, int nperm, double Tobs, double guard, long long *__restrict__ out)
 {

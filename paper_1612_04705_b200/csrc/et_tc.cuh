@@ -28,54 +28,42 @@
 
 #include "et_kernels.cuh"
 
-#ifndef ET_TC_DBG
-#define ET_TC_DBG 0  // timing experiments only (_work probes): 1 no tile generation, 2 no MMAs, 3 no label tile, 4 no psi tile, 5 half of the psi tile
-#endif
-
 namespace et {
 namespace tc {
 
 constexpr int kTM = 128;                 // rows (i) per CTA = UMMA M / 2
 constexpr int kTM2 = 2 * kTM;            // rows per cluster (work unit)
-#ifndef ET_TC_KB
-#define ET_TC_KB 96
-#endif
-constexpr int kKB = ET_TC_KB;            // j per K block: 64 (16 producer warps x 2 rows) or 96 (12 warps x 4 rows, needs ET_TC_A32)
+constexpr int kKB = 96;                  // j per K block: three UMMA K steps of 32
 constexpr int kCols = 512;               // label columns per launch (2 accumulators of N = 256)
 constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
-#ifndef ET_TC_A32
-#define ET_TC_A32 1  // A digit tiles as K chunks of 32 bytes, each a SWIZZLE_32B [128 rows x 32 B] sub-tile; 0: one SWIZZLE_64B tile (K blocks of 64 j only)
-#endif
-#ifndef ET_TC_PW
-#define ET_TC_PW (ET_TC_KB == 96 ? 12 : 16)
-#endif
-constexpr int kProducerWarps = ET_TC_PW;          // four per scheduler: the tile generation is latency-bound with two (profiles/r01b)
-constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // a thread evaluates 8 j x this many rows (2)
+constexpr int kProducerWarps = 12;       // three per scheduler; a thread evaluates 4 rows x 8 j of the psi tile
+constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // 4
 constexpr int kEpiWarps = kProducerWarps / 4;                         // warps per TMEM lane quarter
 constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;          // most 32-column groups a warp reads in the epilogue
 __host__ __device__ constexpr int epi_first(int e) { return 16 * e / kEpiWarps; }  // groups [epi_first(e), epi_first(e + 1)) of warp row e
 constexpr int kProducers = kProducerWarps * 32;
 constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
-constexpr int kStages = kKB == 96 ? 3 : 4;
-constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (16 KB)
+constexpr int kStages = 3;
+constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (24 KB)
 constexpr int kBPlane = kKB * 128;           // one plane of this CTA's half of B: kKB j x 128 columns
 constexpr int kBBytes = 2 * 2 * kBPlane;     // [q 2][digit 2][plane]
 constexpr int kStageBytes = kABytes + kBBytes;
-// ring of j pair-record blocks (kKB / 2 pairs each), filled by bulk copies; slots <= 2 kStages (see the loader)
-__host__ __device__ constexpr int rec_slots(int dim) { return kKB == 96 ? ((dim + 2) / 2 <= 3 ? 4 : 2) : 8; }
+// ring of j pair-record blocks (kKB / 2 pairs each), filled by bulk copies (see the loader)
+__host__ __device__ constexpr int rec_slots(int dim) { return (dim + 2) / 2 <= 3 ? 4 : 2; }
 __host__ __device__ constexpr int rec_slot_bytes(int dim) { return (kKB / 2) * ((dim + 2) / 2) * 16; }
 __host__ __device__ constexpr int smem_tc(int dim) { return kStages * kStageBytes + rec_slots(dim) * rec_slot_bytes(dim) + 1024 /*alignment slack*/; }
-constexpr int kMaxRecSlots = 8;
-// 1.5 * 2^23: fma.rn(psi, 2 sc w_j, kMagic + k) holds u = round(2 sc Psi) + k in its low 16 mantissa bits (two's
-// complement when Psi < 0) and v = u >> 1.  The dither k in {0, 1} alternates over the pairs of a tile, so that the mean
-// of v over k is round(2 sc Psi) / 2 exactly: the rounding is unbiased at 16-bit resolution and leaves no +-1/4 LSB
-// tie bias in the block sums.
+constexpr int kMaxRecSlots = 4;
+// 1.5 * 2^23: fma.rn(psi, sc w_j, kMagic) holds v = round-to-nearest-even(sc Psi) in its low 16 mantissa bits (two's
+// complement when Psi < 0), 0 <= v <= 32767 (or |v| <= 16383 with signed weights).  The two operand digits are the BYTES
+// of v: lo = v & 255 (u8, label plane a) and hi = 2 (v >> 8) (u8 <= 254, or s8; label plane 128 a), 128 hi + lo = v.
+// Rounding to nearest is unbiased and its error has variance 1/12 of a step (kQuantVar).
 constexpr float kMagic = 12582912.0f;
-// K blocks per unit: |Y| <= 32767 * 64 * 1000 = 2 097 088 000 < 2^31.  Longer units mean fewer epilogues and pipeline drains:
-// 512 -> 1000 measured -1.2 % (config 2) and -0.9 % (config 4) per step, identical integer sums.
-constexpr int kMaxUnitKB = kKB == 96 ? 660 : 1000;   // 32767 * 96 * 660 = 2 076 117 120 < 2^31
+constexpr double kQuantVar = 1.0 / 12.0;
+// K blocks per unit: |Y| <= 32767 * 96 * 660 = 2 076 117 120 < 2^31.  Longer units mean fewer epilogues and pipeline
+// drains (512 -> 1000 blocks of 64 j measured -1.2 % at config 2 and -0.9 % at config 4, identical integer sums).
+constexpr int kMaxUnitKB = 660;
 
 // label bit held by byte / TMEM column p of a 32-column word
 __host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
@@ -85,7 +73,7 @@ __host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
 
 struct Unit {
     int I;         // 256-row tile
-    int kb_begin;  // first K block (64 j each), >= 4 I
+    int kb_begin;  // first K block (96 j each), >= the block that holds the tile's first row
     int kb_end;
     int pad;
 };
@@ -300,10 +288,10 @@ __device__ __forceinline__ T lane_transpose_sum(T (&x)[32], int lane)
 }
 
 // Pair records of the j side: recP[pair][entry] float2, entry k < D = (-u_{2 pair, k}, -u_{2 pair + 1, k}), entry D =
-// (s, s') with s = 2 sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
+// (s, s') with s = sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
 // i rows duplicated in registers, d = u_i + (-u_j) and Psi = 2^(-e) s + magic are packed FADD2 / FFMA2 over two j.
 template <int D>
-__global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restrict__ rec, long long npairs, float sc2, float4 *__restrict__ recP)
+__global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restrict__ rec, long long npairs, float sc, float4 *__restrict__ recP)
 {
     constexpr int F = rec_floats(D), NLD = pair_rec_f4(D);
     const long long pr = blockIdx.x * (long long)kThreads + threadIdx.x;
@@ -319,8 +307,8 @@ __global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restri
     for (int k = 0; k < 4 * NLD; ++k) o[k] = 0.f;
 #pragma unroll
     for (int k = 0; k < D; ++k) { o[2 * k] = -a[k]; o[2 * k + 1] = -b[k]; }
-    o[2 * D] = __fmul_rn(a[D], sc2);
-    o[2 * D + 1] = __fmul_rn(b[D], sc2);
+    o[2 * D] = __fmul_rn(a[D], sc);
+    o[2 * D + 1] = __fmul_rn(b[D], sc);
 #pragma unroll
     for (int q = 0; q < NLD; ++q) recP[pr * NLD + q] = make_float4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
 }
@@ -333,9 +321,10 @@ struct TCParams {
     int word0;
     const Unit *units;
     int nunits;
-    float sc2;               // 2 * sc: Psi_ij = w_j psi_ij is quantised to v ~ sc Psi (15 bits); applied in recP
+    float sc;                // Psi_ij = w_j psi_ij is quantised to v = round(sc Psi) (15 bits); applied in recP
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
-    void *partial;           // [gridDim.x][16 warps][4 groups][32 lanes][2] of Acc
+    int nq;                  // 256-column accumulators in use: 2, or 1 when this launch has <= 256 label columns
+    void *partial;           // [gridDim.x][kProducerWarps][kEpiGroups][32 lanes][2] of Acc
 };
 
 // One launch = 512 label columns.  Grid: persistent, one CTA per SM, clusters of 2 (an SM pair); unit u is processed
@@ -353,8 +342,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // one array, so that the hot loop addresses every barrier as bar0 + constant + 8 * index
     constexpr int kRecSlots = rec_slots(D);
-    __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + kMaxRecSlots];
+    __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + 2 * kMaxRecSlots];
     uint64_t *const bar_full = bars_s, *const bar_empty = bars_s + kStages, *const bar_rec = bars_s + 2 * kStages + 2;
+    uint64_t *const bar_recfree = bar_rec + kMaxRecSlots;  // record slot consumed by all producer warps of this CTA
     uint64_t &bar_accfull = bars_s[2 * kStages], &bar_accempty = bars_s[2 * kStages + 1];
     constexpr uint32_t kRecSlotBytes = (kKB / 2) * NLD * 16;
     uint8_t *recs = smem + kStages * kStageBytes;  // record ring
@@ -370,7 +360,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], 2 * kProducerWarps); mbar_init(&bar_empty[s], 1); }
         mbar_init(&bar_accfull, 1);
         mbar_init(&bar_accempty, 2 * kProducerWarps);
-        for (int s = 0; s < kRecSlots; ++s) mbar_init(&bar_rec[s], 1);
+        for (int s = 0; s < kRecSlots; ++s) { mbar_init(&bar_rec[s], 1); mbar_init(&bar_recfree[s], kProducerWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == kProducerWarps) {
@@ -399,17 +389,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                     const uint32_t a_base = smem_u32(smem + s * kStageBytes);
                     const uint32_t b_base = a_base + kABytes;
 #pragma unroll
-                    for (int q = 0; q < 2; ++q)
+                    for (int q = 0; q < 2; ++q) {
+                        if (q >= P.nq) break;
 #pragma unroll
                         for (int d = 0; d < 2; ++d)
 #pragma unroll
                             for (int ks = 0; ks < kKB / 32; ++ks) {
-                                const uint64_t da = ET_TC_A32 ? umma_desc(a_base + d * (kTM * kKB) + ks * (kTM * 32), 16, 256, 6)
-                                                               : umma_desc(a_base + d * (kTM * kKB) + ks * 32, 16, 512, 4);
+                                // A digit tile: K chunks of 32 bytes, each a [128 rows x 32 B] SWIZZLE_32B sub-tile
+                                const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * (kTM * 32), 16, 256, 6);
                                 const uint64_t db = umma_desc(b_base + (q * 2 + d) * kBPlane + ks * 4 * 1024, kBPlane, 1024, 2);
                                 const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
-                                if (ET_TC_DBG != 2) umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
+                                umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
                             }
+                    }
                     umma_commit_pair(&bar_empty[s]);  // frees the stage in both CTAs when these MMAs have read it
                 }
                 umma_commit_pair(&bar_accfull);
@@ -417,23 +409,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         }
     } else if (warp == kProducerWarps + 1) {
         // =========================================================================== record loader (each CTA, one lane)
-        // The pair records of K block `it` go to ring slot it % 8 by one bulk copy, up to 8 blocks ahead of the MMAs:
-        // the slot was last read for block it - 8, whose stage has been released (bar_empty) once its MMAs were done.
+        // The pair records of K block `it` go to ring slot it % kRecSlots by one bulk copy, up to kRecSlots blocks ahead
+        // of the producers.  The slot was last read for block it - kRecSlots; every producer warp arrives on the slot's
+        // own "consumed" barrier after its last load of it, so the awaited phase (use number it / kRecSlots - 1) can
+        // only be followed by the phase that this loader itself enables: no parity aliasing.
         if (lane == 0) {
             uint32_t it = 0;
             for (int u = cluster_id; u < P.nunits; u += nclusters) {
                 const Unit U = P.units[u];
                 for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                    // kRecSlots <= 2 kStages: the awaited phase of bar_empty can be at most one phase old, never aliased
-                    if (it >= kRecSlots) mbar_wait(&bar_empty[(it - kRecSlots) % kStages], ((it - kRecSlots) / kStages) & 1);
                     const uint32_t slot = it & (kRecSlots - 1);
+                    if (it >= kRecSlots) mbar_wait(&bar_recfree[slot], ((it / kRecSlots) - 1) & 1);
                     bulk_g2s(smem_u32(recs + slot * kRecSlotBytes), P.recP + (long long)kb * (kKB / 2) * NLD, kRecSlotBytes, &bar_rec[slot]);
                 }
             }
         }
     } else {
         // =========================================================================== producers + epilogue
-        // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < R.  A half-warp holds
+        // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < R = 4.  A half-warp holds
         // 8 rows x 2 octets, so its 8-byte A-tile stores fall into 16 different bank pairs (no conflicts).
         constexpr int R = kRowsPerThread, G = kEpiGroups;
         const int og = (lane >> 3) & 1, l8 = lane & 7;
@@ -447,21 +440,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         for (int g = 0; g < G; ++g) { accQ[g] = 0; accR[g] = 0; }
         // Thread constants of the main loop.  They are made opaque to the compiler (keep()), which otherwise
         // rematerialises them from the lane index in every K block to save registers (~45 instructions, profiles/r01c).
-        // dither constant: k alternates with the row and with the parity of j
-        float2 magicA = make_float2(kMagic + (float)(l8 & 1), kMagic + (float)((l8 & 1) ^ 1));
-        magicA.x = keep(magicA.x);
-        magicA.y = keep(magicA.y);
-        constexpr int NQ = kKB * 8 / kProducers;         // label words (column halves) per thread: 1 (64 j, 16 warps) or 2
-        const int jw = NQ == 1 ? warp & 7 : warp, qw = NQ == 1 ? warp >> 3 : 0;  // label task: 8 j of the K block, column half q (first of NQ)
-        const int jj = 8 * jw + (lane >> 2);            // j (local) of this thread's label word
+        const float magic1 = keep(kMagic);
+        const float2 magicA = make_float2(magic1, magic1);
+        static_assert(kKB * 8 == 2 * kProducers, "a producer thread expands two label words (one per column half q) per K block");
+        const int jw = warp;                            // label task: 8 j of the K block, both column halves
+        const int jj = 8 * jw + (lane >> 2);            // j (local) of this thread's label words
         const int l3 = lane & 3;
-        // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct; SWIZZLE_64B; row
-        // mrow0 + 16 r is 1024 r further) and B tile (j = jj, hi plane of column half qw, 16-byte chunk 2 l3 of the
-        // 128-column row; SWIZZLE_128B; chunk 2 l3 + 1 is at address ^ 16, the lo plane 8192 further)
-        // ET_TC_A32: the digit tile as K chunks of 32 bytes, each a [128 rows x 32 B] SWIZZLE_32B sub-tile (4 KB)
-        const int offA = ET_TC_A32 ? (oct >> 2) * (kTM * 32) + (mrow0 >> 3) * 256 + (mrow0 & 7) * 32 + (((((oct & 3) >> 1) ^ ((mrow0 >> 2) & 1))) << 4) + ((oct & 1) << 3)
-                                   : (mrow0 >> 3) * 512 + (mrow0 & 7) * 64 + (((oct >> 1) ^ ((mrow0 >> 1) & 3)) << 4) + ((oct & 1) << 3);
-        const int offB = kABytes + qw * (2 * kBPlane) + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
+        // byte offsets inside a stage of this thread's stores: A tile (row mrow0, octet oct: K chunk oct >> 2, a
+        // [128 rows x 32 B] SWIZZLE_32B sub-tile of 4 KB; row mrow0 + 16 r is 512 r further) and B tile (j = jj, hi plane
+        // of column half 0, 16-byte chunk 2 l3 of the 128-column row; SWIZZLE_128B; chunk 2 l3 + 1 is at address ^ 16,
+        // the lo plane kBPlane further, column half 1 another 2 kBPlane)
+        const int offA = (oct >> 2) * (kTM * 32) + (mrow0 >> 3) * 256 + (mrow0 & 7) * 32 + (((((oct & 3) >> 1) ^ ((mrow0 >> 2) & 1))) << 4) + ((oct & 1) << 3);
+        const int offB = kABytes + jw * 1024 + (lane >> 2) * 128 + (((2 * l3) ^ (lane >> 2)) << 4);
         const int offJ = kStages * kStageBytes + 4 * oct * NLD * 16;  // its four j pairs inside a record slot
         // running shared-memory addresses of the current stage / record slot (advanced and wrapped every K block)
         const uint32_t bar0 = smem_u32(bars_s);
@@ -489,21 +479,23 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
             // (r, t) of this thread's tile is dropped when kb * 64 + t <= dthr + 16 r
             const int kb_diag = (row0 + kTM + kKB - 1) / kKB;
             const int dthr = row0 + mrow0 - 8 * oct;
-            // this thread's label word of K block kb (element index < 2^32), prefetched one block ahead into a register
-            uint32_t im = (uint32_t)(U.kb_begin * kKB + jj) * (uint32_t)P.words_total + (uint32_t)(P.word0 + 8 * qw + 4 * (int)rank + l3);
-            uint32_t mw = __ldg(P.maskT + im), mw2 = NQ == 2 ? __ldg(P.maskT + im + 8) : 0u;
+            // this thread's label words of K block kb, prefetched one block ahead into registers.  The element index is
+            // 64 bits wide: npadK * words_total passes 2^32 at 2 M pooled rows with the maximum permutation count.
+            const bool q2 = P.nq > 1;
+            unsigned long long im = (unsigned long long)(U.kb_begin * kKB + jj) * (unsigned)P.words_total + (unsigned)(P.word0 + 4 * (int)rank + l3);
+            uint32_t mw = __ldg(P.maskT + im), mw2 = q2 ? __ldg(P.maskT + im + 8) : 0u;
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
                 const uint32_t mcur = mw, mcur2 = mw2;
                 if (kb + 1 < U.kb_end) {
-                    im += (uint32_t)(kKB * P.words_total);
+                    im += (unsigned)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
-                    if (NQ == 2) mw2 = __ldg(P.maskT + im + 8);
+                    if (q2) mw2 = __ldg(P.maskT + im + 8);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
                 mbar_wait_a(bar0 + 8 * kStages + 8 * st, pe ^ 1);
 
                 // ---- psi tile: rows mrow0 + 16 r, j = 8 oct .. 8 oct + 7; label tile: j = jj, this CTA's word
-                //      8 qw + 4 rank + l3 -> 32 columns, byte p of a word is label bit beta(p): register t of the lo plane is
+                //      8 q + 4 rank + l3 -> 32 columns, byte p of a word is label bit beta(p): register t of the lo plane is
                 //      (m >> t) & 0x01010101 (bytes a), of the hi plane (m << (7 - t)) & 0x80808080 (bytes 128 a).
                 //      The four 16-byte label stores are issued between the four j pairs of the psi tile, so that the ALU-pipe
                 //      work of the expansion overlaps the FMA-pipe work of the distances (profiles/r01e).
@@ -511,7 +503,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 auto tile = [&](auto diag_tag) {
                     constexpr bool DIAG = decltype(diag_tag)::value;
                     const int x = kb * kKB - dthr;  // DIAG: element (r, t) is dropped when x <= 16 r - t
-                    uint32_t pk[R][4];              // (f_2tp, f_2tp+1) low halves: bytes lo', hi of two j
+                    uint32_t pk[R][4];              // (f_2tp, f_2tp+1) low halves: bytes (lo, lo, v >> 8, v >> 8) of two j
 #pragma unroll
                     for (int tp = 0; tp < 4; ++tp) {
                         float2 nu[2 * NLD];
@@ -521,13 +513,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             nu[2 * qq] = make_float2(v.x, v.y);
                             nu[2 * qq + 1] = make_float2(v.z, v.w);
                         }
-                        if (ET_TC_DBG != 1 && ET_TC_DBG != 3) {
+                        {
                             uint32_t q[4];
                             if (tp < 2) {
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur >> (4 * tp + t)) & 0x01010101u;
                                 sts128((tp == 0 ? pbB : pbB1) + kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
-                                if (NQ == 2) {
+                                if (q2) {
 #pragma unroll
                                     for (int t = 0; t < 4; ++t) q[t] = (mcur2 >> (4 * tp + t)) & 0x01010101u;
                                     sts128((tp == 0 ? pbB : pbB1) + 3 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
@@ -536,17 +528,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
                                 sts128(tp == 2 ? pbB : pbB1, make_uint4(q[0], q[1], q[2], q[3]));
-                                if (NQ == 2) {
+                                if (q2) {
 #pragma unroll
                                     for (int t = 0; t < 4; ++t) q[t] = (mcur2 << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
                                     sts128((tp == 2 ? pbB : pbB1) + 2 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
                                 }
                             }
                         }
-                        if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
+                        {
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
-                                if (ET_TC_DBG == 5 && r > 0) { pk[r][tp] = pk[0][tp]; continue; }  // experiment: half the psi work
                                 float2 dd = __fadd2_rn(ui2[r][0], nu[0]);
                                 float2 e = __fmul2_rn(dd, dd);
 #pragma unroll
@@ -564,17 +555,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             }
                         }
                     }
-                    if (ET_TC_DBG != 1 && ET_TC_DBG != 4) {
+                    {
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             uint2 lo, hi;
-                            lo.x = (__byte_perm(pk[r][0], pk[r][1], 0x5410) >> 1) & 0x7f7f7f7fu;
-                            lo.y = (__byte_perm(pk[r][2], pk[r][3], 0x5410) >> 1) & 0x7f7f7f7fu;
+                            lo.x = __byte_perm(pk[r][0], pk[r][1], 0x5410);
+                            lo.y = __byte_perm(pk[r][2], pk[r][3], 0x5410);
                             hi.x = __byte_perm(pk[r][0], pk[r][1], 0x7632);
                             hi.y = __byte_perm(pk[r][2], pk[r][3], 0x7632);
-                            // row m = mrow0 + 16 r: 8-row group m >> 3 advances by 2 (1024 bytes), the swizzle phase is that of mrow0
-                            sts64(paA + (ET_TC_A32 ? 512 : 1024) * r, hi);
-                            sts64(paA + kTM * kKB + (ET_TC_A32 ? 512 : 1024) * r, lo);
+                            // hi digit = 2 (v >> 8) per byte: unweighted, every byte is <= 127 and the word add has no
+                            // carries between bytes; signed bytes take the masked form
+                            hi.x += hi.x;
+                            hi.y += hi.y;
+                            if (WEIGHTED) { hi.x &= 0xfefefefeu; hi.y &= 0xfefefefeu; }
+                            // row m = mrow0 + 16 r: 8-row group m >> 3 advances by 2 (512 bytes), the swizzle phase is that of mrow0
+                            sts64(paA + 512 * r, hi);
+                            sts64(paA + kTM * kKB + 512 * r, lo);
                         }
                     }
                 };
@@ -582,7 +578,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 else tile(std::false_type{});
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * st, 0));
+                if (lane == 0) {
+                    mbar_arrive_cluster(mapa_rank(bar0 + 8 * st, 0));
+                    mbar_arrive(&bar_recfree[it & (kRecSlots - 1)]);  // this warp has read the block's records
+                }
                 const bool wrapS = st == kStages - 1, wrapJ = ((it + 1) & (kRecSlots - 1)) == 0;
                 st = wrapS ? 0 : st + 1;
                 pe ^= wrapS ? 1u : 0u;
@@ -606,6 +605,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 else { wi = 1; zi = (Acc)yones; }
 #pragma unroll 1
                 for (int g = 0; g < ngrp; ++g) {
+                    if (grp0 + g >= 8 * P.nq) break;  // one accumulator in use: columns 256.. were never written
                     const uint32_t mword = __ldg(mp + grp0 + g);
                     uint32_t v[32];
                     tmem_ld32(taddr + 32 * (grp0 + g), v);
@@ -640,10 +640,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 }
 
 // Column sums over CTAs and warps, fixed order: TMEM column 32 gc + lane (gc = c >> 5) is held by the four warps
-// 4 (gc / G) .. + 3 as their group gc % G, and is label column c = 32 gc + beta(lane).  out[c] = {Q, R} as doubles in
-// units of psi (divided by sc).
+// 4 (gc / G) .. + 3 as their group gc % G, and is label column c = 32 gc + beta(lane).  raw[col] = Q, raw[512 + col] = R
+// as exact integers (or doubles when weighted) in units of the quantisation step: what a unit-range shard exchanges.
 template <bool WEIGHTED>
-__global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double *__restrict__ outQ, double *__restrict__ outR)
+__global__ void k_tc_reduce(const void *partial, int ncta, void *raw)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -662,8 +662,18 @@ __global__ void k_tc_reduce(const void *partial, int ncta, double inv_sc, double
             sr += e[1];
         }
     const int col = (c & ~31) + beta(lane);
-    outQ[col] = (double)sq * inv_sc;
-    outR[col] = (double)sr * inv_sc;
+    reinterpret_cast<Acc *>(raw)[col] = sq;
+    reinterpret_cast<Acc *>(raw)[kCols + col] = sr;
+}
+// out[c] = {Q, R} as doubles in units of psi (divided by sc)
+template <bool WEIGHTED>
+__global__ void k_tc_scale(const void *raw, double inv_sc, double *__restrict__ outQ, double *__restrict__ outR)
+{
+    using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= kCols) return;
+    outQ[c] = (double)reinterpret_cast<const Acc *>(raw)[c] * inv_sc;
+    outR[c] = (double)reinterpret_cast<const Acc *>(raw)[kCols + c] * inv_sc;
 }
 
 // Label words of the TC layout: maskT[pos][chunk * 16 + W], column c = 32 W + b of chunk ch:

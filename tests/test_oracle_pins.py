@@ -443,3 +443,67 @@ def test_eq3_permutations_keep_sizes_and_equalise_the_purity():
     assert np.isfinite(t_perm).all() and len(np.unique(t_perm)) == 60
     assert abs(t_perm.mean()) < 4 * t_perm.std() / np.sqrt(60)
     assert 0 <= p <= 1 and count == int((t_perm > t_obs).sum())
+
+
+def test_R18_purity_of_permuted_samples_by_enumeration():
+    """Pin of reading R18's b': tag b + bbar of the n + nbar pooled main events as background,
+    enumerate ALL C(n + nbar, n) reassignments to samples of sizes (n, nbar) and average the number of tagged events
+    that land in X' and in Xbar'.  n != nbar, so that b' = b, swapped sizes or a plain half all fail."""
+    import itertools
+
+    n, nbar, b, bbar = 5, 3, 2, 1
+    N = n + nbar
+    tagged = np.zeros(N, dtype=bool)
+    tagged[[0, 3, 6]] = True  # b + bbar = 3 background events somewhere in the pool
+    in_x = []
+    for sel in itertools.combinations(range(N), n):
+        in_x.append(tagged[list(sel)].sum())
+    mean_x = float(np.mean(in_x))
+    bp, bbp = oracle.bkg_perm_purity(b, bbar, n, nbar)
+    assert bp == pytest.approx(mean_x, abs=1e-14) and bbp == pytest.approx((b + bbar) - mean_x, abs=1e-14)
+    assert bp == pytest.approx(15 / 8) and bbp == pytest.approx(9 / 8)
+    # the plausible mistakes are different numbers here
+    for wrong in ((b, bbar), (bbp, bp), ((b + bbar) / 2, (b + bbar) / 2)):
+        assert abs(wrong[0] - mean_x) > 0.1
+
+
+def _eq3_perm_mean(x, xb, bx, bb, b, bbar, sigma, nperm, seed, purity):
+    """Mean and standard error of the Eq. 3 permutation T values with the permuted samples' background counts given
+    by `purity(b, bbar, n, nbar)`; the reassignment is R18's (labels_range from `seed` and `seed ^ BKG_SEED_XOR`)."""
+    n, nbar, bs, bsb = len(x), len(xb), len(bx), len(bb)
+    main, side = np.vstack([x, xb]), np.vstack([bx, bb])
+    am = oracle.labels_range(n + nbar, n, 0, nperm, seed)
+    ab = oracle.labels_range(bs + bsb, bs, 0, nperm, seed ^ oracle.BKG_SEED_XOR)
+    bp, bbp = purity(b, bbar, n, nbar)
+    t = np.array([oracle.T_bkg(main[am[p] == 1], main[am[p] == 0], side[ab[p] == 1], side[ab[p] == 0], bp, bbp, sigma)
+                  for p in range(nperm)])
+    return t, t.mean(), t.std(ddof=1) / np.sqrt(nperm)
+
+
+def test_R18_wrong_purity_biases_the_permutation_T():
+    """Second pin of R18's b': background whose density differs from the signal's (a cluster on a flat signal), unequal
+    sample sizes (305 : 135) and a background that sits mostly in the smaller sample (5 : 35).  Eq. 3 removes the
+    background on average only when the permuted samples are evaluated with the background counts they have on average,
+    (b + bbar) n / (n + nbar) and (b + bbar) nbar / (n + nbar): then the permutation T values scatter around zero, and
+    `bkg_perm_test` reproduces them.  With b' = b, bbar' = bbar (the observed counts) or with the sizes swapped the mean
+    permutation T is tens of standard errors away from zero.  (R18 uses the EXPECTED counts; the hypergeometric
+    fluctuation of the actual counts around them leaves a second-order term ~ var / w^2 in the mean, which this setup
+    -- a broad cluster, 9 % background -- keeps below the permutation spread: measured +1.5 standard errors.)"""
+    rng = np.random.default_rng(1805)
+    nsig_x, nsig_b, b, bbar, bs, bsb = 300, 100, 5, 35, 60, 60
+    sig = rng.uniform(size=(nsig_x + nsig_b, 2))
+    cl = lambda m: 0.5 + 0.15 * rng.normal(size=(m, 2))  # the background: a cluster
+    x = np.vstack([sig[:nsig_x], cl(b)])
+    xb = np.vstack([sig[nsig_x:], cl(bbar)])
+    bx, bb = cl(bs), cl(bsb)
+    nperm, seed, sigma = 300, 99, 0.2
+    t, m, se = _eq3_perm_mean(x, xb, bx, bb, b, bbar, sigma, nperm, seed, oracle.bkg_perm_purity)
+    assert abs(m) < 4 * se, (m, se)
+    _, m_obs, se_obs = _eq3_perm_mean(x, xb, bx, bb, b, bbar, sigma, nperm, seed, lambda b, bbar, n, nbar: (b, bbar))
+    assert abs(m_obs) > 8 * se_obs, (m_obs, se_obs)
+    _, m_sw, se_sw = _eq3_perm_mean(x, xb, bx, bb, b, bbar, sigma, nperm, seed,
+                                    lambda b, bbar, n, nbar: ((b + bbar) * nbar / (n + nbar), (b + bbar) * n / (n + nbar)))
+    assert abs(m_sw) > 8 * se_sw, (m_sw, se_sw)
+    # bkg_perm_test is this loop with R18's purity
+    t_obs, t_perm, count, p = oracle.bkg_perm_test(x, xb, bx, bb, b, bbar, sigma, 40, seed)
+    assert np.allclose(t_perm, t[:40], rtol=0, atol=1e-13) and count == int((t_perm > t_obs).sum())  # OpenMP sum order
