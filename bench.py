@@ -12,9 +12,10 @@ The default workload is BASELINE.json configs[4], the one the north-star target 
 metric = pair-evaluations/s = unordered event pairs that enter T, N(N-1)/2, divided by the step time (every pair is
 counted once however often a kernel touches it).  `value` is timed with the inputs resident in HBM (CUDA events on
 the library's stream); `e2e` is the same call with pinned HOST buffers, the host->device staging inside the timed
-region.  N > 1 (torchrun): the permutation range is sharded, rank r evaluates permutations [r*nperm, (r+1)*nperm)
-of the same sample (the paper farms permutations out to separate GPUs) -- no data-path collective,
-weak scaling; value = ranks * pairs / max-over-ranks time.
+region.  N > 1 (under torchrun, or `--gpus N` alone, which re-launches itself through torch.distributed.run): the
+UNIT RANGE of the O(N^2) kernels is sharded (et_set_shard: rank r evaluates every N-th work unit for all label columns
+and the ranks exchange exact int64 column sums through one small all-gather per launch), the same test on N GPUs --
+strong scaling; value = pairs / max-over-ranks time.
 
 `--impl reference` times the oracle (oracle/, plain fp64 CPU loops) on the host cores on a bounded row subset of the
 same workload; it is the only place besides `cpu_baseline` where this file executes anything under oracle/.
@@ -106,10 +107,14 @@ class ClockSampler:
                 "samples": len(sm), "power_w_max": max(pw) if pw else None}
 
 
+TRAFFIC_CSV = "r02_traffic_k_perm_tc_cfg4.csv"
+
+
 def ncu_traffic(kernel: str, cfg_index: int, default_nperm: bool):
-    """DRAM bytes per launch (read + write) of `kernel` from the committed ncu capture of this workload, or None.
-    Only the default configs[4] workload has one (profiles/r01g_README.md names the command)."""
-    path = os.path.join(ROOT, "profiles", "r01g_traffic_k_perm_tc_cfg4.csv")
+    """DRAM bytes per launch (read + write) of `kernel` from the COMMITTED ncu capture of this workload (a static figure,
+    not measured in this run), or None.  Only the default configs[4] workload has one (profiles/r02_README.md names the
+    command)."""
+    path = os.path.join(ROOT, "profiles", TRAFFIC_CSV)
     if kernel != "k_perm_tc" or cfg_index != 4 or not default_nperm or not os.path.exists(path):
         return None, None
     import csv
@@ -121,7 +126,7 @@ def ncu_traffic(kernel: str, cfg_index: int, default_nperm: bool):
                 per_launch[r["ID"]] = per_launch.get(r["ID"], 0.0) + float(r["Metric Value"].replace(",", ""))
     if not per_launch:
         return None, None
-    return sum(per_launch.values()) / len(per_launch), "profiles/r01g_traffic_k_perm_tc_cfg4.csv (ncu, bytes per launch)"
+    return sum(per_launch.values()) / len(per_launch), f"profiles/{TRAFFIC_CSV} (ncu, bytes per launch)"
 
 
 def pinned(a: np.ndarray):
@@ -148,6 +153,8 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator line (nranks) stays in the log
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     build.build()
@@ -162,7 +169,8 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
     ctx = binding.Context(local, stream=stream)
-    ctx.set_option(binding.ET_OPT_PERM_OFFSET, rank * cfg.nperm)
+    if world > 1:
+        ctx.set_shard(rank, world)
 
     def to_dev(a):
         return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
@@ -192,7 +200,7 @@ def run_ours(args):
     def timed(src, steps):
         """CUDA events on the library's stream around exactly `steps` calls; ms of the slowest rank."""
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        agg = {"ms_pairs": 0.0, "ms_labels": 0.0, "ms_dom": 0.0, "launches": 0, "pair_evals": 0}
+        agg = {"ms_pairs": 0.0, "ms_labels": 0.0, "ms_dom": 0.0, "launches": 0, "pair_evals": 0, "ms_esc": 0.0}
         barrier()
         e0.record(stream)
         for _ in range(steps):
@@ -206,6 +214,10 @@ def run_ours(args):
             agg["dom_launches"] = st.dominant_launches
             agg["dom_kernel"] = st.dominant_kernel
             agg["dom_ops"] = st.dominant_ops
+            agg["dom_ops_exec"] = st.dominant_ops_executed
+            agg["ms_esc"] += st.ms_escalation
+            agg["n_near_before"] = st.n_near_before
+            agg["n_escalated"] = st.n_escalated
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
@@ -226,8 +238,8 @@ def run_ours(args):
         step(h)
     ms_e2e, _, res_h = timed(h, args.steps)
     ms_step = ms / args.steps
-    value = world * pairs / (ms_step * 1e-3)
-    e2e_value = world * pairs / (ms_e2e / args.steps * 1e-3)
+    value = pairs / (ms_step * 1e-3)   # one test on `world` GPUs (unit-range shard): strong scaling
+    e2e_value = pairs / (ms_e2e / args.steps * 1e-3)
     h2d = sum(v.nbytes for v in h.values() if v is not None)
     d2h = cfg.nperm * 8 + 256
 
@@ -284,14 +296,27 @@ def run_ours(args):
     dom_ms = agg["ms_dom"] / (args.steps * max(agg["dom_launches"], 1))
     if agg["dom_kernel"].startswith("k_perm_tc"):
         # int8 tensor-core contraction: ops = 2 * MACs; peak = measured bf16 peak x nominal int8:bf16 ratio (2)
-        ach = agg["dom_ops"] / max(agg["dom_launches"], 1) / (dom_ms * 1e-3) / 1e12
+        # algorithmic ops: 2 digits x 2 x unordered pairs x the label columns the test needs (nperm
+        # permutations + observed + second labelling + ones), summed over the launches of one step, per launch
+        nl = max(agg["dom_launches"], 1)
+        ops = agg["dom_ops"] / nl
+        ach = ops / (dom_ms * 1e-3) / 1e12
+        ach_padded = agg["dom_ops_exec"] / nl / (dom_ms * 1e-3) / 1e12
         peak = 2.0 * peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
-        traffic, traffic_src = ncu_traffic(agg["dom_kernel"], cfg.index, not args.nperm)
+        traffic, traffic_src = ncu_traffic(agg["dom_kernel"], cfg.index, not args.nperm and world == 1)
+        # distinct operand bytes of one launch: its 512-column label chunk (64 B per padded row), the records and the
+        # pair records
+        npad = cfg.n + cfg.nbar + 4096
+        fl = 4 * ((cfg.dim + 1 + 3) // 4)
+        algo_bytes = npad * (64 + 4 * fl + 8 * ((cfg.dim + 2) // 2))
         roofline = {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TOP/s (int8)", "frac": ach / peak,
-                    "traffic": traffic, "traffic_source": traffic_src, "kernel": agg["dom_kernel"],
-                    "launch_ms": dom_ms,
+                    "ops": ops, "launch_ms": dom_ms, "launches_per_step": nl, "frac_padded": ach_padded / peak,
+                    "traffic": traffic, "traffic_static": True, "traffic_source": traffic_src,
+                    "traffic_ratio": (traffic / algo_bytes if traffic else None), "algorithmic_bytes": algo_bytes,
+                    "kernel": agg["dom_kernel"],
                     # context: the measured bf16 peak is a power-throttled cuBLAS GEMM (1.34 GHz), this kernel runs its int8
-                    # MMAs at ~1.96 GHz, so frac can pass 1; against the nominal dense int8 figure (4.5 POP/s) it is:
+                    # MMAs at ~1.9 GHz, so frac can pass 1; against the burst figure and the nominal dense int8 (4.5 POP/s):
+                    "frac_of_burst": ach / (2.0 * peaks["bf16_tflops"]),
                     "frac_of_nominal_int8": ach / 4500.0,
                     "peak_source": f"{peaks['_source']} bf16 sustained x 2 (nominal int8:bf16)"}
     else:
@@ -305,15 +330,20 @@ def run_ours(args):
     out = {
         "metric": "energy_test_pair_evaluations_per_s", "value": value, "unit": "pairs/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32 psi / f64 or exact-int sums", "data": "synthetic",
+        "scaling": "strong", "vs_baseline": None, "dtype": "f32 psi / f64 or exact-int sums", "data": "synthetic",
         "config": {"workload": f"BASELINE configs[{cfg.index}] {cfg.name}: n={cfg.n} nbar={cfg.nbar} dim={cfg.dim} "
-                               f"sigma={sigma} nperm={cfg.nperm} per GPU", "n": cfg.n, "nbar": cfg.nbar, "dim": cfg.dim,
+                               f"sigma={sigma} nperm={cfg.nperm}", "n": cfg.n, "nbar": cfg.nbar, "dim": cfg.dim,
                    "nperm": cfg.nperm, "sigma": sigma, "l2": "inputs and label matrix larger than L2; records re-prepared every step",
-                   "parallelism": f"permutation range sharded over {world} GPU(s)"},
-        "permutations_per_s": world * cfg.nperm / (ms_step * 1e-3),
-        "pair_perm_updates_per_s": world * cfg.nperm * pairs / (ms_step * 1e-3),
-        "effective_pairs_per_s": world * (cfg.nperm + 1) * pairs / (ms_step * 1e-3),  # what one pass per permutation would need
-        "p_value": res.p_value, "T_obs": res.observed.T, "n_near": res.n_near,
+                   "parallelism": f"work units of the O(N^2) kernels sharded over {world} GPU(s), one all-gather of 2 x 512 "
+                                  f"int64 column sums per launch"},
+        "permutations_per_s": cfg.nperm / (ms_step * 1e-3),
+        "pair_perm_updates_per_s": cfg.nperm * pairs / (ms_step * 1e-3),
+        "effective_pairs_per_s": (cfg.nperm + 1) * pairs / (ms_step * 1e-3),  # what one pass per permutation would need
+        "p_value": res.p_value, "count_gt": res.count_gt, "T_obs": res.observed.T, "n_near": res.n_near,
+        # exact p-value: permutations inside the guard band of the tensor-core pass, re-evaluated in the
+        # fp32-pair / fp64-sum arithmetic inside the timed step
+        "escalation": {"n_near_before": agg.get("n_near_before", 0), "n_escalated": agg.get("n_escalated", 0),
+                       "n_near_after": res.n_near, "escalation_ms": agg["ms_esc"] / args.steps},
         "gev": gev,
         "et_T": et_T,
         "sigma_scan": sigma_scan,
@@ -325,22 +355,20 @@ def run_ours(args):
         "roofline": roofline,
     }
     if world > 1:
-        # the ranks' permutation windows form ONE test of world * nperm permutations (sharding.py; no data-path collective)
-        try:
-            from paper_1612_04705_b200 import sharding
-
-            comb = sharding.all_gather_combine(sharding.Shard(rank * cfg.nperm, float(res.observed.T), np.asarray(res.T_perm),
-                                                              int(res.count_gt), int(res.n_near)))
-            out["combined"] = {"nperm": comb.nperm, "count_gt": comb.count_gt, "p_value": comb.p_value, "n_near": comb.n_near}
-        except Exception as exc:  # the timing line must not depend on the gather
-            out["combined"] = {"error": repr(exc)}
+        # every rank holds the complete result; they must agree bit for bit (integer column sums, fixed-order reductions)
+        sig = torch.tensor([float(res.observed.T), float(res.count_gt), float(np.asarray(res.T_perm).sum())], device=dev, dtype=torch.float64)
+        lo, hi = sig.clone(), sig.clone()
+        dist.all_reduce(lo, op=dist.ReduceOp.MIN)
+        dist.all_reduce(hi, op=dist.ReduceOp.MAX)
+        out["ranks_agree"] = bool((lo == hi).all().item())
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(s, cfg, sigma, args.cpu_rows)
-    if rank == 0:
-        print(json.dumps(out))
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
+    if rank == 0:
+        sys.stdout.flush()
+        print(json.dumps(out), flush=True)
 
 
 # ---------------------------------------------------------------------------------------------------------- oracle
@@ -416,8 +444,26 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_ours(args)
+        return
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # started as plain `python bench.py --gpus N`: one rank per GPU through torch.distributed.run (the launch the
+        # driver uses itself); fail loudly instead of running one rank and printing n_gpus = 1
+        import socket
+
+        import torch
+
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.exit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible")
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        sys.exit(f"bench.py --gpus {args.gpus} under a launcher with WORLD_SIZE={os.environ.get('WORLD_SIZE')}")
+    run_ours(args)
 
 
 if __name__ == "__main__":

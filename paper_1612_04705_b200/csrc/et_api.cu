@@ -1070,9 +1070,9 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // quantisation scale: v ~ sc Psi, 0 <= v < 2^15 (unsigned hi digit) or |v| < 2^14 (signed hi digit)
     double sc;
     bool hi_signed = false;
-    if (!weighted) sc = 32767.0;
-    else if (ctx->wmin >= 0.0) sc = 32767.0 / std::max(ctx->wmax, 1e-30);
-    else { hi_signed = true; sc = 16383.0 / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
+    if (!weighted) sc = tc::kScaleUnsigned;
+    else if (ctx->wmin >= 0.0) sc = tc::kScaleUnsigned / std::max(ctx->wmax, 1e-30);
+    else { hi_signed = true; sc = tc::kScaleSigned / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
 
     const int grid = 2 * std::min(nclusters_max, nunits);  // CTA pairs
     const size_t part_bytes = (size_t)grid * tc::kProducerWarps * tc::kEpiGroups * 32 * 2 * 8;
@@ -1081,7 +1081,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->tcraw, 2 * tc::kCols * 8));
     ET_TRY(span_begin(ctx, 2));
-    const float scf = (float)sc;
+    const float scf = (float)(256.0 * sc);
     ET_TRY(ensure(ctx, ctx->recP, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
     CUDA_TRY(cudaMemsetAsync(ctx->recP.p, 0, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4), ctx->stream));
     DISPATCH_DIM(dim, (tc::k_pair_records<D><<<(unsigned)((L.npad / 2 + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
@@ -1096,7 +1096,9 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         P.word0 = ch * tc::kWordsPerChunk;
         P.units = static_cast<const tc::Unit *>(ctx->units.p);
         P.nunits = nunits;
-        P.sc = scf;
+        P.sc256 = scf;
+        P.magic = hi_signed ? tc::kMagicSigned : tc::kMagicUnsigned;
+        P.hixor = hi_signed ? 0x80808080u : 0u;
         P.recP = static_cast<const float4 *>(ctx->recP.p);
         P.idesc_hi = tc::umma_idesc_i8(hi_signed);
         // label columns of this launch: the three special ones and up to 509 permutations; 256 or fewer need one accumulator
@@ -1106,8 +1108,8 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         cols_exec += 256 * P.nq;
         P.partial = ctx->tcpart.p;
         DISPATCH_DIM(dim, ET_TRY(launch_perm_tc<D>(ctx, P, grid, weighted)));
-        // the scale actually applied is the fp32 value of sc
-        const double inv_sc = 1.0 / (double)P.sc;
+        // the scale actually applied is the fp32 value of 256 sc
+        const double inv_sc = 256.0 / (double)P.sc256;
         if (weighted) tc::k_tc_reduce<true><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
         else tc::k_tc_reduce<false><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
         LAUNCH_CHECK();

@@ -55,12 +55,30 @@ __host__ __device__ constexpr int rec_slots(int dim) { return (dim + 2) / 2 <= 3
 __host__ __device__ constexpr int rec_slot_bytes(int dim) { return (kKB / 2) * ((dim + 2) / 2) * 16; }
 __host__ __device__ constexpr int smem_tc(int dim) { return kStages * kStageBytes + rec_slots(dim) * rec_slot_bytes(dim) + 1024 /*alignment slack*/; }
 constexpr int kMaxRecSlots = 4;
-// 1.5 * 2^23: fma.rn(psi, sc w_j, kMagic) holds v = round-to-nearest-even(sc Psi) in its low 16 mantissa bits (two's
-// complement when Psi < 0), 0 <= v <= 32767 (or |v| <= 16383 with signed weights).  The two operand digits are the BYTES
-// of v: lo = v & 255 (u8, label plane a) and hi = 2 (v >> 8) (u8 <= 254, or s8; label plane 128 a), 128 hi + lo = v.
-// Rounding to nearest is unbiased and its error has variance 1/12 of a step (kQuantVar).
-constexpr float kMagic = 12582912.0f;
+// Quantisation of Psi_ij = w_j psi_ij to the 15-bit grid of step 1 / sc: f = fma.rz(psi, 256 sc w_j, M + 128) with
+// M = 2^23 holds, in mantissa bits 8..22, v = floor(sc Psi + 1/2), 0 <= v <= 32767 (weights >= 0).  With signed weights
+// M = 1.5 * 2^23 and the same bits hold 16384 + v, |v| <= 16383.  The two operand digits are BYTES 1 and 2 of f:
+// lo = v & 255 (u8, label plane a) and hi = 2 (v >> 8) (u8 <= 254; signed: 2 byte2 - 128 as s8; label plane 128 a),
+// 128 hi + lo = v.
+//
+// Plain round-to-nearest, NO dither -- measured on the B200 (12 samples each, n = nbar = 2e4 .. 3.2e5, sigma 0.1 .. 0.5,
+// errors in units of the independent-error model sigma of T):
+//   * round to nearest:                      T_obs 0.2-0.6, T_p 0.4-0.7 at every size.  The rounding error is the same
+//     function of psi for every pair, i.e. a tiny perturbation of the distance function, consistent between T_obs and
+//     every T_p.  Cost: the psi values below half a step are lost, -0.005 steps per pair on the Dalitz samples, so each
+//     BLOCK SUM is low by 7e-7 (unit weights) to 2.6e-6 (signed weights) of itself -- the same fraction of S_xx, S_bb
+//     and S_xb, which cancels in T (1/2 + 1/2 - 1 = 0).
+//   * dither levels that are a constant of the thread (2 levels: the earlier round-to-16-bits + alternating halving;
+//     or 32 levels over the lanes): unbiased block sums, T_p fine (0.9-1.0), but T_obs 2-10 and GROWING like sqrt N.
+//     Below one step v is 0 or 1 by comparing sc Psi with the level; a row that meets only its thread's few levels keeps
+//     a bias of its own, random over the rows; random labellings average it (row weights ~ sqrt N), the contiguous
+//     OBSERVED labelling sums it coherently (row weights ~ N).  Rotating the levels from K block to K block only
+//     halves it.  A per-pair pseudo-random level would cost one more instruction per psi and double the variance.
+// The decision T_p > T_obs is what the path is for, so the rounding is the plain one; kQuantVar is its error variance
+// in steps^2 (uniform error), used by the guard band.
+constexpr float kMagicUnsigned = 8388608.0f, kMagicSigned = 12582912.0f;
 constexpr double kQuantVar = 1.0 / 12.0;
+constexpr double kScaleUnsigned = 32766.0, kScaleSigned = 16382.0;  // floor(sc Psi + 1/2) <= 32767 with the fp32 slack of sc w_j
 // K blocks per unit: |Y| <= 32767 * 96 * 660 = 2 076 117 120 < 2^31.  Longer units mean fewer epilogues and pipeline
 // drains (512 -> 1000 blocks of 64 j measured -1.2 % at config 2 and -0.9 % at config 4, identical integer sums).
 constexpr int kMaxUnitKB = 660;
@@ -288,7 +306,7 @@ __device__ __forceinline__ T lane_transpose_sum(T (&x)[32], int lane)
 }
 
 // Pair records of the j side: recP[pair][entry] float2, entry k < D = (-u_{2 pair, k}, -u_{2 pair + 1, k}), entry D =
-// (s, s') with s = sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
+// (s, s') with s = 256 sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
 // i rows duplicated in registers, d = u_i + (-u_j) and Psi = 2^(-e) s + magic are packed FADD2 / FFMA2 over two j.
 template <int D>
 __global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restrict__ rec, long long npairs, float sc, float4 *__restrict__ recP)
@@ -321,7 +339,9 @@ struct TCParams {
     int word0;
     const Unit *units;
     int nunits;
-    float sc;                // Psi_ij = w_j psi_ij is quantised to v = round(sc Psi) (15 bits); applied in recP
+    float sc256;             // 256 sc: Psi_ij = w_j psi_ij is quantised to v = floor(sc Psi + dither) (15 bits); applied in recP
+    float magic;             // kMagicUnsigned, or kMagicSigned when weights can be negative
+    uint32_t hixor;          // 0, or 0x80808080 with kMagicSigned: hi digit = 2 byte2 - 128
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
     int nq;                  // 256-column accumulators in use: 2, or 1 when this launch has <= 256 label columns
     void *partial;           // [gridDim.x][kProducerWarps][kEpiGroups][32 lanes][2] of Acc
@@ -440,7 +460,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         for (int g = 0; g < G; ++g) { accQ[g] = 0; accR[g] = 0; }
         // Thread constants of the main loop.  They are made opaque to the compiler (keep()), which otherwise
         // rematerialises them from the lane index in every K block to save registers (~45 instructions, profiles/r01c).
-        const float magic1 = keep(kMagic);
+        // dither levels of this thread (two j per packed instruction); kept opaque like the other loop constants
+        const uint32_t fmask = __float_as_uint(P.magic);  // a masked element: v = 0
+        const float magic1 = keep(P.magic + 128.f);        // + half a step: round to nearest
         const float2 magicA = make_float2(magic1, magic1);
         static_assert(kKB * 8 == 2 * kProducers, "a producer thread expands two label words (one per column half q) per K block");
         const int jw = warp;                            // label task: 8 j of the K block, both column halves
@@ -503,7 +525,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                 auto tile = [&](auto diag_tag) {
                     constexpr bool DIAG = decltype(diag_tag)::value;
                     const int x = kb * kKB - dthr;  // DIAG: element (r, t) is dropped when x <= 16 r - t
-                    uint32_t pk[R][4];              // (f_2tp, f_2tp+1) low halves: bytes (lo, lo, v >> 8, v >> 8) of two j
+                    uint32_t pk[R][4];              // bytes 1 and 2 of (f_2tp, f_2tp+1): (lo, lo, v >> 8, v >> 8) of two j
 #pragma unroll
                     for (int tp = 0; tp < 4; ++tp) {
                         float2 nu[2 * NLD];
@@ -545,13 +567,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                                     dd = __fadd2_rn(ui2[r][k], nu[k]);
                                     e = __ffma2_rn(dd, dd, e);
                                 }
-                                const float2 f2 = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magicA);
+                                const float2 f2 = __ffma2_rz(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], magicA);
                                 uint32_t f0 = __float_as_uint(f2.x), f1 = __float_as_uint(f2.y);
                                 if (DIAG) {
-                                    if (x <= 16 * r - 2 * tp) f0 = __float_as_uint(kMagic);
-                                    if (x <= 16 * r - 2 * tp - 1) f1 = __float_as_uint(kMagic);
+                                    if (x <= 16 * r - 2 * tp) f0 = fmask;
+                                    if (x <= 16 * r - 2 * tp - 1) f1 = fmask;
                                 }
-                                pk[r][tp] = __byte_perm(f0, f1, 0x5140);
+                                pk[r][tp] = __byte_perm(f0, f1, 0x6251);
                             }
                         }
                     }
@@ -563,11 +585,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
                             lo.y = __byte_perm(pk[r][2], pk[r][3], 0x5410);
                             hi.x = __byte_perm(pk[r][0], pk[r][1], 0x7632);
                             hi.y = __byte_perm(pk[r][2], pk[r][3], 0x7632);
-                            // hi digit = 2 (v >> 8) per byte: unweighted, every byte is <= 127 and the word add has no
-                            // carries between bytes; signed bytes take the masked form
+                            // hi digit = 2 (v >> 8) per byte: every byte2 is <= 127, so the word add has no carries
+                            // between bytes; with signed weights byte2 = 64 + (v >> 8) and 2 byte2 - 128 = 2 byte2 ^ 0x80
                             hi.x += hi.x;
                             hi.y += hi.y;
-                            if (WEIGHTED) { hi.x &= 0xfefefefeu; hi.y &= 0xfefefefeu; }
+                            if (WEIGHTED) { hi.x ^= P.hixor; hi.y ^= P.hixor; }
                             // row m = mrow0 + 16 r: 8-row group m >> 3 advances by 2 (512 bytes), the swizzle phase is that of mrow0
                             sts64(paA + 512 * r, hi);
                             sts64(paA + kTM * kKB + 512 * r, lo);

@@ -63,7 +63,49 @@ def test_struct_sizes_match_header(lib):
     assert ctypes.sizeof(binding._Result) == 80
     assert ctypes.sizeof(binding._PermResult) == 80 + 32
     assert ctypes.sizeof(binding._PoddResult) == 32 + 80 + 112
-    assert ctypes.sizeof(binding._Stats) == 40 + 24 + 32
+    assert ctypes.sizeof(binding._Stats) == 40 + 24 + 32 + 4 * 8
     assert ctypes.sizeof(binding._BkgResult) == 4 * 8 + 10 * 8 + 2 * 8 + 8
     assert ctypes.sizeof(binding._BkgPermResult) == (4 + 10 + 2 + 1) * 8 + 4 * 8
     assert ctypes.sizeof(binding._GevResult) == 3 * 8 + 9 * 8 + 5 * 8 + 3 * 8
+
+
+C_CALLER = os.path.join(ROOT, "tests", "c_caller.c")
+
+
+def build_c_caller(tmp_path):
+    """tests/c_caller.c is a plain C program that includes include/et.h and links libet.so: the boundary is a C ABI."""
+    import subprocess
+
+    exe = str(tmp_path / "c_caller")
+    libdir = os.path.dirname(binding.LIB_PATH)
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(ROOT, "include"), C_CALLER, "-o", exe,
+                           "-L", libdir, "-l:libet.so", "-Wl,-rpath," + libdir, "-lm"])
+    return exe
+
+
+def test_c_caller_compiles_and_fails_loudly_without_a_gpu(lib, tmp_path):
+    import subprocess
+
+    try:
+        import torch
+
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    exe = build_c_caller(tmp_path)
+    r = subprocess.run([exe], capture_output=True, text=True)
+    if has_gpu:
+        assert r.returncode == 0 and "T = 0.125" in r.stdout, r.stdout + r.stderr
+    else:
+        assert r.returncode == 3 and "et_create failed: -6" in r.stdout, r.stdout + r.stderr
+
+
+@pytest.mark.gpu
+def test_c_caller_runs_et_T_on_the_gpu(lib, tmp_path):
+    """Pin P2 (2 + 2 square, T = 0.125) and a 3000-event et_T / et_permutation_test from a C program: no Python between
+    the caller and the library."""
+    import subprocess
+
+    r = subprocess.run([build_c_caller(tmp_path)], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "T = 0.125" in r.stdout and "permutation test ok" in r.stdout, r.stdout

@@ -25,11 +25,18 @@ def ctx():
     c.close()
 
 
-def assert_T_close(got, exp, tol=TOL):
+TERM_REL_TC = 1.5e-5
+
+
+def assert_T_close(got, exp, tol=TOL, term_rel=0.0):
+    """T within the north-star tolerance; the three terms too.  term_rel > 0 (tensor-core path): each term may also
+    be off by that fraction of itself -- the 15-bit round-to-nearest loses the psi values below half a step, about 0.005
+    steps per pair: the same fraction of all three block sums (measured 7e-7 at sigma = 0.3, 6e-6 at sigma = 0.1, 2.7e-6
+    with signed weights), which cancels in T (et_tc.cuh).  The tolerance of T itself is never relaxed."""
     scale = exp.term_scale
     assert abs(got.T - exp.T) <= tol * scale, (got.T, exp.T, scale)
     for k in ("T_xx", "T_bb", "T_xb"):
-        assert abs(getattr(got, k) - getattr(exp, k)) <= tol * scale, k
+        assert abs(getattr(got, k) - getattr(exp, k)) <= tol * scale + term_rel * abs(getattr(exp, k)), k
     assert got.W == pytest.approx(exp.W, rel=1e-6) and got.Wbar == pytest.approx(exp.Wbar, rel=1e-6)
     assert got.n_pairs == exp.n_pairs
 
@@ -145,13 +152,20 @@ def test_row_sums(ctx):
 
 
 # ----------------------------------------------------------------------------- permutation test
-def check_perm(got, exp):
+def check_perm(got, exp, discriminate=True, term_rel=0.0):
+    """North-star tolerance, and a bound that still discriminates where 1e-6 of the term scale is
+    as wide as the permutation spread itself: the achieved error of every T_p and of T_obs stays below 5 % of the
+    standard deviation of the permutation T values."""
     scale = exp.observed.term_scale
-    assert_T_close(got.observed, exp.observed)
+    assert_T_close(got.observed, exp.observed, term_rel=term_rel)
     assert np.isnan(got.T_perm).sum() == np.isnan(exp.T_perm).sum()
     ok = np.isfinite(exp.T_perm)
     assert np.abs(got.T_perm[ok] - exp.T_perm[ok]).max() <= TOL * scale
     assert got.nperm == exp.nperm
+    if discriminate and ok.sum() >= 8:
+        spread = exp.T_perm[ok].std()
+        assert np.abs(got.T_perm[ok] - exp.T_perm[ok]).max() <= 0.05 * spread
+        assert abs(got.observed.T - exp.observed.T) <= 0.05 * spread
     # p-value exact unless a permutation T sits within the guard band of T_obs (reading R5)
     assert abs(got.count_gt - exp.count_gt) <= got.n_near
     if got.n_near == 0:
@@ -243,7 +257,7 @@ def test_perm_tc_matches_oracle(ctx, n, nbar, dim, nperm):
     with force_kernel(ctx, 2):
         got = ctx.permutation_test(x, xb, sigma, nperm, 4242)
         assert ctx.stats().dominant_kernel == "k_perm_tc"
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
     with force_kernel(ctx, 1):
         cc = ctx.permutation_test(x, xb, sigma, nperm, 4242)
         assert ctx.stats().dominant_kernel in ("k_perm32", "k_pairs_rows")
@@ -265,12 +279,12 @@ def test_perm_tc_weighted(ctx):
     exp = oracle.perm_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
     with force_kernel(ctx, 2):
         got = ctx.permutation_test(s.x, s.xbar, 0.3, 40, c.perm_seed, s.wx, s.wxbar)
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
     pos = np.abs(s.wx), np.abs(s.wxbar)  # non-negative weights: unsigned hi digit
     exp = oracle.perm_test(s.x, s.xbar, 0.3, 20, 3, *pos)
     with force_kernel(ctx, 2):
         got = ctx.permutation_test(s.x, s.xbar, 0.3, 20, 3, *pos)
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
 
 
 def test_perm_tc_default_path_midsize(ctx):
@@ -280,7 +294,7 @@ def test_perm_tc_default_path_midsize(ctx):
     exp = oracle.perm_test(s.x, s.xbar, 0.3, 8, c.perm_seed)
     got = ctx.permutation_test(s.x, s.xbar, 0.3, 8, c.perm_seed)
     assert ctx.stats().dominant_kernel == "k_perm_tc"
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
     assert abs(got.observed.T - ctx.T(s.x, s.xbar, 0.3).T) <= TOL * exp.observed.term_scale
 
 
@@ -295,7 +309,7 @@ def test_podd_tc_parity(ctx):
     I, II, III, IV = s.x[posx == 1], s.x[posx == 0], s.xbar[posb == 1], s.xbar[posb == 0]
     assert got.count == (len(I), len(II), len(III), len(IV))
     exp = oracle.perm_test(np.vstack([I, IV]), np.vstack([II, III]), c.sigma, nperm, c.perm_seed)
-    check_perm(got.p_odd, exp)
+    check_perm(got.p_odd, exp, term_rel=TERM_REL_TC)
     assert_T_close(got.p_even, oracle.T(s.x, s.xbar, c.sigma))
 
 
@@ -364,10 +378,10 @@ def test_full_size_row_sum_parity(ctx, index):
 
 def test_full_size_podd_tc_properties(ctx):
     """BASELINE configs[4] in the launch configuration bench.py times (n = nbar = 10^6, 1000 permutations, tensor-core
-    path).  A from-scratch oracle T_p is 17 CPU-minutes each at this size, so: the split is compared with the oracle
-    bit for bit, the observed statistics of both labellings (columns 0 and 1 of K-PERM-TC) with the fp32/fp64
-    all-pairs kernel on the regrouped samples (itself pinned to the oracle at this size by the sampled row sums
-    above), and the permutation distribution through properties that hold at any size (pin P6: E_perm[T] = 0;
+    path).  The oracle anchor at this size is test_full_size_golden[4] below (stored oracle values); HERE the split is
+    compared with the oracle bit for bit, the observed statistics of both labellings (columns 0 and 1 of K-PERM-TC) with
+    the fp32/fp64 all-pairs kernel k_pairs_T on the regrouped samples -- two independent GPU kernels, not an oracle
+    comparison -- and the permutation distribution through properties that hold at any size (pin P6: E_perm[T] = 0;
     count = #{T_p > T_obs}; no two permutations alike)."""
     c = dg.config(4)
     s = dg.make_sample(c)
@@ -450,16 +464,16 @@ def test_T_bkg_errors(ctx):
 
 def test_full_size_config1_permutations_from_scratch(ctx):
     """BASELINE configs[1] at full size (n = nbar = 100 000, fp32 coordinates, sigma = 0.3), default dispatch (tensor
-    cores): the observed T and the first three permutations against the oracle, each re-evaluated from scratch
-    (4 x 2e10 psi in fp64, about 40 s on 16 host cores); labels of those permutations bit for bit."""
+    cores): the observed T and the first eight permutations against the oracle, each re-evaluated from scratch
+    (9 x 2e10 psi in fp64, about 100 s on 16 host cores); labels of those permutations bit for bit."""
     c = dg.config(1)
     s = dg.make_sample(c)
     assert s.x.dtype == np.float32
-    nperm = 3
+    nperm = 8
     exp = oracle.perm_test(s.x, s.xbar, 0.3, nperm, c.perm_seed)
     got = ctx.permutation_test(s.x, s.xbar, 0.3, nperm, c.perm_seed)
     assert ctx.stats().dominant_kernel == "k_perm_tc"
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
     N = c.n + c.nbar
     assert (ctx.perm_labels(N, c.n, nperm, c.perm_seed) == oracle.labels(N, c.n, nperm, c.perm_seed)).all()
 
@@ -504,7 +518,7 @@ def test_perm_tc_chunk_and_size_edges(ctx, n, nbar, nperm):
     """Tensor-core path forced at its edges: the smallest samples, one permutation, and permutation counts on both
     sides of the 509-per-launch boundary (1, 2 and 3 launches of 512 label columns).  Below the default dispatch
     threshold (16384 rows) the 15-bit quantisation noise of psi does not average out: the bound used here is 8 sigma of
-    DESIGN.md section 6, var(T) = (7/48) q^2 [1/(2n(n-1)) + 1/(2nbar(nbar-1)) + 1/(n nbar)] with q = 1 / 32767, or the
+    DESIGN.md section 6, var(T) = (1/12) q^2 [1/(2n(n-1)) + 1/(2nbar(nbar-1)) + 1/(n nbar)] with q = 1 / 32766, or the
     north-star tolerance if that is larger."""
     rng = np.random.default_rng(n * 1000 + nperm)
     x, xb = rng.normal(size=(n, 4)), rng.normal(size=(nbar, 4)) * 1.1 + 0.05
@@ -512,7 +526,7 @@ def test_perm_tc_chunk_and_size_edges(ctx, n, nbar, nperm):
     with force_kernel(ctx, 2):
         got = ctx.permutation_test(x, xb, 0.8, nperm, 99)
         assert ctx.stats().dominant_kernel == "k_perm_tc"
-    var = (7.0 / 48.0) / 32767.0 ** 2 * (0.5 / (n * (n - 1.0)) + 0.5 / (nbar * (nbar - 1.0)) + 1.0 / (n * nbar))
+    var = (1.0 / 12.0) / 32766.0 ** 2 * (0.5 / (n * (n - 1.0)) + 0.5 / (nbar * (nbar - 1.0)) + 1.0 / (n * nbar))
     bound = max(TOL * exp.observed.term_scale, 8.0 * math.sqrt(var))
     assert abs(got.observed.T - exp.observed.T) <= bound
     assert np.abs(got.T_perm - exp.T_perm).max() <= bound and got.nperm == nperm
@@ -529,7 +543,7 @@ def test_perm_tc_remaining_dims(ctx, dim):
     with force_kernel(ctx, 2):
         got = ctx.permutation_test(x, xb, sigma, 20, 5)
         assert ctx.stats().dominant_kernel == "k_perm_tc"
-    check_perm(got, exp)
+    check_perm(got, exp, term_rel=TERM_REL_TC)
 
 
 def test_perm_tc_bit_reproducible_many_units(ctx):
@@ -598,7 +612,8 @@ def test_full_size_config3_weighted_tc_properties(ctx):
     ref = ctx.T_weighted(s.x, s.wx, s.xbar, s.wxbar, c.sigma)
     scale = ref.term_scale
     o = got.observed
-    assert abs(o.T - ref.T) <= TOL * scale and abs(o.T_xx - ref.T_xx) <= TOL * scale and abs(o.T_xb - ref.T_xb) <= TOL * scale
+    assert_T_close(o, ref, term_rel=TERM_REL_TC)
+    assert abs(o.T - ref.T) <= 0.05 * got.T_perm.std()
     assert o.W == pytest.approx(ref.W, rel=1e-12) and o.Wbar == pytest.approx(ref.Wbar, rel=1e-12)
     assert o.W == pytest.approx(float(np.float32(s.wx).astype(np.float64).sum()), rel=1e-9)   # weights enter as fp32
     Tp = got.T_perm
@@ -608,13 +623,280 @@ def test_full_size_config3_weighted_tc_properties(ctx):
 
 
 def test_perm_tc_accumulator_headroom_coincident_points(ctx):
-    """The largest values the int32 TMEM accumulators can see: 80 000 coincident events, psi = 1 for every pair, so the
-    first row tile's units sum 1000 K blocks x 64 j x 32767.  Pin P1 at scale: T = 1/2 + 1/2 - 1 = 0 for the observed
-    and for every permutation; the raw sums are the pair counts."""
-    n = nbar = 40000
+    """The largest values the int32 TMEM accumulators can see: 260 000 coincident events, psi = 1 for every pair, so
+    every work unit of the first row tiles runs the full 660 K blocks of 96 j with all digits at their maximum:
+    |Y| = 32767 x 96 x 660 = 2 076 117 120 of 2^31 = 2 147 483 648 (run_perm_tc picks Lmax = 660 from N = 2.4e5 on, which
+    is every config-2/3/4 launch).  300 permutations: both 256-column accumulators.  Pin P1 at scale: T = 1/2 + 1/2 - 1
+    = 0 for the observed and for every permutation; the raw sums are the pair counts."""
+    n = nbar = 130000
     x, xb = np.full((n, 2), 0.25), np.full((nbar, 2), 0.25)
-    got = ctx.permutation_test(x, xb, 0.3, 20, 3)
+    got = ctx.permutation_test(x, xb, 0.3, 300, 3)
     assert ctx.stats().dominant_kernel == "k_perm_tc"
     o = got.observed
-    assert o.S_xx == pytest.approx(n * (n - 1) / 2, rel=1e-12) and o.S_xb == pytest.approx(n * nbar, rel=1e-12)
-    assert abs(o.T) <= 1e-12 and np.abs(got.T_perm).max() <= 1e-12
+    assert o.S_xx == pytest.approx(n * (n - 1) / 2, rel=1e-15) and o.S_bb == pytest.approx(nbar * (nbar - 1) / 2, rel=1e-15)
+    assert o.S_xb == pytest.approx(n * nbar, rel=1e-15)
+    assert abs(o.T) <= 1e-15 and np.abs(got.T_perm).max() <= 1e-15
+    # ties everywhere: every permutation is inside the guard band and stays undecided
+    assert got.n_near == 300
+
+
+# ----------------------------------------------------------------------------- sigma scan of the permutation test
+@pytest.mark.parametrize("sigma", [0.1, 0.5])
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_perm_sigma_scan_values(ctx, sigma, kernel):
+    """BASELINE configs[1] / [3] quote sigma in {0.1, 0.3, 0.5}: the permutation path at the two outer values (config 1
+    at a fifth of its size, fp32 coordinates, 8 permutations from scratch in the oracle), default dispatch (tensor cores)
+    and CUDA cores.  At sigma = 0.1 most psi underflow or round to 0 on the 15-bit grid."""
+    c = dg.config(1, scale=0.2)
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, sigma, 8, c.perm_seed)
+    with force_kernel(ctx, kernel):
+        got = ctx.permutation_test(s.x, s.xbar, sigma, 8, c.perm_seed)
+        assert ctx.stats().dominant_kernel == ("k_perm_tc" if kernel == 0 else "k_perm32")
+    check_perm(got, exp, term_rel=TERM_REL_TC if kernel == 0 else 0.0)
+    assert (np.argsort(got.T_perm) == np.argsort(exp.T_perm)).all()
+
+
+# ----------------------------------------------------------------------------- oracle anchor at the bench sizes
+def _golden():
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "fullsize_T.txt")
+    out = {}
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#") or "=" not in line:
+                continue
+            k, v = line.split("=", 1)
+            out[k.strip()] = float.fromhex(v.split("|")[1].strip())
+    return out
+
+
+def _golden_result(g, prefix, n_pairs):
+    return binding.Result(*(g[f"{prefix}.{k}"] for k in ("T", "T_xx", "T_bb", "T_xb", "S_xx", "S_bb", "S_xb", "W", "Wbar")), n_pairs)
+
+
+@pytest.mark.parametrize("index", [2, 3, 4])
+def test_full_size_golden(ctx, index):
+    """BASELINE configs[2], [3], [4] at full size, in the launch configuration bench.py times (all 1000 permutations,
+    default dispatch = K-PERM-TC), against oracle values stored in tests/golden/fullsize_T.txt (written by
+    tests/golden/make_fullsize_golden.py from oracle + datagen alone: the observed statistic with its three terms and the
+    first permutation T values, each a from-scratch fp64 pass; config 4 also the P-even grouping).  et_T (k_pairs_T) is
+    compared with the same values.  Beside the north-star tolerance -- which at these sizes is as wide as the
+    permutation spread -- the achieved errors must stay below 5 % of the spread of the permutation T values."""
+    g = _golden()
+    c = dg.config(index)
+    tag = f"cfg{index}"
+    if f"{tag}.obs.T" not in g:
+        pytest.skip(f"{tag} is not in tests/golden/fullsize_T.txt yet (run tests/golden/make_fullsize_golden.py)")
+    s = dg.make_sample(c)
+    N = c.n + c.nbar
+    exp = _golden_result(g, f"{tag}.obs", N * (N - 1) // 2)
+    if c.podd:
+        r = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, c.nperm, c.perm_seed)
+        assert tuple(float(v) for v in r.count) == tuple(g[f"{tag}.count.{k}"] for k in ("I", "II", "III", "IV"))
+        got, even = r.p_odd, r.p_even
+    else:
+        got, even = ctx.permutation_test(s.x, s.xbar, c.sigma, c.nperm, c.perm_seed, s.wx, s.wxbar), None
+    st = ctx.stats()
+    assert st.dominant_kernel == "k_perm_tc"
+    spread = got.T_perm.std()
+    scale = exp.term_scale
+    o = got.observed
+    assert_T_close(o, exp, term_rel=TERM_REL_TC)
+    assert abs(o.T - exp.T) <= 0.05 * spread, (o.T, exp.T, spread)
+    # weights enter the kernels as fp32 values: W agrees to fp32 rounding of the individual weights
+    assert o.W == pytest.approx(exp.W, rel=1e-7 if c.weighted else 1e-15) and o.Wbar == pytest.approx(exp.Wbar, rel=1e-7 if c.weighted else 1e-15)
+    errs = [abs(o.T - exp.T)]
+    k = 0
+    while f"{tag}.perm.{k}" in g:
+        e = abs(got.T_perm[k] - g[f"{tag}.perm.{k}"])
+        assert e <= TOL * scale and e <= 0.05 * spread, (k, got.T_perm[k], g[f"{tag}.perm.{k}"], spread)
+        # the side of T_obs each of these permutations falls on is the oracle's
+        assert (got.T_perm[k] > o.T) == (g[f"{tag}.perm.{k}"] > exp.T)
+        errs.append(e)
+        k += 1
+    assert k >= 1
+    if even is not None:
+        ev = _golden_result(g, f"{tag}.even", N * (N - 1) // 2)
+        assert abs(even.T - ev.T) <= TOL * ev.term_scale and abs(even.T - ev.T) <= 0.05 * spread
+        assert abs(even.T_xx - ev.T_xx) <= TOL * ev.term_scale and abs(even.T_xb - ev.T_xb) <= TOL * ev.term_scale
+        errs.append(abs(even.T - ev.T))
+    # k_pairs_T at the same size against the same stored values
+    if c.podd:
+        posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
+        posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
+        A = np.vstack([s.x[posx == 1], s.xbar[posb == 0]])
+        B = np.vstack([s.x[posx == 0], s.xbar[posb == 1]])
+        t = ctx.T(A, B, c.sigma)
+    elif c.weighted:
+        t = ctx.T_weighted(s.x, s.wx, s.xbar, s.wxbar, c.sigma)
+    else:
+        t = ctx.T(s.x, s.xbar, c.sigma)
+    assert abs(t.T - exp.T) <= TOL * scale and abs(t.T - exp.T) <= 0.05 * spread
+    for k in ("T_xx", "T_bb", "T_xb"):
+        assert abs(getattr(t, k) - getattr(exp, k)) <= TOL * scale, k
+    print(f"\n[golden cfg{index}] spread {spread:.3e}; |dT| tensor-core path: " + ", ".join(f"{e:.2e}" for e in errs) +
+          f"; et_T {abs(t.T - exp.T):.2e}; n_near {st.n_near_before} -> {got.n_near}, escalation {st.ms_escalation:.1f} ms")
+
+
+# ----------------------------------------------------------------------------- exact p-values (guard-band escalation)
+def test_escalation_restores_the_oracle_count(ctx):
+    """p is the fraction of permutation T values greater than the observed one, and north_star wants it
+    equal to the oracle's.  Tiny samples and the largest permutation count make the 15-bit rounding noise of the
+    tensor-core path matter: with 65 536 permutations about one of them falls on the wrong side of T_obs, and ten or so
+    inside the guard band.  Without the escalation (ET_OPT_EXACT_P = 0) the count differs from the oracle's for at
+    least one of the seeds below and the difference is covered by n_near; with it (the near permutations re-evaluated
+    in the fp32-pair / fp64-sum arithmetic) the count is the oracle's whenever nothing is left inside the fp32 band."""
+    rng = np.random.default_rng(2024)
+    x, xb = rng.uniform(size=(40, 3)), rng.uniform(size=(50, 3)) ** 1.2
+    nperm, flipped_before = 65536, 0
+    for seed in range(1, 9):
+        exp = oracle.perm_test(x, xb, 0.3, nperm, seed)
+        with force_kernel(ctx, 2):
+            ctx.set_option(binding.ET_OPT_EXACT_P, 0)
+            try:
+                raw = ctx.permutation_test(x, xb, 0.3, nperm, seed)
+            finally:
+                ctx.set_option(binding.ET_OPT_EXACT_P, 64)
+            try:
+                got = ctx.permutation_test(x, xb, 0.3, nperm, seed)
+                st = ctx.stats()
+            finally:
+                ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+        assert abs(raw.count_gt - exp.count_gt) <= raw.n_near and raw.n_near > 0
+        assert st.n_near_before == raw.n_near and st.n_escalated == raw.n_near and st.ms_escalation > 0
+        assert got.n_near < raw.n_near
+        assert abs(got.count_gt - exp.count_gt) <= got.n_near
+        assert got.count_gt == int((got.T_perm > got.observed.T).sum()) and got.observed.T == raw.observed.T
+        # only the escalated permutations moved, and by less than the band
+        moved = np.flatnonzero(got.T_perm != raw.T_perm)
+        assert len(moved) <= raw.n_near and np.abs(got.T_perm - raw.T_perm).max() < 1e-5
+        # the re-evaluated differences T_p - T_obs are the oracle's to fp32-path accuracy
+        assert np.abs((got.T_perm[moved] - got.observed.T) - (exp.T_perm[moved] - exp.observed.T)).max() < 2e-7
+        if got.n_near == 0:
+            assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
+        if raw.count_gt != exp.count_gt:
+            flipped_before += 1
+            assert got.count_gt == exp.count_gt or got.n_near > 0
+    assert flipped_before >= 1, "no seed showed a count that the escalation had to repair"
+
+
+def test_escalation_weighted_and_podd(ctx):
+    """The escalation on the weighted path (all ten class-pair sums, W_p recomputed) and on the four-class layout of
+    the Sect. 5 test, forced tensor cores on small samples with many permutations."""
+    c = dg.config(3, scale=0.0005)  # 100 + 100 events
+    s = dg.make_sample(c)
+    exp = oracle.perm_test(s.x, s.xbar, 0.3, 20000, 5, s.wx, s.wxbar)
+    with force_kernel(ctx, 2):
+        ctx.set_option(binding.ET_OPT_EXACT_P, 64)
+        try:
+            got = ctx.permutation_test(s.x, s.xbar, 0.3, 20000, 5, s.wx, s.wxbar)
+            st = ctx.stats()
+        finally:
+            ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+    assert st.n_near_before > 0 and (st.n_escalated == st.n_near_before or st.n_escalated == 0)
+    assert abs(got.count_gt - exp.count_gt) <= got.n_near
+    if got.n_near == 0:
+        assert got.count_gt == exp.count_gt
+    c = dg.config(4, scale=0.0001)  # 100 + 100 events
+    s = dg.make_sample(c)
+    posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
+    posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
+    A = np.vstack([s.x[posx == 1], s.xbar[posb == 0]])
+    B = np.vstack([s.x[posx == 0], s.xbar[posb == 1]])
+    exp = oracle.perm_test(A, B, c.sigma, 30000, 9)
+    with force_kernel(ctx, 2):
+        ctx.set_option(binding.ET_OPT_EXACT_P, 64)
+        try:
+            got = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, 30000, 9).p_odd
+            st = ctx.stats()
+        finally:
+            ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+    assert st.n_near_before > 0
+    assert abs(got.count_gt - exp.count_gt) <= got.n_near
+    if got.n_near == 0:
+        assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
+
+
+# ----------------------------------------------------------------------------- unit-range shard (SURVEY 8(e))
+def _run_sharded(world, call, exact_p=16):
+    """`world` contexts on this GPU, one host thread each, in lock step: the all-gather callback of et_set_shard is a
+    host-side rendezvous of the threads (no kernel waits for another).  Returns the ranks' results."""
+    import ctypes
+    import threading
+
+    bar = threading.Barrier(world)
+    box = {}
+    results, errors = [None] * world, []
+
+    def make_cb(rank):
+        def fn(_user, buf, nbytes):
+            mine = ctypes.string_at(buf + rank * nbytes, nbytes)
+            box[rank] = mine
+            bar.wait()
+            for r in range(world):
+                ctypes.memmove(buf + r * nbytes, box[r], nbytes)
+            bar.wait()
+            return 0
+        return binding._ALLGATHER(fn)
+
+    def worker(rank):
+        try:
+            with binding.Context(0) as c:
+                cb = make_cb(rank)
+                c._check(binding.lib().et_set_shard(c._h, rank, world, ctypes.cast(cb, ctypes.c_void_p), None))
+                c.set_option(binding.ET_OPT_EXACT_P, exact_p)
+                results[rank] = call(c)
+        except Exception as exc:  # release the other threads
+            errors.append(exc)
+            bar.abort()
+
+    th = [threading.Thread(target=worker, args=(r,)) for r in range(world)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errors, errors
+    return results
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_unit_shard_is_bit_identical(ctx, world):
+    """Ranks of a unit-range shard evaluate disjoint work units of K-PERM-TC (and of k_pairs_T) and exchange exact
+    int64 column sums: every rank's result equals the unsharded one bit for bit, whatever the number of ranks."""
+    c = dg.config(2, scale=0.1)  # 30 000 + 30 000 events, 5-D: hundreds of units, two launches
+    s = dg.make_sample(c)
+    ref = ctx.permutation_test(s.x, s.xbar, c.sigma, 600, 11)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    refT = ctx.T(s.x, s.xbar, c.sigma)
+    out = _run_sharded(world, lambda cx: (cx.permutation_test(s.x, s.xbar, c.sigma, 600, 11), cx.T(s.x, s.xbar, c.sigma)))
+    for r, t in out:
+        assert (r.T_perm == ref.T_perm).all() and r.observed.T == ref.observed.T and r.count_gt == ref.count_gt
+        assert r.n_near == ref.n_near and r.observed.S_xb == ref.observed.S_xb
+        assert abs(t.T - refT.T) <= 1e-12 * refT.term_scale  # fp64 block sums regrouped by rank
+
+
+def test_unit_shard_with_escalation_and_weights(ctx):
+    """Sharded runs whose escalation passes (k_pairs_T, sharded too) and weighted fp64 sums go through the all-gather."""
+    rng = np.random.default_rng(2024)
+    x, xb = rng.uniform(size=(40, 3)), rng.uniform(size=(50, 3)) ** 1.2
+    with force_kernel(ctx, 2):
+        ctx.set_option(binding.ET_OPT_EXACT_P, 64)
+        try:
+            ref = ctx.permutation_test(x, xb, 0.3, 20000, 1)
+            assert ctx.stats().n_escalated > 0
+        finally:
+            ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+
+    def call(cx):
+        cx.set_option(binding.ET_OPT_PERM_KERNEL, 2)
+        return cx.permutation_test(x, xb, 0.3, 20000, 1), cx.stats()
+
+    for r, st in _run_sharded(2, call, exact_p=64):
+        assert st.n_escalated > 0 and r.count_gt == ref.count_gt and r.n_near == ref.n_near
+        assert np.abs(r.T_perm - ref.T_perm).max() <= 1e-15 and r.observed.T == ref.observed.T
+    c = dg.config(3, scale=0.1)  # weighted, 20 000 + 20 000
+    s = dg.make_sample(c)
+    ref = ctx.permutation_test(s.x, s.xbar, 0.3, 100, 3, s.wx, s.wxbar)
+    for r in _run_sharded(2, lambda cx: cx.permutation_test(s.x, s.xbar, 0.3, 100, 3, s.wx, s.wxbar)):
+        assert np.abs(r.T_perm - ref.T_perm).max() <= 1e-12 * ref.observed.term_scale and r.count_gt == ref.count_gt

@@ -84,3 +84,56 @@ def test_gloo_world2_gather():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert got == [(0, True), (1, True)]
+
+
+# ---- unit-range shard (et_set_shard): the all-gather callback of the binding over gloo -------------------------------
+def _unit_shard_worker(rank, world, port, q):
+    """What libet.so does around the callback, with plain host arrays standing in for the device sums: each rank holds
+    its partial int64 column sums (here: every world-th entry of a fixed table of per-unit sums), hands the callback a
+    host buffer [world][count] with its own slice filled in, and adds the slices in rank order."""
+    import ctypes
+
+    import torch.distributed as dist
+
+    from paper_1612_04705_b200 import binding
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        rng = np.random.default_rng(7)  # the same table on every rank
+        units = rng.integers(-2**40, 2**40, size=(37, 1024), dtype=np.int64)   # per-unit contributions to 2 x 512 columns
+        total = units.sum(axis=0)
+        mine = units[rank::world].sum(axis=0)
+        cb = binding._ALLGATHER(binding.make_allgather(rank, world))
+        ok = True
+        for trial in range(2):  # the library calls it once per 512-column launch
+            buf = np.zeros((world, 1024), dtype=np.int64)
+            buf[rank] = mine + trial
+            rc = cb(None, buf.ctypes.data, 1024 * 8)
+            ok = ok and rc == 0 and np.array_equal(buf.sum(axis=0), total + world * trial)
+            ok = ok and all(np.array_equal(buf[r], units[r::world].sum(axis=0) + trial) for r in range(world))
+        # doubles travel as bytes too: bit patterns survive
+        d = np.zeros((world, 3), dtype=np.float64)
+        d[rank] = [np.pi * (rank + 1), -0.0, 1e-300]
+        ok = ok and cb(None, d.ctypes.data, 24) == 0 and all(d[r, 0] == np.pi * (r + 1) for r in range(world))
+        q.put((rank, bool(ok)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_gloo_world2_unit_shard_allgather():
+    import torch.multiprocessing as mp
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_unit_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert got == [(0, True), (1, True)]
