@@ -267,6 +267,30 @@ typedef struct {
 et_status et_gev_pvalue(const double *T_perm, int64_t nperm, double T_obs,
                         const double *z, int64_t nresample, et_gev_result *out);
 
+/* Binned S_CP chi^2 of Sect. 2.1 (Eq. 1): the paper's comparison method.
+ *   S_CP^i = (N^i(X) - alpha N^i(Xbar)) / sqrt(N^i(X) + alpha^2 N^i(Xbar)),  alpha = N_tot(X) / N_tot(Xbar),
+ *   chi^2 = sum_i (S_CP^i)^2, ndf = bins - 1, p = upper tail of chi^2(ndf).
+ * The paper leaves the binning to the analyst; readings R19-R21 of DESIGN.md: a uniform rectangular
+ * grid, axis k has nbins[k] equal bins over [lo[k], hi[k]] (lo, hi, nbins: HOST arrays [dim], lo < hi, nbins >= 1,
+ * product <= 2^24); bin = floor(((x - lo) / (hi - lo)) nbins) in fp64 in this order, x == hi in the last bin, flat
+ * index with axis 0 slowest; events outside the box (or not finite) are left out and counted in n_outside; N_tot are
+ * the yields inside the grid; a bin empty in both samples is not a bin (S = 0, not counted in ndf).
+ * S, Nx, Nxbar: optional HOST outputs [product of nbins] (NULL to skip).  ET_ERR_DEGENERATE when a sample has no
+ * event inside the grid or fewer than two bins have entries.  Here n, nbar >= 1 suffice and sigma plays no role. */
+typedef struct {
+    double chi2;
+    int64_t ndf;           /* bins with entries - 1                                              */
+    double p_value;        /* Q(ndf / 2, chi2 / 2)                                               */
+    double alpha;
+    int64_t n_in_x, n_in_xbar, n_outside;
+    int64_t bins_used, bins_total;
+} et_scp_result;
+
+et_status et_scp(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar,
+                 int dim, et_dtype dtype, et_memspace mem,
+                 const double *lo, const double *hi, const int32_t *nbins,
+                 double *S, int64_t *Nx, int64_t *Nxbar, et_scp_result *out);
+
 /* Test hook: the permutation labels of reading R4, bit-packed,
  * mask[i * ceil(nperm/32) + (p >> 5)] bit (p & 31) = 1 iff pooled event i is in
  * sample X of permutation p.  `mask` lives in `mem`. */

@@ -28,7 +28,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_set_shard", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums", "et_scp"]
 
 
 class EtError(RuntimeError):
@@ -65,6 +65,12 @@ class _GevResult(C.Structure):
     _fields_ = ([(k, C.c_double) for k in ("mu", "sigma", "xi")] + [("cov", C.c_double * 9)] +
                 [(k, C.c_double) for k in ("nll", "p_value", "p_lo", "p_med", "p_hi")] +
                 [(k, C.c_int64) for k in ("n_used", "converged", "n_resampled")])
+
+
+class _ScpResult(C.Structure):
+    _fields_ = [("chi2", C.c_double), ("ndf", C.c_int64), ("p_value", C.c_double), ("alpha", C.c_double),
+                ("n_in_x", C.c_int64), ("n_in_xbar", C.c_int64), ("n_outside", C.c_int64), ("bins_used", C.c_int64),
+                ("bins_total", C.c_int64)]
 
 
 class _Stats(C.Structure):
@@ -167,6 +173,22 @@ def gev_pvalue(T_perm, T_obs: float, z=None) -> GevResult:
 
 
 @dataclass
+class ScpResult:
+    chi2: float
+    ndf: int
+    p_value: float
+    alpha: float
+    n_in_x: int
+    n_in_xbar: int
+    n_outside: int
+    bins_used: int
+    bins_total: int
+    S: np.ndarray
+    Nx: np.ndarray
+    Nxbar: np.ndarray
+
+
+@dataclass
 class Stats:
     ms_total: float
     ms_pairs: float
@@ -218,6 +240,7 @@ def lib():
             "et_podd_test": [vp] + wsample + tail + [i64, u64, vp, vp],
             "et_perm_labels": [vp, i64, i64, i64, u64, ci, vp],
             "et_row_sums": [vp] + wsample + tail + [vp, i64, vp, vp],
+            "et_scp": [vp] + sample + [ci, ci, ci, vp, vp, vp, vp, vp, vp, vp],
         }.items():
             getattr(L, name).argtypes = args
         assert all(getattr(L, n).argtypes is not None for n in SYMBOLS)
@@ -508,3 +531,25 @@ class Context:
                                       rows.ctypes.data_as(C.c_void_p), C.c_int64(len(rows)),
                                       rx.ctypes.data_as(C.c_void_p), rb.ctypes.data_as(C.c_void_p)))
         return rx, rb
+
+    # ---------------------------------------------------------------- Sect. 2.1
+    def scp(self, x, xbar, lo, hi, nbins) -> ScpResult:
+        """Binned S_CP chi^2 (Eq. 1) on a uniform grid: axis k has nbins[k] equal bins over [lo[k], hi[k]]."""
+        ax, ab = _coords(x, xbar)
+        dim = ax.shape[1]
+        alo = np.ascontiguousarray(np.asarray(lo, dtype=np.float64).reshape(-1))
+        ahi = np.ascontiguousarray(np.asarray(hi, dtype=np.float64).reshape(-1))
+        anb = np.ascontiguousarray(np.asarray(nbins, dtype=np.int32).reshape(-1))
+        if not (len(alo) == len(ahi) == len(anb) == dim):
+            raise ValueError(f"lo, hi, nbins must have one entry per axis ({dim})")
+        if (anb < 1).any() or int(np.prod(anb.astype(np.int64))) > 1 << 24:
+            raise ValueError("nbins must be >= 1 per axis and at most 2^24 bins in total")
+        total = int(np.prod(anb.astype(np.int64)))
+        S, Nx, Nb = np.zeros(total), np.zeros(total, dtype=np.int64), np.zeros(total, dtype=np.int64)
+        out = _ScpResult()
+        self._check(lib().et_scp(self._h, ax.ptr, C.c_int64(ax.shape[0]), ab.ptr, C.c_int64(ab.shape[0]), C.c_int(dim),
+                                 C.c_int(ax.dtype), C.c_int(ax.mem), alo.ctypes.data_as(C.c_void_p), ahi.ctypes.data_as(C.c_void_p),
+                                 anb.ctypes.data_as(C.c_void_p), S.ctypes.data_as(C.c_void_p), Nx.ctypes.data_as(C.c_void_p),
+                                 Nb.ctypes.data_as(C.c_void_p), C.byref(out)))
+        return ScpResult(out.chi2, out.ndf, out.p_value, out.alpha, out.n_in_x, out.n_in_xbar, out.n_outside, out.bins_used,
+                         out.bins_total, S, Nx, Nb)

@@ -13,6 +13,7 @@
 #include "../../include/et.h"
 #include "et_kernels.cuh"
 #include "et_tc.cuh"
+#include "et_scp.cuh"
 
 using namespace et;
 
@@ -67,6 +68,7 @@ struct et_ctx {
     Buf rec2, tilecls2, esccls, escD, nearbuf, escw;
     double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
+    Buf scpcnt, scpS;
     bool tc_attr_set = false;
 };
 
@@ -1711,6 +1713,82 @@ et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n, c
     CUDA_TRY(cudaMemcpyAsync(r_x, ctx->rowsout.p, (size_t)nrows * 8, cudaMemcpyDeviceToHost, ctx->stream));
     CUDA_TRY(cudaMemcpyAsync(r_xbar, static_cast<double *>(ctx->rowsout.p) + nrows, (size_t)nrows * 8, cudaMemcpyDeviceToHost, ctx->stream));
     ET_TRY(end_call(ctx));
+    return ET_OK;
+}
+
+et_status et_scp(et_ctx *ctx, const void *x, int64_t n, const void *xbar, int64_t nbar, int dim, et_dtype dtype, et_memspace mem,
+                 const double *lo, const double *hi, const int32_t *nbins, double *S, int64_t *Nx, int64_t *Nxbar, et_scp_result *out)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!x || !xbar || !lo || !hi || !nbins || !out) return fail(ctx, ET_ERR_INVALID, "null pointer");
+    if (n < 1 || nbar < 1) return fail(ctx, ET_ERR_INVALID, "n and nbar must be >= 1");
+    if (dim < 1 || dim > scp::kMaxAxes) return fail(ctx, ET_ERR_INVALID, "dim must be in 1..%d; got %d", scp::kMaxAxes, dim);
+    if (dtype != ET_F32 && dtype != ET_F64) return fail(ctx, ET_ERR_INVALID, "bad dtype");
+    if (mem != ET_HOST && mem != ET_DEVICE) return fail(ctx, ET_ERR_INVALID, "bad memspace");
+    scp::Grid G{};
+    G.dim = dim;
+    long long total = 1;
+    for (int k = 0; k < dim; ++k) {
+        if (!std::isfinite(lo[k]) || !std::isfinite(hi[k]) || !(lo[k] < hi[k])) return fail(ctx, ET_ERR_INVALID, "axis %d: need finite lo < hi", k);
+        if (nbins[k] < 1) return fail(ctx, ET_ERR_INVALID, "axis %d: nbins must be >= 1", k);
+        G.lo[k] = lo[k]; G.hi[k] = hi[k]; G.nbins[k] = nbins[k];
+        total *= nbins[k];
+        if (total > scp::kMaxBins) return fail(ctx, ET_ERR_INVALID, "more than 2^24 bins");
+    }
+    G.total = (int)total;
+    ET_TRY(begin_call(ctx));
+    const void *dx = nullptr, *dxb = nullptr;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    // counts: [Nx total][Nxbar total][outside 1]
+    const size_t cnt_bytes = (2 * (size_t)total + 1) * sizeof(unsigned long long);
+    ET_TRY(ensure(ctx, ctx->scpcnt, cnt_bytes));
+    ET_TRY(ensure(ctx, ctx->scpS, (size_t)total * sizeof(double)));
+    ET_TRY(ensure(ctx, ctx->result, sizeof(scp::DevScp)));
+    CUDA_TRY(cudaMemsetAsync(ctx->scpcnt.p, 0, cnt_bytes, ctx->stream));
+    unsigned long long *cx = static_cast<unsigned long long *>(ctx->scpcnt.p), *cb = cx + total, *coutside = cx + 2 * total;
+    const int grid = ctx->num_sms * 8;
+    const bool sm = total <= scp::kSmemBins;
+    auto hist = [&](const void *p, long long cnt, unsigned long long *dst) {
+        const int g = (int)std::min<long long>(grid, (cnt + 255) / 256);
+        if (dtype == ET_F32) {
+            if (sm) scp::k_scp_hist<float, true><<<g, 256, 0, ctx->stream>>>(static_cast<const float *>(p), cnt, G, dst, coutside);
+            else scp::k_scp_hist<float, false><<<g, 256, 0, ctx->stream>>>(static_cast<const float *>(p), cnt, G, dst, coutside);
+        } else {
+            if (sm) scp::k_scp_hist<double, true><<<g, 256, 0, ctx->stream>>>(static_cast<const double *>(p), cnt, G, dst, coutside);
+            else scp::k_scp_hist<double, false><<<g, 256, 0, ctx->stream>>>(static_cast<const double *>(p), cnt, G, dst, coutside);
+        }
+    };
+    hist(dx, n, cx);
+    LAUNCH_CHECK();
+    hist(dxb, nbar, cb);
+    LAUNCH_CHECK();
+    scp::k_scp_stat<<<1, 1024, 0, ctx->stream>>>(cx, cb, G.total, static_cast<double *>(ctx->scpS.p), static_cast<scp::DevScp *>(ctx->result.p));
+    LAUNCH_CHECK();
+    scp::DevScp r;
+    ET_TRY(fetch(ctx, ctx->result.p, &r));
+    unsigned long long n_out = 0;
+    CUDA_TRY(cudaMemcpyAsync(&n_out, coutside, sizeof(n_out), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    if (r.n_in_x < 1 || r.n_in_xbar < 1 || r.bins_used < 2) {
+        ET_TRY(end_call(ctx));
+        return fail(ctx, ET_ERR_DEGENERATE, "S_CP needs events of both samples inside the grid and two bins with entries (in-grid %lld, %lld; bins %lld)",
+                    r.n_in_x, r.n_in_xbar, r.bins_used);
+    }
+    static_assert(sizeof(unsigned long long) == sizeof(int64_t), "counts are copied out as int64");
+    if (S) CUDA_TRY(cudaMemcpyAsync(S, ctx->scpS.p, (size_t)total * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (Nx) CUDA_TRY(cudaMemcpyAsync(Nx, cx, (size_t)total * sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+    if (Nxbar) CUDA_TRY(cudaMemcpyAsync(Nxbar, cb, (size_t)total * sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+    ET_TRY(end_call(ctx));
+    out->chi2 = r.chi2;
+    out->ndf = r.bins_used - 1;
+    out->p_value = scp::chi2_sf(r.chi2, r.bins_used - 1);
+    out->alpha = r.alpha;
+    out->n_in_x = r.n_in_x;
+    out->n_in_xbar = r.n_in_xbar;
+    out->n_outside = (int64_t)n_out;
+    out->bins_used = r.bins_used;
+    out->bins_total = total;
     return ET_OK;
 }
 

@@ -67,6 +67,7 @@ def test_struct_sizes_match_header(lib):
     assert ctypes.sizeof(binding._BkgResult) == 4 * 8 + 10 * 8 + 2 * 8 + 8
     assert ctypes.sizeof(binding._BkgPermResult) == (4 + 10 + 2 + 1) * 8 + 4 * 8
     assert ctypes.sizeof(binding._GevResult) == 3 * 8 + 9 * 8 + 5 * 8 + 3 * 8
+    assert ctypes.sizeof(binding._ScpResult) == 9 * 8
 
 
 C_CALLER = os.path.join(ROOT, "tests", "c_caller.c")
