@@ -165,7 +165,12 @@ def run_ours(args):
         cfg.nperm = args.nperm
     s = dg.make_sample(cfg)
     sigma = cfg.sigma
-    pairs = n_pairs(cfg.n, cfg.nbar)
+    # BASELINE configs[1] / [3] are a sigma scan (three sigma x the same 1000 permutations): the step is the whole scan,
+    # one et_permutation_test_sigmas call, and every (pair, sigma) counts as a pair evaluation
+    scan = list(getattr(cfg, "sigmas", ()) or ()) if not args.one_sigma else []
+    scan = scan if len(scan) > 1 else []
+    pairs1 = n_pairs(cfg.n, cfg.nbar)
+    pairs = pairs1 * max(len(scan), 1)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
     ctx = binding.Context(local, stream=stream)
@@ -190,6 +195,9 @@ def run_ours(args):
         if cfg.podd:
             r = ctx.podd_test(src["x"], src["mom_x"], src["xbar"], src["mom_xbar"], sigma, cfg.nperm, cfg.perm_seed)
             return r.p_odd
+        if scan:
+            rs = ctx.permutation_test_sigmas(src["x"], src["xbar"], scan, cfg.nperm, cfg.perm_seed, src["wx"], src["wxbar"])
+            return rs[scan.index(sigma)] if sigma in scan else rs[0]
         return ctx.permutation_test(src["x"], src["xbar"], sigma, cfg.nperm, cfg.perm_seed, src["wx"], src["wxbar"])
 
     def barrier():
@@ -241,7 +249,7 @@ def run_ours(args):
     value = pairs / (ms_step * 1e-3)   # one test on `world` GPUs (unit-range shard): strong scaling
     e2e_value = pairs / (ms_e2e / args.steps * 1e-3)
     h2d = sum(v.nbytes for v in h.values() if v is not None)
-    d2h = cfg.nperm * 8 + 256
+    d2h = (cfg.nperm * 8 + 256) * max(len(scan), 1)
 
     # et_T alone (H1-H3, H6): the psi kernel against the FP32/SFU roofline
     def T_only():
@@ -259,9 +267,9 @@ def run_ours(args):
         msT_k += st.ms_pairs
     sm_mhz_max = peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)
     roofT = alu_roofline_pairs_per_s(cfg.dim, sm_mhz_max)
-    et_T = {"pairs_per_s": pairs / (msT / nT * 1e-3), "kernel_pairs_per_s": pairs / (msT_k / nT * 1e-3),
-            "ms": msT / nT, "roofline_pairs_per_s": roofT, "frac": pairs / (msT_k / nT * 1e-3) / roofT,
-            "frac_at_sampled_clock": (pairs / (msT_k / nT * 1e-3) / alu_roofline_pairs_per_s(cfg.dim, clocks["sm_mhz"])
+    et_T = {"pairs_per_s": pairs1 / (msT / nT * 1e-3), "kernel_pairs_per_s": pairs1 / (msT_k / nT * 1e-3),
+            "ms": msT / nT, "roofline_pairs_per_s": roofT, "frac": pairs1 / (msT_k / nT * 1e-3) / roofT,
+            "frac_at_sampled_clock": (pairs1 / (msT_k / nT * 1e-3) / alu_roofline_pairs_per_s(cfg.dim, clocks["sm_mhz"])
                                       if clocks.get("sm_mhz") else None),
             "peak_model": "min(128/(2D+1),16) pairs/clk/SM x 148 SMs x sm_max_mhz (FP32/SFU pipes)"}
 
@@ -283,7 +291,7 @@ def run_ours(args):
             sep = sum(ms_of(lambda v=v: ctx.T_weighted(d["x"], d["wx"], d["xbar"], d["wxbar"], v)) for v in sg)
         else:
             sep = sum(ms_of(lambda v=v: ctx.T(d["x"], d["xbar"], v)) for v in sg)
-        sigma_scan = {"sigmas": sg, "ms_fused": fused, "ms_separate": sep, "pair_sigma_evals_per_s": len(sg) * pairs / (fused * 1e-3)}
+        sigma_scan = {"sigmas": sg, "ms_fused": fused, "ms_separate": sep, "pair_sigma_evals_per_s": len(sg) * pairs1 / (fused * 1e-3)}
 
     # GEV fit of this step's permutation T values: the p-value where counting gives 0 (host-only, ~ms)
     try:
@@ -332,11 +340,11 @@ def run_ours(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "strong", "vs_baseline": None, "dtype": "f32 psi / f64 or exact-int sums", "data": "synthetic",
         "config": {"workload": f"BASELINE configs[{cfg.index}] {cfg.name}: n={cfg.n} nbar={cfg.nbar} dim={cfg.dim} "
-                               f"sigma={sigma} nperm={cfg.nperm}", "n": cfg.n, "nbar": cfg.nbar, "dim": cfg.dim,
-                   "nperm": cfg.nperm, "sigma": sigma, "l2": "inputs and label matrix larger than L2; records re-prepared every step",
+                               f"sigma={scan if scan else sigma} nperm={cfg.nperm}", "n": cfg.n, "nbar": cfg.nbar, "dim": cfg.dim,
+                   "nperm": cfg.nperm, "sigma": scan if scan else sigma, "l2": "inputs and label matrix larger than L2; records re-prepared every step",
                    "parallelism": f"work units of the O(N^2) kernels sharded over {world} GPU(s), one all-gather of 2 x 512 "
                                   f"int64 column sums per launch"},
-        "permutations_per_s": cfg.nperm / (ms_step * 1e-3),
+        "permutations_per_s": cfg.nperm * max(len(scan), 1) / (ms_step * 1e-3),
         "pair_perm_updates_per_s": cfg.nperm * pairs / (ms_step * 1e-3),
         "effective_pairs_per_s": (cfg.nperm + 1) * pairs / (ms_step * 1e-3),  # what one pass per permutation would need
         "p_value": res.p_value, "count_gt": res.count_gt, "T_obs": res.observed.T, "n_near": res.n_near,
@@ -441,6 +449,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-rows", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--one-sigma", action="store_true", help="configs 1 / 3: time the middle sigma alone instead of the scan")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -170,6 +170,18 @@ et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int6
                               int dim, et_dtype dtype, et_memspace mem, double sigma,
                               int64_t nperm, uint64_t seed, double *T_perm, et_perm_result *out);
 
+/* The permutation test at nsig <= ET_MAX_SCAN values of sigma: the sigma scan of Sect. 2.2 (Fig. 2
+ * shows "p-values versus sigma"; BASELINE configs[1] and [3] quote three sigma x 1000 permutations).  Results are those
+ * of nsig et_permutation_test calls with the same (nperm, seed) -- the same permutations serve every sigma -- bit for
+ * bit; the staging copies, the permutation labels (radix select + label matrix) and the layout are made once.
+ * T_perm[nsig][nperm] and out[nsig] are HOST memory. */
+#define ET_MAX_SCAN 16
+et_status et_permutation_test_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n,
+                                     const void *xbar, const double *wxbar, int64_t nbar,
+                                     int dim, et_dtype dtype, et_memspace mem,
+                                     const double *sigmas, int nsig, int64_t nperm, uint64_t seed,
+                                     double *T_perm, et_perm_result *out);
+
 /* Sect. 5 split (Eq. 4): C = pB . (pC x pD), momenta [n][3]
  * double in the mother rest frame.  positive[i] = 1 iff C > 0 (is_conjugate = 0)
  * or -C > 0 (is_conjugate = 1, momenta of the C-conjugate particles); C == 0 is

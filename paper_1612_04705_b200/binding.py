@@ -28,7 +28,7 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_set_shard", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums", "et_scp"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_permutation_test_sigmas", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums", "et_scp"]
 
 
 class EtError(RuntimeError):
@@ -236,6 +236,7 @@ def lib():
             "et_bkg_permutation_test": bkg + [i64, u64, vp, vp],
             "et_gev_pvalue": [vp, i64, dbl, vp, i64, vp],
             "et_permutation_test": [vp] + wsample + tail + [i64, u64, vp, vp],
+            "et_permutation_test_sigmas": [vp] + wsample + [ci, ci, ci, vp, ci, i64, u64, vp, vp],
             "et_podd_split": [vp, vp, vp, vp, i64, ci, ci, vp, vp],
             "et_podd_test": [vp] + wsample + tail + [i64, u64, vp, vp],
             "et_perm_labels": [vp, i64, i64, i64, u64, ci, vp],
@@ -478,6 +479,20 @@ class Context:
                                               C.c_double(sigma), C.c_int64(nperm), C.c_uint64(seed),
                                               Tp.ctypes.data_as(C.c_void_p), C.byref(out)))
         return PermResult(_res(out.observed), out.p_value, out.count_gt, out.n_near, out.nperm, Tp)
+
+    def permutation_test_sigmas(self, x, xbar, sigmas, nperm: int, seed: int, wx=None, wxbar=None) -> list:
+        """The permutation test at several sigma (the scan of Fig. 2): one PermResult per sigma, labels generated once."""
+        ax, ab = _coords(x, xbar)
+        awx, awb = _weights(ax, ab, wx, wxbar)
+        sg = np.ascontiguousarray(np.asarray(sigmas, dtype=np.float64).reshape(-1))
+        Tp = np.zeros((max(len(sg), 1), max(int(nperm), 1)), dtype=np.float64)
+        out = (_PermResult * max(len(sg), 1))()
+        self._check(lib().et_permutation_test_sigmas(
+            self._h, ax.ptr, awx.ptr, C.c_int64(ax.shape[0]), ab.ptr, awb.ptr, C.c_int64(ab.shape[0]), C.c_int(ax.shape[1]),
+            C.c_int(ax.dtype), C.c_int(ax.mem), sg.ctypes.data_as(C.c_void_p), C.c_int(len(sg)), C.c_int64(nperm), C.c_uint64(seed),
+            Tp.ctypes.data_as(C.c_void_p), out))
+        return [PermResult(_res(out[k].observed), out[k].p_value, out[k].count_gt, out[k].n_near, out[k].nperm, Tp[k].copy())
+                for k in range(len(sg))]
 
     # ---------------------------------------------------------------- Sect. 5
     def podd_split(self, pB, pC, pD, is_conjugate: bool):

@@ -1008,22 +1008,24 @@ et_status run_escalation(et_ctx *ctx, const Layout &L, int dim, int nperm, uint6
 // Labels (TC layout), the contraction for every 512-column chunk, W_c, then the statistic.
 // lab2_classes: class segments that form sample X of the second labelling (column 1).
 et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted, unsigned lab2_classes,
-                      long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second)
+                      long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second,
+                      bool reuse_labels = false)
 {
     const int nchunks = (nperm + tc::kPermsPerChunk - 1) / tc::kPermsPerChunk;
     const int words_total = nchunks * tc::kWordsPerChunk;
-    // labels
+    // labels (reuse_labels: ctx->sel and ctx->maskT still hold those of the same (layout, nperm, seed), written by the
+    // previous sigma of et_permutation_test_sigmas)
     ET_TRY(span_begin(ctx, 4));
-    ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
     // the j range of the contraction is padded to whole K blocks: rows npad .. npadK - 1 carry zero labels and zero records
     const long long npadK = (L.npad + tc::kKB - 1) / tc::kKB * tc::kKB;
-    ET_TRY(ensure(ctx, ctx->maskT, (size_t)npadK * words_total * sizeof(uint32_t)));
-    CUDA_TRY(cudaMemsetAsync(ctx->maskT.p, 0, (size_t)npadK * words_total * sizeof(uint32_t), ctx->stream));
     LabelOut lo{};
     lo.nseg = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
     for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
-    {
+    if (!reuse_labels) {
+        ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
+        ET_TRY(ensure(ctx, ctx->maskT, (size_t)npadK * words_total * sizeof(uint32_t)));
+        CUDA_TRY(cudaMemsetAsync(ctx->maskT.p, 0, (size_t)npadK * words_total * sizeof(uint32_t), ctx->stream));
         const dim3 grid((unsigned)((L.N + kThreads - 1) / kThreads), (unsigned)words_total);
         tc::k_label_write_tc<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, ctx->opt_perm_offset, (uint32_t)(seed & 0xffffffffu),
                                                                 (uint32_t)(seed >> 32), static_cast<const SelState *>(ctx->sel.p), lo,
@@ -1522,6 +1524,48 @@ et_status et_permutation_test(et_ctx *ctx, const void *x, const double *wx, int6
     }
     ET_TRY(end_call(ctx));
     *out = r;
+    return ET_OK;
+}
+
+et_status et_permutation_test_sigmas(et_ctx *ctx, const void *x, const double *wx, int64_t n, const void *xbar, const double *wxbar,
+                                     int64_t nbar, int dim, et_dtype dtype, et_memspace mem, const double *sigmas, int nsig,
+                                     int64_t nperm, uint64_t seed, double *T_perm, et_perm_result *out)
+{
+    if (!ctx) return ET_ERR_INVALID;
+    if (!sigmas || nsig < 1 || nsig > ET_MAX_SCAN) return fail(ctx, ET_ERR_INVALID, "nsig must be in 1..%d", ET_MAX_SCAN);
+    for (int s = 0; s < nsig; ++s) ET_TRY(check_common(ctx, x, n, xbar, nbar, dim, dtype, mem, sigmas[s]));
+    if (!out || !T_perm) return fail(ctx, ET_ERR_INVALID, "null output");
+    if ((wx == nullptr) != (wxbar == nullptr)) return fail(ctx, ET_ERR_INVALID, "give both weight arrays or neither");
+    if (nperm < 1 || nperm > ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "nperm must be in 1..%d", ET_MAX_NPERM);
+    ET_TRY(begin_call(ctx));
+    const void *dx = nullptr, *dxb = nullptr, *dwx = nullptr, *dwb = nullptr;
+    ET_TRY(stage_in(ctx, x, (size_t)n * dim * elem_size(dtype), mem, ctx->in_x, &dx));
+    ET_TRY(stage_in(ctx, xbar, (size_t)nbar * dim * elem_size(dtype), mem, ctx->in_xbar, &dxb));
+    ET_TRY(stage_in(ctx, wx, (size_t)n * 8, mem, ctx->in_wx, &dwx));
+    ET_TRY(stage_in(ctx, wxbar, (size_t)nbar * 8, mem, ctx->in_wxbar, &dwb));
+    Layout L;
+    layout_two(L, n, nbar);
+    ET_TRY(upload_tile_classes(ctx, L));
+    std::vector<et_perm_result> res((size_t)nsig);
+    std::vector<double> tp((size_t)nsig * (size_t)nperm);
+    const bool tcpath = use_tc(ctx, L);
+    int nwords = 0;
+    for (int s = 0; s < nsig; ++s) {
+        // the records carry the scale of sigma; the labels depend on (N, n, nperm, seed) only and are generated once
+        ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigmas[s]));
+        if (tcpath) {
+            ET_TRY(run_perm_tc(ctx, L, dim, (int)nperm, seed, wx != nullptr, 0x1u, pairs_two(n, nbar), pairs_two(n, nbar),
+                               tp.data() + (size_t)s * nperm, &res[(size_t)s], nullptr, s > 0));
+        } else {
+            if (s == 0) ET_TRY(run_labels_internal(ctx, L, (int)nperm, seed, &nwords));
+            ET_TRY(run_pairs_rows(ctx, L, dim));
+            ET_TRY(run_perm_sums(ctx, L, dim, nwords));
+            ET_TRY(finish_perm(ctx, nwords, nperm, pairs_two(n, nbar), (double)n, (double)nbar, tp.data() + (size_t)s * nperm, &res[(size_t)s]));
+        }
+    }
+    ET_TRY(end_call(ctx));
+    memcpy(T_perm, tp.data(), tp.size() * sizeof(double));
+    for (int s = 0; s < nsig; ++s) out[s] = res[(size_t)s];
     return ET_OK;
 }
 

@@ -657,6 +657,44 @@ def test_perm_sigma_scan_values(ctx, sigma, kernel):
     assert (np.argsort(got.T_perm) == np.argsort(exp.T_perm)).all()
 
 
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("weighted", [False, True])
+def test_permutation_test_sigmas_is_the_scan_of_single_calls(ctx, kernel, weighted):
+    """et_permutation_test_sigmas (Fig. 2: p-value versus sigma; BASELINE configs[1] / [3]: three sigma x the
+    same permutations): every sigma equals its own et_permutation_test call bit for bit (labels generated once, records
+    re-scaled per sigma), and the oracle within the tolerance (8 permutations from scratch per sigma)."""
+    c = dg.config(3 if weighted else 1, scale=0.1)
+    s = dg.make_sample(c)
+    sig = (0.1, 0.3, 0.5)
+    with force_kernel(ctx, kernel):
+        scan = ctx.permutation_test_sigmas(s.x, s.xbar, sig, 8, c.perm_seed, s.wx, s.wxbar)
+        assert len(scan) == 3
+        for sg, got in zip(sig, scan):
+            one = ctx.permutation_test(s.x, s.xbar, sg, 8, c.perm_seed, s.wx, s.wxbar)
+            # CUDA-core path with one mask word: the row sums (k_pairs_rows) outweigh the one k_perm32 launch
+            assert ctx.stats().dominant_kernel in (("k_perm_tc",) if kernel == 0 else ("k_perm32", "k_pairs_rows"))
+            assert (got.T_perm == one.T_perm).all() and got.observed == one.observed
+            assert (got.count_gt, got.n_near, got.p_value) == (one.count_gt, one.n_near, one.p_value)
+            exp = oracle.perm_test(s.x, s.xbar, sg, 8, c.perm_seed, s.wx, s.wxbar)
+            check_perm(got, exp, term_rel=TERM_REL_TC * (4 if weighted else 1) if kernel == 0 else 0.0)
+    # the scan sees the injected asymmetry differently at each sigma: three distinct observed T values
+    assert len({r.observed.T for r in scan}) == 3
+
+
+def test_permutation_test_sigmas_errors(ctx):
+    rng = np.random.default_rng(5)
+    x, xb = rng.uniform(size=(300, 2)), rng.uniform(size=(200, 2))
+    with pytest.raises(binding.EtError) as e:
+        ctx.permutation_test_sigmas(x, xb, (0.3, -1.0), 4, 1)
+    assert e.value.status == -2
+    with pytest.raises(binding.EtError) as e:
+        ctx.permutation_test_sigmas(x, xb, [0.1] * 17, 4, 1)
+    assert e.value.status == -1
+    one = ctx.permutation_test_sigmas(x, xb, (0.25,), 40, 9)[0]
+    ref = ctx.permutation_test(x, xb, 0.25, 40, 9)
+    assert (one.T_perm == ref.T_perm).all() and one.count_gt == ref.count_gt
+
+
 # ----------------------------------------------------------------------------- oracle anchor at the bench sizes
 def _golden():
     import os
