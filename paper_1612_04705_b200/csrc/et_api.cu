@@ -367,8 +367,19 @@ et_status run_pairs_T_multi_ns(et_ctx *ctx, const Layout &L, int dim, const floa
 }
 
 // K-ROW: rowsum[c][row] for all rows.
+// Grid of the CUDA-core permutation sums (grid_term, kFlushJ): step G = 2^(e + k - 24) with 2^e >= max |w| and
+// 2^k >= min(N, kFlushJ), the most terms of one fp32 partial sum that can be non-zero; magic = 1.5 * 2^23 G.
+double perm32_grid(const et_ctx *ctx, long long N)
+{
+    const double wabs = std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin));
+    int e = 0, k = 0;
+    if (std::frexp(wabs > 0 ? wabs : 1.0, &e) == 0.5) --e;  // wabs = m 2^e, 0.5 <= m < 1: the smallest e with 2^e >= wabs
+    while ((1ll << k) < std::min<long long>(N, kFlushJ)) ++k;
+    return std::ldexp(1.0, e + k - 24);
+}
+
 template <int C>
-et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
+et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim, float magic)
 {
     const int nT = (int)(L.npad / (kThreads * kRRow));
     RowSegs segs{};
@@ -381,7 +392,7 @@ et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
         int grid = resident_blocks(ctx, k_pairs_rows<D, kRRow, C>);
         if (grid > nT) grid = nT;
         k_pairs_rows<D, kRRow, C><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), nT, L.npad,
-                                                                    static_cast<const uint8_t *>(ctx->tilecls.p), segs,
+                                                                    static_cast<const uint8_t *>(ctx->tilecls.p), segs, magic,
                                                                     static_cast<int *>(ctx->counter.p),
                                                                     static_cast<double *>(ctx->rowsum.p));
         LAUNCH_CHECK();
@@ -390,9 +401,11 @@ et_status run_pairs_rows_c(et_ctx *ctx, const Layout &L, int dim)
     ctx->stats.pair_evals += L.npad * L.npad;
     return ET_OK;
 }
-et_status run_pairs_rows(et_ctx *ctx, const Layout &L, int dim)
+// on_grid: the permutation path (terms rounded to the grid); false: plain fp32 terms (et_row_sums)
+et_status run_pairs_rows(et_ctx *ctx, const Layout &L, int dim, bool on_grid = true)
 {
-    return L.ncls == 2 ? run_pairs_rows_c<2>(ctx, L, dim) : run_pairs_rows_c<4>(ctx, L, dim);
+    const float magic = on_grid ? (float)(12582912.0 * perm32_grid(ctx, L.N)) : 0.0f;
+    return L.ncls == 2 ? run_pairs_rows_c<2>(ctx, L, dim, magic) : run_pairs_rows_c<4>(ctx, L, dim, magic);
 }
 
 // ---- labels ----------------------------------------------------------------------------------------------
@@ -561,7 +574,7 @@ struct DevPerm {
     int status;
 };
 __global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q, const double *__restrict__ RW, int nwords, int nperm,
-                                                  long long npairs, double nA, double nB, double wabs, double *__restrict__ T_perm, DevPerm *out)
+                                                  long long npairs, double nA, double nB, double wabs, double qstep, double *__restrict__ T_perm, DevPerm *out)
 {
     // RW layout: [g][which][kRWCols]
     __shared__ DevT obs;
@@ -576,7 +589,9 @@ __global__ void __launch_bounds__(256) k_perm_stat(const double *__restrict__ Q,
     }
     __syncthreads();
     const double Tobs = obs.r.T;
-    const double guard = guard_band(kPairErrF32 * wabs * wabs, nA, nB, obs.r.W, obs.r.Wbar, fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb));
+    // every term w_j psi_ij sits on the grid of step qstep / |w_i| (grid_term): a rounding error of variance qstep^2 / 12
+    const double e32 = kPairErrF32 * wabs * wabs;
+    const double guard = guard_band(sqrt(e32 * e32 + qstep * qstep / 12.0), nA, nB, obs.r.W, obs.r.Wbar, fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb));
     unsigned long long cnt = 0, near = 0;
     for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
         const int c = p + 1, g = c >> 5, b = c & 31;
@@ -750,6 +765,7 @@ et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
     const long long nunits = (long long)nT * (nT + 1) / 2;
     ET_TRY(ensure(ctx, ctx->Q, (size_t)nwords * 32 * sizeof(double)));
     ET_TRY(span_begin(ctx, 2));
+    const float magic = (float)(12582912.0 * perm32_grid(ctx, L.N));
     DISPATCH_DIM(dim, {
         int grid = resident_blocks(ctx, k_perm32<D>);
         if ((long long)grid > nunits) grid = (int)nunits;
@@ -757,7 +773,7 @@ et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
         for (int g = 0; g < nwords; ++g) {
             k_perm32<D><<<grid, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p),
                                                            static_cast<const uint32_t *>(ctx->mask.p) + (long long)g * L.npad, nT,
-                                                           nunits, static_cast<double *>(ctx->partQ.p));
+                                                           nunits, magic, static_cast<double *>(ctx->partQ.p));
             LAUNCH_CHECK();
             k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partQ.p), grid, 32,
                                                      static_cast<double *>(ctx->Q.p) + g * 32);
@@ -794,10 +810,11 @@ et_status run_perm_sums(et_ctx *ctx, const Layout &L, int dim, int nwords)
 
 et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, double nA, double nB, double *T_perm, et_perm_result *out)
 {
+    const double wabs_ = std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin));
     ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
     k_perm_stat<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->Q.p), static_cast<const double *>(ctx->RW.p), nwords,
-                                            (int)nperm, npairs, nA, nB, std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin)),
+                                            (int)nperm, npairs, nA, nB, wabs_, perm32_grid(ctx, (long long)(nA + nB)) * wabs_,
                                             static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p));
     LAUNCH_CHECK();
     DevPerm r;
@@ -1744,7 +1761,7 @@ et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n, c
     layout_two(L, n, nbar);
     ET_TRY(upload_tile_classes(ctx, L));
     ET_TRY(run_prep(ctx, dx, dxb, static_cast<const double *>(dwx), static_cast<const double *>(dwb), nullptr, L, dim, dtype, sigma));
-    ET_TRY(run_pairs_rows(ctx, L, dim));
+    ET_TRY(run_pairs_rows(ctx, L, dim, false));
     std::vector<long long> pos((size_t)nrows);
     for (int64_t k = 0; k < nrows; ++k) pos[(size_t)k] = rows[k] < n ? rows[k] : L.seg_pos[1] + (rows[k] - n);
     ET_TRY(ensure(ctx, ctx->rows, (size_t)nrows * 8));

@@ -11,6 +11,18 @@ constexpr int kTileJ = 256;     // j rows staged in shared memory per step
 constexpr int kPad = 1024;      // every class segment is padded to a multiple of this many rows
 constexpr int kMaxCls = 4;      // classes in the pooled layout (2 for X/Xbar, 4 for the Sect. 5 split)
 constexpr int kSumSlots = 16;   // class-pair block sums, slot c1 * 4 + c2 with c1 <= c2
+// The CUDA-core PERMUTATION kernels (k_pairs_rows, k_perm32) keep an fp32 partial sum over this many pairs only, and the
+// terms they add are first rounded to a fixed grid on which such a partial sum is exact (grid_term, et_kernels.cuh).  Why: an
+// fp32 accumulator of size A drops the part of every addend below ulp(A) / 2; psi has most of its mass near 0 (far
+// pairs, density ~ 1 / psi), so the loss is a bias proportional to ulp(A) -- and the accumulators of a random labelling
+// (half the j of a block) are half as large as those of the row sums r_i and of the contiguous observed labelling.
+// Measured against the oracle (tests/test_gpu_parity.py::test_error_model_of_the_decision): with 256 plain fp32 adds per
+// partial every T_p sat +7e-9 above its oracle value at sigma = 0.3 while T_obs was exact (2e-8 of the term scale, far
+// inside the 1e-6 tolerance of T but 30 sigma of the error model that certifies T_p > T_obs); 32 adds left +5e-10; on the
+// grid Q_p, R_p and S are exact sums of the same numbers and the offset is gone, as on the tensor-core path.
+// (k_pairs_T sums whole blocks of contiguous classes: every class pair carries the same relative loss, which cancels in
+// T like the 6e-8 bias of ex2.approx.)
+constexpr int kFlushJ = 32;
 
 // Floats per event record in the pooled layout: dim coordinates, then the weight, zero padded to a float4 multiple.
 __host__ __device__ constexpr int rec_floats(int dim) { return (dim + 1 + 3) / 4 * 4; }

@@ -127,6 +127,11 @@ __global__ void k_prep(const TIn *__restrict__ x, const TIn *__restrict__ xbar, 
 }
 
 // ------------------------------------------------------------------------------------------------ all pairs
+// w_j psi_ij rounded to the nearest multiple of the grid step G that `magic` = 1.5 * 2^23 G encodes (magic = 0: no
+// rounding).  The CUDA-core permutation kernels sum these terms: up to kFlushJ of them, |term| <= 2^23 G / kFlushJ, add up
+// EXACTLY in fp32, so Q_p, the row sums r_i and S are sums of the same numbers whatever the labels (kFlushJ, et_device.cuh).
+__device__ __forceinline__ float grid_term(float psi, float w, float magic) { return __fadd_rn(__fmaf_rn(psi, w, magic), -magic); }
+
 // One j record from shared memory: coordinates and weight.
 template <int D>
 struct JRec {
@@ -392,7 +397,7 @@ struct RowSegs {
 };
 template <int D, int R, int C>
 __global__ void __launch_bounds__(kThreads) k_pairs_rows(const float *__restrict__ rec, int nT, long long npad,
-                                                        const uint8_t *__restrict__ tile_cls, RowSegs segs,
+                                                        const uint8_t *__restrict__ tile_cls, RowSegs segs, float magic,
                                                         int *__restrict__ counter, double *__restrict__ rowsum)
 {
     constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
@@ -433,22 +438,25 @@ __global__ void __launch_bounds__(kThreads) k_pairs_rows(const float *__restrict
                     for (int q = 0; q < F4; ++q) sj[tid * F4 + q] = __ldg(p + q);
                 }
                 __syncthreads();
-                float acc[R];
+                // fp32 over kFlushJ pairs only (see kFlushJ), fp64 beyond
+                for (int jb = 0; jb < kTileJ; jb += kFlushJ) {
+                    float acc[R];
 #pragma unroll
-                for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+                    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
 #pragma unroll 4
-                for (int j = 0; j < kTileJ; ++j) {
-                    const JRec<D> rj = load_jrec<D>(sj, j);
+                    for (int j = jb; j < jb + kFlushJ; ++j) {
+                        const JRec<D> rj = load_jrec<D>(sj, j);
 #pragma unroll
-                    for (int r = 0; r < R; ++r) acc[r] = __fmaf_rn(psi_pair<D>(ui[r], rj.u), rj.w, acc[r]);
+                        for (int r = 0; r < R; ++r) acc[r] = __fadd_rn(acc[r], grid_term(psi_pair<D>(ui[r], rj.u), rj.w, magic));
+                    }
+#pragma unroll
+                    for (int r = 0; r < R; ++r) racc[r][c] += (double)acc[r];
                 }
-#pragma unroll
-                for (int r = 0; r < R; ++r) racc[r][c] += (double)acc[r];
             }
             // the row's own term w_i * psi_ii = w_i sits in its own class
             if (c == ci) {
 #pragma unroll
-                for (int r = 0; r < R; ++r) racc[r][c] -= (double)wi[r];
+                for (int r = 0; r < R; ++r) racc[r][c] -= (double)grid_term(1.0f, wi[r], magic);
             }
 #pragma unroll
             for (int r = 0; r < R; ++r) rowsum[(long long)c * npad + (long long)I * TI + r * kThreads + tid] = racc[r][c];
@@ -462,11 +470,11 @@ __global__ void __launch_bounds__(kThreads) k_pairs_rows(const float *__restrict
 // the end.  Columns: c = 0 is the observed labelling, c = p + 1 permutation p.
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1) k_perm32(const float *__restrict__ rec, const uint32_t *__restrict__ maskg,
-                                                       int nT, long long nunits, double *__restrict__ partialQ)
+                                                       int nT, long long nunits, float magic, double *__restrict__ partialQ)
 {
     constexpr int R = 2, F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
     __shared__ float4 sj[kTileJ * F4];
-    __shared__ float4 lab[kTileJ * 8];  // lab[j][c] = a_jc * w_j
+    __shared__ float4 lab[kTileJ * 8];  // lab[j][c] = a_jc as 0.f / 1.f
     const int tid = threadIdx.x;
     double q[32];
 #pragma unroll
@@ -499,60 +507,58 @@ __global__ void __launch_bounds__(kThreads, 1) k_perm32(const float *__restrict_
             {
                 const long long row = (long long)J * TI + sub * kTileJ + tid;
                 const float4 *p = reinterpret_cast<const float4 *>(rec + row * F);
-                float wj = 0.f;
 #pragma unroll
-                for (int qq = 0; qq < F4; ++qq) {
-                    const float4 t = __ldg(p + qq);
-                    sj[tid * F4 + qq] = t;
-                    if (qq == D / 4) wj = (D % 4 == 0) ? t.x : (D % 4 == 1) ? t.y : (D % 4 == 2) ? t.z : t.w;
-                }
+                for (int qq = 0; qq < F4; ++qq) sj[tid * F4 + qq] = __ldg(p + qq);
                 const uint32_t m = __ldg(maskg + row);
 #pragma unroll
                 for (int c4 = 0; c4 < 8; ++c4) {
                     float4 l;
-                    l.x = (m >> (4 * c4) & 1u) ? wj : 0.f;
-                    l.y = (m >> (4 * c4 + 1) & 1u) ? wj : 0.f;
-                    l.z = (m >> (4 * c4 + 2) & 1u) ? wj : 0.f;
-                    l.w = (m >> (4 * c4 + 3) & 1u) ? wj : 0.f;
+                    l.x = (m >> (4 * c4) & 1u) ? 1.f : 0.f;
+                    l.y = (m >> (4 * c4 + 1) & 1u) ? 1.f : 0.f;
+                    l.z = (m >> (4 * c4 + 2) & 1u) ? 1.f : 0.f;
+                    l.w = (m >> (4 * c4 + 3) & 1u) ? 1.f : 0.f;
                     lab[tid * 8 + c4] = l;
                 }
             }
             __syncthreads();
-            float y[R][32];
+            // fp32 over kFlushJ pairs only (see kFlushJ), fp64 beyond
+            for (int jb = 0; jb < kTileJ; jb += kFlushJ) {
+                float y[R][32];
 #pragma unroll
-            for (int r = 0; r < R; ++r)
+                for (int r = 0; r < R; ++r)
 #pragma unroll
-                for (int c = 0; c < 32; ++c) y[r][c] = 0.f;
+                    for (int c = 0; c < 32; ++c) y[r][c] = 0.f;
 #pragma unroll 2
-            for (int j = 0; j < kTileJ; ++j) {
-                const JRec<D> rj = load_jrec<D>(sj, j);
-                float ps[R];
+                for (int j = jb; j < jb + kFlushJ; ++j) {
+                    const JRec<D> rj = load_jrec<D>(sj, j);
+                    float ps[R];
 #pragma unroll
-                for (int r = 0; r < R; ++r) ps[r] = psi_pair<D>(ui[r], rj.u);
+                    for (int r = 0; r < R; ++r) ps[r] = grid_term(psi_pair<D>(ui[r], rj.u), rj.w, magic);  // w_j psi_ij on the grid
 #pragma unroll
-                for (int c4 = 0; c4 < 8; ++c4) {
-                    const float4 l = lab[j * 8 + c4];
+                    for (int c4 = 0; c4 < 8; ++c4) {
+                        const float4 l = lab[j * 8 + c4];
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        y[r][4 * c4] = __fmaf_rn(ps[r], l.x, y[r][4 * c4]);
-                        y[r][4 * c4 + 1] = __fmaf_rn(ps[r], l.y, y[r][4 * c4 + 1]);
-                        y[r][4 * c4 + 2] = __fmaf_rn(ps[r], l.z, y[r][4 * c4 + 2]);
-                        y[r][4 * c4 + 3] = __fmaf_rn(ps[r], l.w, y[r][4 * c4 + 3]);
+                        for (int r = 0; r < R; ++r) {
+                            y[r][4 * c4] = __fmaf_rn(ps[r], l.x, y[r][4 * c4]);
+                            y[r][4 * c4 + 1] = __fmaf_rn(ps[r], l.y, y[r][4 * c4 + 1]);
+                            y[r][4 * c4 + 2] = __fmaf_rn(ps[r], l.z, y[r][4 * c4 + 2]);
+                            y[r][4 * c4 + 3] = __fmaf_rn(ps[r], l.w, y[r][4 * c4 + 3]);
+                        }
                     }
                 }
-            }
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const double fw = f * (double)wi[r];
+                for (int r = 0; r < R; ++r) {
+                    const double fw = f * (double)wi[r];
 #pragma unroll
-                for (int c = 0; c < 32; ++c)
-                    if (mi[r] >> c & 1u) q[c] += fw * (double)y[r][c];
+                    for (int c = 0; c < 32; ++c)
+                        if (mi[r] >> c & 1u) q[c] += fw * (double)y[r][c];
+                }
             }
         }
         if (diag) {  // remove the i == j terms: a_ic w_i^2 psi_ii, halved like the rest of the diagonal tile
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const double s = 0.5 * (double)wi[r] * (double)wi[r];
+                const double s = 0.5 * (double)wi[r] * (double)grid_term(1.0f, wi[r], magic);
 #pragma unroll
                 for (int c = 0; c < 32; ++c)
                     if (mi[r] >> c & 1u) q[c] -= s;

@@ -856,6 +856,41 @@ def test_escalation_weighted_and_podd(ctx):
         assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
 
 
+# ----------------------------------------------------------------------------- the error model behind the guard band
+@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("index,scale,sigma", [(1, 0.2, 0.3), (1, 0.2, 0.1), (2, 0.1, 0.2)])
+def test_error_model_of_the_decision(ctx, kernel, index, scale, sigma):
+    """the guard band is 8 sigma of T_p - T_obs under the model 'every pair carries an independent
+    error' -- 2^-22 of the fp32 psi and step / sqrt(12) of the rounding of w_j psi_ij to the path's grid.  Measured against
+    the oracle over 24 permutations (n = nbar = 20 000 and 30 000): the errors of T_p, of T_obs and of T_p - T_obs stay
+    within the model -- rms below 1.5, maximum below 5 model sigmas, and no common offset of the T_p against T_obs (the
+    fp32 partial sums of the CUDA-core path had one of 10 .. 30 sigma before kFlushJ, et_device.cuh)."""
+    c = dg.config(index, scale=scale)
+    s = dg.make_sample(c)
+    n, nbar, nperm = c.n, c.nbar, 24
+    exp = oracle.perm_test(s.x, s.xbar, sigma, nperm, c.perm_seed)
+    ctx.set_option(binding.ET_OPT_EXACT_P, 0)
+    try:
+        with force_kernel(ctx, kernel):
+            got = ctx.permutation_test(s.x, s.xbar, sigma, nperm, c.perm_seed)
+            assert ctx.stats().dominant_kernel in (("k_perm_tc",) if kernel == 2 else ("k_perm32", "k_pairs_rows"))
+    finally:
+        ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+    # rounding step of w_j psi_ij: 1 / 32766 on the tensor-core path, 2^-19 on the CUDA-core path (grid_term: unit weights,
+    # fp32 partial sums of 32 terms)
+    step = 1 / 32766.0 if kernel == 2 else 2.0 ** -19
+    pair_err = math.sqrt(step ** 2 / 12 + (2.0 ** -22) ** 2)
+    var = 1 / (2.0 * n * (n - 1)) + 1 / (2.0 * nbar * (nbar - 1)) + 1.0 / (n * nbar)
+    sig = pair_err * math.sqrt(var)                       # model sigma of one T
+    e_p, e_o = got.T_perm - exp.T_perm, got.observed.T - exp.observed.T
+    e_d = (e_p - e_o) / math.sqrt(2.0)                    # T_p - T_obs, in units of ITS model sigma
+    report = (math.sqrt((e_p ** 2).mean()) / sig, e_p.mean() / sig, e_o / sig, math.sqrt((e_d ** 2).mean()) / sig)
+    assert math.sqrt((e_p ** 2).mean()) <= 1.5 * sig and np.abs(e_p).max() <= 5.0 * sig, report
+    assert abs(e_o) <= 5.0 * sig, report
+    assert math.sqrt((e_d ** 2).mean()) <= 1.5 * sig and np.abs(e_d).max() <= 5.0 * sig, report
+    assert abs(e_p.mean()) <= 5.0 * sig / math.sqrt(nperm) + 0.5 * sig, report
+
+
 # ----------------------------------------------------------------------------- unit-range shard (SURVEY 8(e))
 def _run_sharded(world, call, exact_p=16):
     """`world` contexts on this GPU, one host thread each, in lock step: the all-gather callback of et_set_shard is a
