@@ -265,13 +265,21 @@ def run_ours(args):
         st = ctx.stats()
         msT += st.ms_total
         msT_k += st.ms_pairs
+        formT = st.distance_form
     sm_mhz_max = peaks.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)
     roofT = alu_roofline_pairs_per_s(cfg.dim, sm_mhz_max)
     et_T = {"pairs_per_s": pairs1 / (msT / nT * 1e-3), "kernel_pairs_per_s": pairs1 / (msT_k / nT * 1e-3),
             "ms": msT / nT, "roofline_pairs_per_s": roofT, "frac": pairs1 / (msT_k / nT * 1e-3) / roofT,
             "frac_at_sampled_clock": (pairs1 / (msT_k / nT * 1e-3) / alu_roofline_pairs_per_s(cfg.dim, clocks["sm_mhz"])
                                       if clocks.get("sm_mhz") else None),
-            "peak_model": "min(128/(2D+1),16) pairs/clk/SM x 148 SMs x sm_max_mhz (FP32/SFU pipes)"}
+            "peak_model": "min(128/(2D+1),16) pairs/clk/SM x 148 SMs x sm_max_mhz (FP32/SFU pipes): the difference form of "
+                          "the distance, 2D+1 FP32 lane-ops and one MUFU.EX2 per pair (SURVEY 8(d))",
+            # the Gram form (ET_OPT_DISTANCE, default for D >= 4) needs D+2 lane-ops per pair: its own bound is
+            # min(128/(D+2),16), the SFU's 16 pairs/clk/SM for every D <= 6
+            "distance_form": {1: "differences", 2: "gram"}.get(formT, "?"),
+            "pairs_per_clk_per_sm": pairs1 / (msT_k / nT * 1e-3) / (NUM_SMS * sm_mhz_max * 1e6),
+            "frac_of_form_roofline": pairs1 / (msT_k / nT * 1e-3) / (min(128.0 / ((cfg.dim + 2) if formT == 2 else (2 * cfg.dim + 1)), 16.0)
+                                                                     * NUM_SMS * sm_mhz_max * 1e6)}
 
     # sigma scan (configs with several sigma values, BASELINE configs[1] / [3]): one fused pass against separate et_T calls
     sigma_scan = None

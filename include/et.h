@@ -105,6 +105,8 @@ typedef struct {
     double ms_escalation;      /* device time of the guard-band escalation (ET_OPT_EXACT_P)         */
     int64_t n_near_before;     /* n_near of the tensor-core pass, before the escalation             */
     int64_t n_escalated;       /* permutations re-evaluated by the escalation                       */
+    int64_t distance_form;     /* ET_OPT_DISTANCE value the last all-pairs (k_pairs_T) launch of the
+                                  call ran with: 1 or 2; 0 if the call had none                      */
 } et_stats;
 
 /* Options for et_set_option. */
@@ -121,10 +123,18 @@ typedef enum {
                                disjoint ranges on several GPUs / calls form one test
                                (PAPER.md:219 farms permutations out the same way).
                                p0 + nperm must stay below 2^34                                    */
-    ET_OPT_EXACT_P = 2      /* guard-band escalation of the tensor-core path: re-evaluate up to this
+    ET_OPT_EXACT_P = 2,     /* guard-band escalation of the tensor-core path: re-evaluate up to this
                                many permutations (default 16, at most 64; 0 = off) whose T_p lies
                                inside the guard band of T_obs, one 5/8 all-pairs pass each on the
                                CUDA cores (a full pass when weighted); skipped when more are inside  */
+    ET_OPT_DISTANCE = 3     /* distance arithmetic of the all-pairs kernel of et_T / et_T_weighted /
+                               et_T_bkg and of the escalation: 1 = differences, e = sum_k (u_ik - u_jk)^2
+                               (2 dim + 1 FP32 operations per pair); 2 = Gram form, e = |u_i|^2 +
+                               |u_j|^2 - 2 u_i.u_j (dim + 2 operations; psi then carries a relative
+                               rounding error of about 8e-8 |u|^2_max, |u|^2_max the squared half
+                               diagonal of the bounding box over 2 sigma^2 / log2 e); 0 (default) =
+                               Gram form when dim >= 4, n + nbar >= 4096 and |u|^2_max <= 48, else differences
+                               (DESIGN.md section 6).  T stays within the 1e-6 tolerance either way    */
 } et_option;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t to

@@ -23,6 +23,7 @@ ET_HOST, ET_DEVICE = 0, 1
 ET_OPT_PERM_KERNEL = 0
 ET_OPT_PERM_OFFSET = 1
 ET_OPT_EXACT_P = 2
+ET_OPT_DISTANCE = 3
 STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ERR_NONFINITE", -4: "ET_ERR_DEGENERATE",
                 -5: "ET_ERR_NOMEM", -6: "ET_ERR_CUDA"}
 
@@ -77,7 +78,8 @@ class _Stats(C.Structure):
     _fields_ = [("ms_total", C.c_double), ("ms_pairs", C.c_double), ("ms_labels", C.c_double), ("launches", C.c_int64),
                 ("pair_evals", C.c_int64), ("ms_dominant", C.c_double), ("dominant_launches", C.c_int64),
                 ("dominant_ops", C.c_int64), ("dominant_kernel", C.c_char * 32), ("dominant_ops_executed", C.c_int64),
-                ("ms_escalation", C.c_double), ("n_near_before", C.c_int64), ("n_escalated", C.c_int64)]
+                ("ms_escalation", C.c_double), ("n_near_before", C.c_int64), ("n_escalated", C.c_int64),
+                ("distance_form", C.c_int64)]
 
 
 @dataclass
@@ -203,6 +205,7 @@ class Stats:
     ms_escalation: float = 0.0
     n_near_before: int = 0
     n_escalated: int = 0
+    distance_form: int = 0
 
 
 _lib = None
@@ -409,7 +412,7 @@ class Context:
         self._check(lib().et_get_stats(self._h, C.byref(s)))
         return Stats(s.ms_total, s.ms_pairs, s.ms_labels, s.launches, s.pair_evals, s.ms_dominant, s.dominant_launches,
                      s.dominant_ops, s.dominant_kernel.decode(), s.dominant_ops_executed, s.ms_escalation, s.n_near_before,
-                     s.n_escalated)
+                     s.n_escalated, s.distance_form)
 
     # ---------------------------------------------------------------- Eq. 2
     def T(self, x, xbar, sigma: float) -> Result:

@@ -67,6 +67,8 @@ struct et_ctx {
     Buf shardbuf;
     Buf rec2, tilecls2, esccls, escD, nearbuf, escw;
     double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
+    double umax2 = 0.0;             // bound of |u|^2 over the records of the last prep: squared half diagonal of the bounding box, scaled
+    int64_t opt_distance = 0;       // ET_OPT_DISTANCE
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     Buf scpcnt, scpS;
     bool tc_attr_set = false;
@@ -271,6 +273,11 @@ et_status run_prep_t(et_ctx *ctx, const TIn *x, const TIn *xbar, const double *w
     PrepParams P{};
     for (int k = 0; k < dim; ++k) P.centre[k] = 0.5 * ((double)key2f(h[32 + 2 * k]) + (double)key2f(h[32 + 2 * k + 1]));
     P.scale = std::sqrt(1.4426950408889634074 / (2.0 * sigma * sigma));
+    ctx->umax2 = 0.0;
+    for (int k = 0; k < dim; ++k) {
+        const double half = 0.5 * ((double)key2f(h[32 + 2 * k + 1]) - (double)key2f(h[32 + 2 * k])) * P.scale;
+        ctx->umax2 += half * half;
+    }
     P.n = L.n; P.nbar = L.nbar; P.npad = L.npad; P.dim = dim; P.ncls = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) P.seg_pos[c] = L.seg_pos[c];
     for (int c = 0; c < L.ncls; ++c) P.seg_count[c] = L.seg_count[c];
@@ -317,6 +324,20 @@ et_status shard_sum(et_ctx *ctx, void *dev, int count, bool is_f64);
 // K-T: class-pair sums into ctx->sums (device, kSumSlots doubles).  rec / tilecls default to the call's own layout;
 // skip_mask drops class pairs (k_pairs_T); `booked` = false keeps the pass out of the per-kernel-class statistics (the
 // escalation books its own time).
+// Distance arithmetic of k_pairs_T (et_kernels.cuh): the Gram form when it pays -- dim >= 4, where the difference form is
+// bound by the FP32 pipe (2 dim + 1 > 8 lane-ops per pair against 16 MUFU per clock and SM; measured at dim = 2: 14.9 vs
+// 14.5 pairs/clk/SM, at dim = 5: 9.1 vs 11.4) -- and when the sample is large enough for its rounding noise to average far
+// below the tolerance of T (>= kGramMinN events: the noise of T falls like 1 / N) and compact enough in units of sigma
+// (|u|^2 <= kGramMaxU2: a per-pair error of psi below 4e-6); else differences.  ET_OPT_DISTANCE overrides.
+constexpr long long kGramMinN = 4096;
+constexpr double kGramMaxU2 = 48.0;
+bool use_gram(const et_ctx *ctx, const Layout &L, int dim)
+{
+    if (ctx->opt_distance == 1) return false;
+    if (ctx->opt_distance == 2) return true;
+    return dim >= 4 && L.N >= kGramMinN && ctx->umax2 <= kGramMaxU2;
+}
+
 et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim, const float *rec = nullptr, const uint8_t *tilecls = nullptr,
                       unsigned skip_mask = 0u, bool booked = true)
 {
@@ -326,13 +347,19 @@ et_status run_pairs_T(et_ctx *ctx, const Layout &L, int dim, const float *rec = 
     const long long nunits = (long long)nT * (nT + 1) / 2;
     ET_TRY(ensure(ctx, ctx->sums, kSumSlots * sizeof(double)));
     if (booked) ET_TRY(span_begin(ctx, 2));
+    const bool gram = use_gram(ctx, L, dim);
+    ctx->stats.distance_form = gram ? 2 : 1;
     DISPATCH_DIM(dim, {
-        int grid = resident_blocks(ctx, k_pairs_T<D, kRT>);
+        int grid = gram ? resident_blocks(ctx, k_pairs_T<D, kRT, true>) : resident_blocks(ctx, k_pairs_T<D, kRT, false>);
         const long long mine = (nunits - ctx->shard_rank + ctx->shard_world - 1) / ctx->shard_world;  // units of this rank
         if ((long long)grid > mine) grid = (int)std::max<long long>(mine, 1);
         ET_TRY(ensure(ctx, ctx->partials, (size_t)grid * kSumSlots * sizeof(double)));
-        k_pairs_T<D, kRT><<<grid, kThreads, 0, ctx->stream>>>(rec, nT, tilecls, nunits, skip_mask, ctx->shard_rank, ctx->shard_world,
-                                                             static_cast<double *>(ctx->partials.p));
+        if (gram)
+            k_pairs_T<D, kRT, true><<<grid, kThreads, 0, ctx->stream>>>(rec, nT, tilecls, nunits, skip_mask, ctx->shard_rank, ctx->shard_world,
+                                                                       static_cast<double *>(ctx->partials.p));
+        else
+            k_pairs_T<D, kRT, false><<<grid, kThreads, 0, ctx->stream>>>(rec, nT, tilecls, nunits, skip_mask, ctx->shard_rank, ctx->shard_world,
+                                                                        static_cast<double *>(ctx->partials.p));
         LAUNCH_CHECK();
         k_reduce_cols<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->partials.p), grid, kSumSlots,
                                                  static_cast<double *>(ctx->sums.p));
@@ -830,7 +857,7 @@ et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, 
 // ---- tensor-core permutation sums (K-PERM-TC) -------------------------------------------------------------
 // T for every label column of the TC layout (et_tc.cuh): chunk ch, column c at index ch * 512 + c.
 __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__ Q, const double *__restrict__ R, const double *__restrict__ W,
-                                                     int nperm, long long npairs_obs, long long npairs_second, double qstep, double wabs,
+                                                     int nperm, long long npairs_obs, long long npairs_second, double qstep, double egram, double wabs,
                                                      double nA, double nB, double *__restrict__ T_perm, DevPerm *out, DevT *second, DevNear *nearout)
 {
     __shared__ DevT obs;
@@ -854,7 +881,8 @@ __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__
     const double scale = fabs(obs.r.T_xx) + fabs(obs.r.T_bb) + fabs(obs.r.T_xb);
     const double e32 = kPairErrF32 * wabs * wabs;
     const double guard = guard_band(sqrt(tc::kQuantVar * qstep * qstep + e32 * e32), nA, nB, obs.r.W, obs.r.Wbar, scale);
-    if (threadIdx.x == 0) { nearout->guard = guard; nearout->guard_f32 = guard_band(e32, nA, nB, obs.r.W, obs.r.Wbar, scale); }
+    // the band of the escalation's arithmetic (k_pairs_T): fp32 psi, plus the rounding noise of the Gram form when it is used
+    if (threadIdx.x == 0) { nearout->guard = guard; nearout->guard_f32 = guard_band(sqrt(e32 * e32 + egram * egram), nA, nB, obs.r.W, obs.r.Wbar, scale); }
     unsigned long long cnt = 0, near = 0;
     for (int p = threadIdx.x; p < nperm; p += blockDim.x) {
         const int k = (p / tc::kPermsPerChunk) * tc::kCols + tc::kSpecial + p % tc::kPermsPerChunk;
@@ -1172,12 +1200,13 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // statistic
     const double wabs = std::max(std::fabs(ctx->wmax), std::fabs(ctx->wmin));
     const double qstep = wabs / sc;  // one rounding step of w_j psi_ij, times |w_i| <= wabs
+    const double egram = use_gram(ctx, L, dim) ? kGramErr * ctx->umax2 * wabs * wabs : 0.0;  // error of Psi_ij in the escalation's k_pairs_T
     ET_TRY(ensure(ctx, ctx->tperm, (size_t)nperm * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->result, sizeof(DevPerm) + sizeof(DevT) * 4));
     DevT *dev_second = reinterpret_cast<DevT *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm));
     ET_TRY(ensure(ctx, ctx->nearbuf, sizeof(DevNear)));
     k_perm_stat_tc<<<1, 256, 0, ctx->stream>>>(static_cast<const double *>(ctx->tcQ.p), static_cast<const double *>(ctx->tcR.p),
-                                               static_cast<const double *>(ctx->tcW.p), nperm, npairs_obs, npairs_second, qstep, wabs,
+                                               static_cast<const double *>(ctx->tcW.p), nperm, npairs_obs, npairs_second, qstep, egram, wabs,
                                                (double)L.n_a, (double)(L.N - L.n_a),
                                                static_cast<double *>(ctx->tperm.p), static_cast<DevPerm *>(ctx->result.p), dev_second,
                                                static_cast<DevNear *>(ctx->nearbuf.p));
@@ -1270,6 +1299,11 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
         // the Philox counter word of reading R4 is (uint32)(p >> 2): permutation indices stay below 2^34
         if (value < 0 || value > (1ll << 34) - ET_MAX_NPERM) return fail(ctx, ET_ERR_INVALID, "permutation offset out of range (p0 + nperm must stay below 2^34)");
         ctx->opt_perm_offset = value;
+        return ET_OK;
+    }
+    if (opt == ET_OPT_DISTANCE) {
+        if (value < 0 || value > 2) return fail(ctx, ET_ERR_INVALID, "ET_OPT_DISTANCE must be 0, 1 or 2");
+        ctx->opt_distance = value;
         return ET_OK;
     }
     if (opt == ET_OPT_EXACT_P) {

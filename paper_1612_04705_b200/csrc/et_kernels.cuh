@@ -168,14 +168,24 @@ __device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int 
 // skip_mask: bit c1 * 4 + c2 (c1 <= c2) set = tile pairs of that class pair are not evaluated (their slot stays 0);
 // the guard-band escalation needs six of the ten class-pair sums only.  Units unit0 + k * unit_step (k = 0, 1, ...) are
 // this launch's share: (0, 1) on one GPU, (rank, world) when the unit range is sharded over ranks.
-template <int D, int R>
+// GRAM: e_ij = |u_i|^2 + |u_j|^2 + sum_k u_ik (-2 u_jk) -- one FADD2 and D FFMA2 per two pairs instead of D FADD2, one
+// FMUL2 and D - 1 FFMA2, i.e. D + 2 instead of 2 D + 1 FP32-pipe lane-ops per pair (D = 5: 7 instead of 11; the kernel is
+// then bound by the 16 MUFU.EX2 per clock and SM).  Every operation rounds a value of size <= 2 (|u_i|^2 + |u_j|^2)
+// instead of the small difference, so psi carries a relative error of about kGramErr umax2 (umax2 = the largest |u|^2: the
+// squared half diagonal of the bounding box in units of sigma sqrt(2 / log2 e)) -- zero-mean rounding noise that averages
+// over the pairs, plus a per-event part from the rounding of |u_i|^2 that acts like a weight 1 + O(1e-7 umax2) on event i.
+// The host takes this form only for samples large enough for the noise to average far below the 1e-6 tolerance of T and
+// compact enough in units of sigma (run_pairs_T); the guard band of the escalation carries the extra term.
+constexpr double kGramErr = 8.262958e-08;  // 2^-23 ln 2
+template <int D, int R, bool GRAM>
 __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ rec, int nT,
                                                      const uint8_t *__restrict__ tile_cls, long long nunits,
                                                      unsigned skip_mask, int unit0, int unit_step,
                                                      double *__restrict__ partials)
 {
     constexpr int F = rec_floats(D), F4 = F / 4, TI = kThreads * R;
-    constexpr int NP = D + 1, NLD = (NP + 1) / 2;  // float2 entries / LDS.128 per j pair
+    constexpr int NP = D + (GRAM ? 2 : 1), NLD = (NP + 1) / 2;  // float2 entries / LDS.128 per j pair
+    constexpr int WI = GRAM ? D + 1 : D;                        // entry that holds the weights
     __shared__ float4 sj[kTileJ / 2 * NLD];
     __shared__ double s_sum[kSumSlots];
     __shared__ double s_warp[kThreads / 32];
@@ -188,7 +198,8 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
         const int slot = tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad];
         if (skip_mask >> slot & 1u) continue;
         float2 ui[R][D];
-        float wi[R];
+        float2 ai[GRAM ? R : 1];
+        float wi[R], self[R];   // self: w_i psi_ii as this kernel evaluates it (1 exactly with the difference form)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
@@ -202,6 +213,19 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
 #pragma unroll
             for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             wi[r] = v[D];
+            self[r] = v[D];
+            if (GRAM) {
+                float na = __fmul_rn(v[0], v[0]);
+#pragma unroll
+                for (int k = 1; k < D; ++k) na = __fmaf_rn(v[k], v[k], na);
+                ai[r] = __fadd2_rn(make_float2(na, na), make_float2(0.f, 0.f));
+                // psi_ii by the instruction sequence of the loop below (each half of a packed instruction rounds like
+                // the scalar one): what the diagonal tile adds for j = i, removed again after the loop
+                float e = __fadd_rn(na, na);
+#pragma unroll
+                for (int k = 0; k < D; ++k) e = __fmaf_rn(v[k], -2.f * v[k], e);
+                self[r] = __fmul_rn(ex2_approx(-e), v[D]);
+            }
         }
         double racc[R];
 #pragma unroll
@@ -218,9 +242,18 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
                     v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
                 }
                 float *o = reinterpret_cast<float *>(sj) + (tid >> 1) * (NLD * 4) + (tid & 1);
+                if (GRAM) {
+                    float nb = __fmul_rn(v[0], v[0]);
 #pragma unroll
-                for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
-                o[2 * D] = v[D];
+                    for (int k = 1; k < D; ++k) nb = __fmaf_rn(v[k], v[k], nb);
+#pragma unroll
+                    for (int k = 0; k < D; ++k) o[2 * k] = -2.f * v[k];
+                    o[2 * D] = nb;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < D; ++k) o[2 * k] = -v[k];
+                }
+                o[2 * WI] = v[D];
                 if (NP & 1) o[2 * NP] = 0.f;
             }
             __syncthreads();
@@ -238,14 +271,21 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
                 }
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    float2 d = __fadd2_rn(ui[r][0], nu[0]);
-                    float2 e = __fmul2_rn(d, d);
+                    float2 e;
+                    if (GRAM) {
+                        e = __fadd2_rn(ai[r], nu[D]);
 #pragma unroll
-                    for (int k = 1; k < D; ++k) {
-                        d = __fadd2_rn(ui[r][k], nu[k]);
-                        e = __ffma2_rn(d, d, e);
+                        for (int k = 0; k < D; ++k) e = __ffma2_rn(ui[r][k], nu[k], e);
+                    } else {
+                        float2 d = __fadd2_rn(ui[r][0], nu[0]);
+                        e = __fmul2_rn(d, d);
+#pragma unroll
+                        for (int k = 1; k < D; ++k) {
+                            d = __fadd2_rn(ui[r][k], nu[k]);
+                            e = __ffma2_rn(d, d, e);
+                        }
                     }
-                    acc[r] = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[D], acc[r]);
+                    acc[r] = __ffma2_rn(make_float2(ex2_approx(-e.x), ex2_approx(-e.y)), nu[WI], acc[r]);
                 }
             }
 #pragma unroll
@@ -254,7 +294,7 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
         double t = 0.0;
         const bool diag = I == J;
 #pragma unroll
-        for (int r = 0; r < R; ++r) t += (double)wi[r] * (diag ? racc[r] - (double)wi[r] : racc[r]);
+        for (int r = 0; r < R; ++r) t += (double)wi[r] * (diag ? racc[r] - (double)self[r] : racc[r]);
         if (diag) t *= 0.5;
         t = warp_sum(t);
         if ((tid & 31) == 0) s_warp[tid >> 5] = t;

@@ -63,7 +63,7 @@ def test_struct_sizes_match_header(lib):
     assert ctypes.sizeof(binding._Result) == 80
     assert ctypes.sizeof(binding._PermResult) == 80 + 32
     assert ctypes.sizeof(binding._PoddResult) == 32 + 80 + 112
-    assert ctypes.sizeof(binding._Stats) == 40 + 24 + 32 + 4 * 8
+    assert ctypes.sizeof(binding._Stats) == 40 + 24 + 32 + 5 * 8
     assert ctypes.sizeof(binding._BkgResult) == 4 * 8 + 10 * 8 + 2 * 8 + 8
     assert ctypes.sizeof(binding._BkgPermResult) == (4 + 10 + 2 + 1) * 8 + 4 * 8
     assert ctypes.sizeof(binding._GevResult) == 3 * 8 + 9 * 8 + 5 * 8 + 3 * 8

@@ -67,6 +67,64 @@ def test_T_random_all_dims(ctx, dim, dtype):
     assert_T_close(ctx.T(x, xb, sigma), oracle.T(x, xb, sigma))
 
 
+class force_distance:
+    """ET_OPT_DISTANCE for the duration of a block: 1 = differences, 2 = Gram form (k_pairs_T)."""
+
+    def __init__(self, ctx, form):
+        self.ctx, self.form = ctx, form
+
+    def __enter__(self):
+        self.ctx.set_option(binding.ET_OPT_DISTANCE, self.form)
+
+    def __exit__(self, *exc):
+        self.ctx.set_option(binding.ET_OPT_DISTANCE, 0)
+
+
+@pytest.mark.parametrize("dim", [1, 2, 4, 5, 8])
+@pytest.mark.parametrize("weighted", [False, True])
+def test_T_gram_form_matches_oracle(ctx, dim, weighted):
+    """The Gram form of the distance in k_pairs_T (|u_i|^2 + |u_j|^2 - 2 u_i.u_j: dim + 2 instead of 2 dim + 1 FP32
+    operations per pair), forced, against the oracle at the north-star tolerance; ragged sizes, diagonal tiles (the i = j
+    term is removed as evaluated), signed weights."""
+    rng = np.random.default_rng(300 + dim)
+    n, nbar = 2500 + 37 * dim, 2111
+    x, xb = rng.uniform(size=(n, dim)), rng.uniform(size=(nbar, dim)) ** 1.1
+    wx = rng.uniform(-0.5, 1.5, size=n) if weighted else None
+    wb = rng.uniform(-0.5, 1.5, size=nbar) if weighted else None
+    sigma = 0.2 * math.sqrt(dim)
+    exp = oracle.T(x, xb, sigma, wx, wb)
+    with force_distance(ctx, 2):
+        got = ctx.T_weighted(x, wx, xb, wb, sigma) if weighted else ctx.T(x, xb, sigma)
+        assert ctx.stats().distance_form == 2
+    assert_T_close(got, exp)
+    with force_distance(ctx, 1):
+        ref = ctx.T_weighted(x, wx, xb, wb, sigma) if weighted else ctx.T(x, xb, sigma)
+        assert ctx.stats().distance_form == 1
+    # the two forms agree far inside the tolerance at this size (errors of either: 1e-9 of the term scale or less)
+    assert abs(got.T - ref.T) <= 2e-8 * exp.term_scale
+
+
+def test_T_distance_form_dispatch(ctx):
+    """Default rule (et.h, ET_OPT_DISTANCE): Gram form only for dim >= 4, n + nbar >= 4096 and a sample that is compact in
+    units of sigma; everything else keeps the differences."""
+    rng = np.random.default_rng(9)
+    x5, y5 = rng.uniform(size=(3000, 5)), rng.uniform(size=(2000, 5))
+    ctx.T(x5, y5, 0.2)
+    assert ctx.stats().distance_form == 2
+    ctx.T(x5[:1500], y5, 0.2)                      # fewer than 4096 events
+    assert ctx.stats().distance_form == 1
+    ctx.T(x5, y5, 0.02)                            # half diagonal of the box >> sigma: |u|^2_max = 5 (0.5 * 42)^2 >> 48
+    assert ctx.stats().distance_form == 1
+    ctx.T(x5[:, :2].copy(), y5[:, :2].copy(), 0.2)  # dim = 2 is bound by the SFU either way
+    assert ctx.stats().distance_form == 1
+    far = x5.copy()
+    far[0] += 100.0                                # one outlier stretches the box
+    ctx.T(far, y5, 0.2)
+    assert ctx.stats().distance_form == 1
+    with pytest.raises(binding.EtError):
+        ctx.set_option(binding.ET_OPT_DISTANCE, 3)
+
+
 def test_T_config0_full(ctx):
     s = dg.make_sample(dg.config(0))
     exp = oracle.T(s.x, s.xbar, 0.3)
@@ -854,6 +912,32 @@ def test_escalation_weighted_and_podd(ctx):
     assert abs(got.count_gt - exp.count_gt) <= got.n_near
     if got.n_near == 0:
         assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
+
+
+def test_escalation_through_the_gram_form(ctx):
+    """dim = 5 and >= 4096 events: the escalation's k_pairs_T pass runs in the Gram form (default rule) and its guard band
+    carries the form's rounding term.  Forced tensor cores at n = nbar = 3000 with 3000 permutations put a few of them
+    inside the 15-bit band; after the escalation the count is the oracle's unless something stays inside the fp32 band."""
+    c = dg.config(2, scale=0.01)
+    s = dg.make_sample(c)
+    nperm = 3000
+    exp = oracle.perm_test(s.x, s.xbar, c.sigma, nperm, 77)
+    with force_kernel(ctx, 2):
+        ctx.set_option(binding.ET_OPT_EXACT_P, 64)
+        try:
+            got = ctx.permutation_test(s.x, s.xbar, c.sigma, nperm, 77)
+            st = ctx.stats()
+        finally:
+            ctx.set_option(binding.ET_OPT_EXACT_P, 16)
+    assert st.dominant_kernel == "k_perm_tc" and st.distance_form == 2
+    assert st.n_near_before > 0 and st.n_escalated == st.n_near_before
+    assert abs(got.count_gt - exp.count_gt) <= got.n_near
+    if got.n_near == 0:
+        assert got.count_gt == exp.count_gt and got.p_value == exp.p_value
+    # the re-evaluated differences are the oracle's to the accuracy of the escalation's arithmetic
+    d_got, d_exp = got.T_perm - got.observed.T, exp.T_perm - exp.observed.T
+    near = np.argsort(np.abs(d_exp))[: int(st.n_escalated)]
+    assert np.abs(d_got[near] - d_exp[near]).max() <= 5e-9   # 4 sigma of the band's model at n = 3000 (1.3e-9)
 
 
 # ----------------------------------------------------------------------------- the error model behind the guard band
