@@ -1517,11 +1517,30 @@ et_status et_bkg_permutation_test(et_ctx *ctx, const void *x, int64_t n, const v
     BP.seedb_lo = (uint32_t)(seed_b & 0xffffffffu); BP.seedb_hi = (uint32_t)(seed_b >> 32);
     DevBkg *scratch = reinterpret_cast<DevBkg *>(static_cast<char *>(ctx->result.p) + sizeof(DevPerm) + sizeof(DevT) * 4);
     const long long Nall = n + nbar + bs + bsbar;
+    // per permutation: class of every source event, stable four-way partition (multi-block: k_part_*), gather, one pass
+    const int nblk = (int)((Nall + kPartBlock - 1) / kPartBlock);
+    ET_TRY(ensure(ctx, ctx->esccls, (size_t)Nall));
+    ET_TRY(ensure(ctx, ctx->blkcnt, (size_t)nblk * 4 * sizeof(int)));
+    ET_TRY(ensure(ctx, ctx->totals, 16 * sizeof(long long)));
+    CUDA_TRY(cudaMemcpyAsync(static_cast<long long *>(ctx->totals.p) + 8, L.seg_pos, 4 * sizeof(long long), cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    LabelOut lo{};
+    lo.nseg = L.ncls;
+    for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
+    for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
     for (int64_t p = 0; p < nperm; ++p) {
-        k_bkg_perm_map<<<1, 1024, 0, ctx->stream>>>(BP, ctx->opt_perm_offset + p, sel_m + p, sel_b + p, static_cast<int *>(ctx->src.p));
+        k_bkg_class<<<(unsigned)((Nall + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(BP, ctx->opt_perm_offset + p, sel_m + p, sel_b + p,
+                                                                                              static_cast<uint8_t *>(ctx->esccls.p));
         LAUNCH_CHECK();
-        k_gather_rec<<<ctx->num_sms * 2, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->recP.p), static_cast<const int *>(ctx->src.p),
-                                                               L.npad, F / 4, static_cast<float4 *>(ctx->rec.p));
+        k_part_count<<<nblk, kPartBlock, 0, ctx->stream>>>(Nall, static_cast<const uint8_t *>(ctx->esccls.p), static_cast<int *>(ctx->blkcnt.p));
+        LAUNCH_CHECK();
+        k_part_scan<<<1, 32, 0, ctx->stream>>>(nblk, static_cast<int *>(ctx->blkcnt.p), static_cast<long long *>(ctx->totals.p));
+        LAUNCH_CHECK();
+        k_part_scatter<<<nblk, kPartBlock, 0, ctx->stream>>>(Nall, static_cast<const uint8_t *>(ctx->esccls.p), static_cast<const int *>(ctx->blkcnt.p),
+                                                            static_cast<const long long *>(ctx->totals.p) + 8, static_cast<int *>(ctx->src.p));
+        LAUNCH_CHECK();
+        k_esc_gather<<<ctx->num_sms * 4, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->recP.p), static_cast<const int *>(ctx->src.p), L.npad,
+                                                               F / 4, lo, static_cast<float4 *>(ctx->rec.p));
         LAUNCH_CHECK();
         ET_TRY(run_pairs_T(ctx, L, dim));
         k_stat_eq3<<<1, 32, 0, ctx->stream>>>(static_cast<const double *>(ctx->sums.p), (double)n, (double)nbar, (double)bs, (double)bsbar, bp, bbp,

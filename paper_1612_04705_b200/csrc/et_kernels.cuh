@@ -918,68 +918,29 @@ struct BkgPermParams {
     long long pos0[4];   // first record row of the identity layout's class segments (X, Bx, Xbar, Bxbar)
     uint32_t seedm_lo, seedm_hi, seedb_lo, seedb_hi;
 };
-// rowmap[row] = row of the identity-layout records that permutation pg (global index; `sm`, `sb` its select states for
-// the main and the background pool) puts into layout row `row`: classes (X', Bx', Xbar', Bxbar'), each in source order
-// (stable), padding rows untouched (-1 from the caller's fill).  One CTA of 1024 threads, chunked block scan: the
-// statistic is for background-subtraction studies of modest size (PAPER.md:105 uses 7 200 events).
-__global__ void __launch_bounds__(1024) k_bkg_perm_map(BkgPermParams P, long long pg, const SelState *__restrict__ sm,
-                                                      const SelState *__restrict__ sb, int *__restrict__ rowmap)
+// cls[s] = class (X', Bx', Xbar', Bxbar') = (0, 1, 2, 3) that permutation pg (global index; `sm`, `sb` its select states
+// for the main and the background pool) gives source event s, s running over X | Bx | Xbar | Bxbar in input order (the
+// class segments of the identity layout).  The stable four-way partition k_part_* then lists, class by class and in
+// source order, which source event every row of the permuted layout holds; the class sizes are those of the identity
+// layout (the labels preserve sample sizes), so the layout never changes.
+__global__ void __launch_bounds__(kThreads) k_bkg_class(BkgPermParams P, long long pg, const SelState *__restrict__ sm,
+                                                       const SelState *__restrict__ sb, uint8_t *__restrict__ cls)
 {
-    __shared__ int warp_cnt[32][4];
-    __shared__ long long run[4];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid < 4) run[tid] = 0;
-    __syncthreads();
     const long long Nx = P.n + P.bs, Ntot = Nx + P.nbar + P.bsbar;
-    const unsigned long long pre_m = sm->prefix, pre_b = sb->prefix;
-    for (long long base = 0; base < Ntot; base += 1024) {
-        const long long s = base + tid;
-        int c = -1;
-        long long row0 = 0;
-        if (s < Ntot) {
-            bool bkg;
-            long long idx;  // index in its pool
-            if (s < Nx) { bkg = s >= P.n; idx = bkg ? s - P.n : s; row0 = bkg ? P.pos0[1] + idx : P.pos0[0] + idx; }
-            else {
-                const long long t = s - Nx;
-                bkg = t >= P.nbar;
-                idx = bkg ? P.bs + (t - P.nbar) : P.n + t;
-                row0 = bkg ? P.pos0[3] + (t - P.nbar) : P.pos0[2] + t;
-            }
-            uint64_t K[4];
-            label_keys4((uint32_t)idx, (uint32_t)(pg >> 2), bkg ? P.seedb_lo : P.seedm_lo, bkg ? P.seedb_hi : P.seedm_hi, K);
-            const bool in_x = K[pg & 3] <= (bkg ? pre_b : pre_m);
-            c = (in_x ? 0 : 2) + (bkg ? 1 : 0);
-        }
-        unsigned bal[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) bal[k] = __ballot_sync(0xffffffffu, c == k);
-        if (lane == 0)
-#pragma unroll
-            for (int k = 0; k < 4; ++k) warp_cnt[warp][k] = __popc(bal[k]);
-        __syncthreads();
-        if (c >= 0) {
-            long long r = run[c] + __popc(bal[c] & ((1u << lane) - 1u));
-            for (int w = 0; w < warp; ++w) r += warp_cnt[w][c];
-            rowmap[P.pos0[c] + r] = (int)row0;   // class segments of the permuted layout start where the identity ones do
-        }
-        __syncthreads();
-        if (tid < 4) {
-            long long t = 0;
-            for (int w = 0; w < 32; ++w) t += warp_cnt[w][tid];
-            run[tid] += t;
-        }
-        __syncthreads();
+    const long long s = blockIdx.x * (long long)kThreads + threadIdx.x;
+    if (s >= Ntot) return;
+    bool bkg;
+    long long idx;  // index in its pool
+    if (s < Nx) { bkg = s >= P.n; idx = bkg ? s - P.n : s; }
+    else {
+        const long long t = s - Nx;
+        bkg = t >= P.nbar;
+        idx = bkg ? P.bs + (t - P.nbar) : P.n + t;
     }
-}
-// rec[row] = rec0[rowmap[row]] (zero record on padding rows), F floats per row
-__global__ void k_gather_rec(const float4 *__restrict__ rec0, const int *__restrict__ rowmap, long long npad, int F4, float4 *__restrict__ rec)
-{
-    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < npad * F4; k += (long long)gridDim.x * blockDim.x) {
-        const long long row = k / F4;
-        const int q = (int)(k % F4), src = rowmap[row];
-        rec[k] = src >= 0 ? rec0[(long long)src * F4 + q] : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+    uint64_t K[4];
+    label_keys4((uint32_t)idx, (uint32_t)(pg >> 2), bkg ? P.seedb_lo : P.seedm_lo, bkg ? P.seedb_hi : P.seedm_hi, K);
+    const bool in_x = K[pg & 3] <= (bkg ? sb->prefix : sm->prefix);
+    cls[s] = (uint8_t)((in_x ? 0 : 2) + (bkg ? 1 : 0));
 }
 // ---- guard-band escalation (exact p-value) ------------------------------------------------
 // Class of pooled (label) index i for the re-evaluation of permutation p: 2 (1 - a_obs) + (1 - a_perm), i.e.
