@@ -966,15 +966,15 @@ __global__ void __launch_bounds__(256) k_esc_apply(const DevNear *__restrict__ n
     }
 }
 
-template <int D>
+template <int D, class G>
 et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted)
 {
     if (weighted) {
-        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_tc(D)));
-        tc::k_perm_tc<D, true><<<grid, tc::kThreadsTC, tc::smem_tc(D), ctx->stream>>>(P);
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
+        tc::k_perm_tc<D, true, G><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
     } else {
-        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::smem_tc(D)));
-        tc::k_perm_tc<D, false><<<grid, tc::kThreadsTC, tc::smem_tc(D), ctx->stream>>>(P);
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
+        tc::k_perm_tc<D, false, G><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
     }
     LAUNCH_CHECK();
     return ET_OK;
@@ -1051,10 +1051,11 @@ et_status run_escalation(et_ctx *ctx, const Layout &L, int dim, int nperm, uint6
 }
 
 // Labels (TC layout), the contraction for every 512-column chunk, W_c, then the statistic.
-// lab2_classes: class segments that form sample X of the second labelling (column 1).
-et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted, unsigned lab2_classes,
-                      long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second,
-                      bool reuse_labels = false)
+// lab2_classes: class segments that form sample X of the second labelling (column 1).  G: geometry of k_perm_tc (et_tc.cuh).
+template <class G>
+et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted, unsigned lab2_classes,
+                        long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second,
+                        bool reuse_labels)
 {
     const int nchunks = (nperm + tc::kPermsPerChunk - 1) / tc::kPermsPerChunk;
     const int words_total = nchunks * tc::kWordsPerChunk;
@@ -1062,7 +1063,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // previous sigma of et_permutation_test_sigmas)
     ET_TRY(span_begin(ctx, 4));
     // the j range of the contraction is padded to whole K blocks: rows npad .. npadK - 1 carry zero labels and zero records
-    const long long npadK = (L.npad + tc::kKB - 1) / tc::kKB * tc::kKB;
+    const long long npadK = (L.npad + G::kKB - 1) / G::kKB * G::kKB;
     LabelOut lo{};
     lo.nseg = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
@@ -1085,15 +1086,15 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     // fell from 640 GB to the order of the matrix itself, profiles/r01d), then the shorter ones, longest first.
     // unit u -> cluster u % nclusters
     const int nclusters_max = ctx->num_sms / 2;
-    const int nT = (int)(L.npad / tc::kTM2), NK = (int)(npadK / tc::kKB);
-    auto first_kb = [](int I) { return (long long)I * tc::kTM2 / tc::kKB; };  // K block that holds the tile's first row
+    const int nT = (int)(L.npad / tc::kTM2), NK = (int)(npadK / G::kKB);
+    auto first_kb = [](int I) { return (long long)I * tc::kTM2 / G::kKB; };  // K block that holds the tile's first row
     long long total_kb = 0;
     for (int I = 0; I < nT; ++I) total_kb += NK - first_kb(I);
     // about 24 units per cluster and rank (ranks of a unit-range shard take every world-th unit of the same table)
     const long long nshare = (long long)nclusters_max * 24 * ctx->shard_world;
     long long Lmax = (total_kb + nshare - 1) / nshare;
     if (Lmax < 8) Lmax = 8;
-    if (Lmax > tc::kMaxUnitKB) Lmax = tc::kMaxUnitKB;
+    if (Lmax > G::kMaxUnitKB) Lmax = G::kMaxUnitKB;
     std::vector<tc::Unit> full, tail;
     for (long long m = 0; m * Lmax < NK; ++m)
         for (int I = 0; I < nT && first_kb(I) < (m + 1) * Lmax; ++I) {
@@ -1124,7 +1125,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     else { hi_signed = true; sc = tc::kScaleSigned / std::max(std::fabs(ctx->wmin), std::fabs(ctx->wmax)); }
 
     const int grid = 2 * std::min(nclusters_max, nunits);  // CTA pairs
-    const size_t part_bytes = (size_t)grid * tc::kProducerWarps * tc::kEpiGroups * 32 * 2 * 8;
+    const size_t part_bytes = (size_t)grid * G::kProducerWarps * G::kEpiGroups * 32 * 2 * 8;
     ET_TRY(ensure(ctx, ctx->tcpart, part_bytes));
     ET_TRY(ensure(ctx, ctx->tcQ, (size_t)nchunks * tc::kCols * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->tcR, (size_t)nchunks * tc::kCols * sizeof(double)));
@@ -1156,11 +1157,11 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         cols_algo += ch == 0 ? cols_used : cols_used - tc::kSpecial;  // the special columns are algorithmic work once
         cols_exec += 256 * P.nq;
         P.partial = ctx->tcpart.p;
-        DISPATCH_DIM(dim, ET_TRY(launch_perm_tc<D>(ctx, P, grid, weighted)));
+        DISPATCH_DIM(dim, ET_TRY((launch_perm_tc<D, G>(ctx, P, grid, weighted))));
         // the scale actually applied is the fp32 value of 256 sc
         const double inv_sc = 256.0 / (double)P.sc256;
-        if (weighted) tc::k_tc_reduce<true><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
-        else tc::k_tc_reduce<false><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
+        if (weighted) tc::k_tc_reduce<true, G><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
+        else tc::k_tc_reduce<false, G><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
         LAUNCH_CHECK();
         ET_TRY(shard_sum(ctx, ctx->tcraw.p, 2 * tc::kCols, weighted));  // exact int64 (or fp64) column sums over the ranks
         if (weighted)
@@ -1178,7 +1179,7 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
         // special columns repeated in every chunk) is kept beside it
         ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * cols_algo));
         ctx->stats.dominant_ops_executed = 2ll * 2 * pairs * cols_exec;
-        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM2 * tc::kKB;
+        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM2 * G::kKB;
     }
 
     // W_c
@@ -1226,6 +1227,16 @@ et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t
     *out = r.r;
     if (second) *second = sec.r;
     return ET_OK;
+}
+
+// Geometry by dimension (et_tc.cuh): the 16-producer-warp / 128-j layout while the i rows fit its 96 registers.
+et_status run_perm_tc(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64_t seed, bool weighted, unsigned lab2_classes,
+                      long long npairs_obs, long long npairs_second, double *T_perm, et_perm_result *out, et_result *second,
+                      bool reuse_labels = false)
+{
+    if (dim <= 5)
+        return run_perm_tc_g<tc::Geo128>(ctx, L, dim, nperm, seed, weighted, lab2_classes, npairs_obs, npairs_second, T_perm, out, second, reuse_labels);
+    return run_perm_tc_g<tc::Geo96>(ctx, L, dim, nperm, seed, weighted, lab2_classes, npairs_obs, npairs_second, T_perm, out, second, reuse_labels);
 }
 
 bool use_tc(const et_ctx *ctx, const Layout &L)

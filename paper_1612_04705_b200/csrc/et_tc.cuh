@@ -33,28 +33,48 @@ namespace tc {
 
 constexpr int kTM = 128;                 // rows (i) per CTA = UMMA M / 2
 constexpr int kTM2 = 2 * kTM;            // rows per cluster (work unit)
-constexpr int kKB = 96;                  // j per K block: three UMMA K steps of 32
 constexpr int kCols = 512;               // label columns per launch (2 accumulators of N = 256)
 constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
-constexpr int kProducerWarps = 12;       // three per scheduler; a thread evaluates 4 rows x 8 j of the psi tile
-constexpr int kRowsPerThread = kTM * kKB / 8 / (kProducerWarps * 32);  // 4
-constexpr int kEpiWarps = kProducerWarps / 4;                         // warps per TMEM lane quarter
-constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;          // most 32-column groups a warp reads in the epilogue
-__host__ __device__ constexpr int epi_first(int e) { return 16 * e / kEpiWarps; }  // groups [epi_first(e), epi_first(e + 1)) of warp row e
-constexpr int kProducers = kProducerWarps * 32;
-constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
-constexpr int kStages = 3;
-constexpr int kABytes = 2 * kTM * kKB;       // hi and lo digit tiles (24 KB)
-constexpr int kBPlane = kKB * 128;           // one plane of this CTA's half of B: kKB j x 128 columns
-constexpr int kBBytes = 2 * 2 * kBPlane;     // [q 2][digit 2][plane]
-constexpr int kStageBytes = kABytes + kBBytes;
-// ring of j pair-record blocks (kKB / 2 pairs each), filled by bulk copies (see the loader)
-__host__ __device__ constexpr int rec_slots(int dim) { return (dim + 2) / 2 <= 3 ? 4 : 2; }
-__host__ __device__ constexpr int rec_slot_bytes(int dim) { return (kKB / 2) * ((dim + 2) / 2) * 16; }
-__host__ __device__ constexpr int smem_tc(int dim) { return kStages * kStageBytes + rec_slots(dim) * rec_slot_bytes(dim) + 1024 /*alignment slack*/; }
 constexpr int kMaxRecSlots = 4;
+// float4 per pair record: dim + 1 float2 entries, padded to an even count
+__host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
+
+// Geometry of the kernel: K blocks of KB j (KB / 32 UMMA K steps), PW producer warps (a thread evaluates 4 rows x 8 j of
+// the 128 x KB psi tile of its CTA: PW = KB / 8), ST shared-memory stages.  Two are built:
+//   Geo<96, 12, 3>:  14 warps x 128 registers, three 72 KB stages.  No register spills for any dim.
+//   Geo<128, 16, 2>: 18 warps x 96 registers, two 96 KB stages: a fourth producer warp per scheduler hides more of the
+//                    producers' latency (profiles/r02_README.md: -4.6 % at config 4, same at dim = 2), but the i rows of
+//                    dim >= 6 no longer fit the registers (dim = 8: +75 %).  run_perm_tc takes it for dim <= 5.
+template <int KB, int PW, int ST>
+struct Geo {
+    static constexpr int kKB = KB;                  // j per K block
+    static constexpr int kProducerWarps = PW;
+    static constexpr int kStages = ST;
+    static constexpr int kRowsPerThread = kTM * KB / 8 / (PW * 32);  // 4
+    static constexpr int kEpiWarps = PW / 4;                         // warps per TMEM lane quarter
+    static constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;  // most 32-column groups a warp reads in the epilogue
+    __host__ __device__ static constexpr int epi_first(int e) { return 16 * e / kEpiWarps; }  // groups [epi_first(e), epi_first(e + 1)) of warp row e
+    static constexpr int kProducers = PW * 32;
+    static constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
+    static constexpr int kABytes = 2 * kTM * KB;        // hi and lo digit tiles
+    static constexpr int kBPlane = KB * 128;            // one plane of this CTA's half of B: KB j x 128 columns
+    static constexpr int kBBytes = 2 * 2 * kBPlane;     // [q 2][digit 2][plane]
+    static constexpr int kStageBytes = kABytes + kBBytes;
+    // ring of j pair-record blocks (KB / 2 pairs each), filled by bulk copies (see the loader)
+    __host__ __device__ static constexpr int rec_slots(int dim) { return pair_rec_f4(dim) <= 3 ? 4 : 2; }
+    __host__ __device__ static constexpr int rec_slot_bytes(int dim) { return (KB / 2) * pair_rec_f4(dim) * 16; }
+    __host__ __device__ static constexpr int smem_tc(int dim) { return ST * kStageBytes + rec_slots(dim) * rec_slot_bytes(dim) + 1024 /*alignment slack*/; }
+    // K blocks per unit: |Y| <= 32767 * KB * kMaxUnitKB < 2^31 (660 for KB = 96: 2 076 117 120; 511 for KB = 128).  Longer
+    // units mean fewer epilogues and pipeline drains (512 -> 1000 blocks of 64 j measured -1.2 % at config 2 and -0.9 % at
+    // config 4, identical integer sums).
+    static constexpr int kMaxUnitKB = 2147483647ll / (32767ll * KB) > 660 ? 660 : (int)(2147483647ll / (32767ll * KB));
+    static_assert(32767ll * KB * kMaxUnitKB < 2147483648ll, "int32 accumulator headroom");
+    static_assert(PW * 8 == KB && PW % 4 == 0, "one producer warp per 8 j, whole warp rows in the epilogue");
+};
+using Geo96 = Geo<96, 12, 3>;
+using Geo128 = Geo<128, 16, 2>;
 // Quantisation of Psi_ij = w_j psi_ij to the 15-bit grid of step 1 / sc: f = fma.rz(psi, 256 sc w_j, M + 128) with
 // M = 2^23 holds, in mantissa bits 8..22, v = floor(sc Psi + 1/2), 0 <= v <= 32767 (weights >= 0).  With signed weights
 // M = 1.5 * 2^23 and the same bits hold 16384 + v, |v| <= 16383.  The two operand digits are BYTES 1 and 2 of f:
@@ -79,15 +99,9 @@ constexpr int kMaxRecSlots = 4;
 constexpr float kMagicUnsigned = 8388608.0f, kMagicSigned = 12582912.0f;
 constexpr double kQuantVar = 1.0 / 12.0;
 constexpr double kScaleUnsigned = 32766.0, kScaleSigned = 16382.0;  // floor(sc Psi + 1/2) <= 32767 with the fp32 slack of sc w_j
-// K blocks per unit: |Y| <= 32767 * 96 * 660 = 2 076 117 120 < 2^31.  Longer units mean fewer epilogues and pipeline
-// drains (512 -> 1000 blocks of 64 j measured -1.2 % at config 2 and -0.9 % at config 4, identical integer sums).
-constexpr int kMaxUnitKB = 660;
 
 // label bit held by byte / TMEM column p of a 32-column word
 __host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
-
-// float4 per pair record: dim + 1 float2 entries, padded to an even count
-__host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
 
 struct Unit {
     int I;         // 256-row tile
@@ -344,24 +358,27 @@ struct TCParams {
     uint32_t hixor;          // 0, or 0x80808080 with kMagicSigned: hi digit = 2 byte2 - 128
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
     int nq;                  // 256-column accumulators in use: 2, or 1 when this launch has <= 256 label columns
-    void *partial;           // [gridDim.x][kProducerWarps][kEpiGroups][32 lanes][2] of Acc
+    void *partial;           // [gridDim.x][GEO::kProducerWarps][GEO::kEpiGroups][32 lanes][2] of Acc
 };
 
 // One launch = 512 label columns.  Grid: persistent, one CTA per SM, clusters of 2 (an SM pair); unit u is processed
 // by cluster u % (gridDim.x / 2).  CTA rank r of the pair owns rows 256 I + 128 r .. + 127 (its psi tile, its half of
 // the accumulator rows in its own TMEM) and the label columns [256 q + 128 r, 256 q + 128 r + 128), q = 0, 1.
 // WEIGHTED: accumulate w_i Y in double; else exact int64.
-template <int D, bool WEIGHTED>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_perm_tc(TCParams P)
+template <int D, bool WEIGHTED, class GEO>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) k_perm_tc(TCParams P)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
+    constexpr int kKB = GEO::kKB, kProducerWarps = GEO::kProducerWarps, kStages = GEO::kStages, kRowsPerThread = GEO::kRowsPerThread;
+    constexpr int kEpiGroups = GEO::kEpiGroups, kProducers = GEO::kProducers;
+    constexpr int kABytes = GEO::kABytes, kBPlane = GEO::kBPlane, kStageBytes = GEO::kStageBytes;
     constexpr int F = rec_floats(D);
     constexpr int NLD = pair_rec_f4(D);     // 16-byte loads per j pair: float2 (-u_j0k, -u_j1k) k < D, then (s_j0, s_j1)
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 1024-byte alignment of the operand tiles (SWIZZLE_128B atoms), keeping the pointer in the shared state space
     uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // one array, so that the hot loop addresses every barrier as bar0 + constant + 8 * index
-    constexpr int kRecSlots = rec_slots(D);
+    constexpr int kRecSlots = GEO::rec_slots(D);
     __shared__ __align__(8) uint64_t bars_s[2 * kStages + 2 + 2 * kMaxRecSlots];
     uint64_t *const bar_full = bars_s, *const bar_empty = bars_s + kStages, *const bar_rec = bars_s + 2 * kStages + 2;
     uint64_t *const bar_recfree = bar_rec + kMaxRecSlots;  // record slot consumed by all producer warps of this CTA
@@ -453,7 +470,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
         constexpr int OW = kKB / 16;                 // warps along j (two octets each)
         const int oct = 2 * (warp % OW) + og;
         const int mrow0 = 16 * R * (warp / OW) + 8 * (lane >> 4) + l8;
-        const int grp0 = epi_first(warp >> 2), ngrp = epi_first((warp >> 2) + 1) - grp0;  // this warp's column groups in the epilogue
+        const int grp0 = GEO::epi_first(warp >> 2), ngrp = GEO::epi_first((warp >> 2) + 1) - grp0;  // this warp's column groups in the epilogue
         const int lane_base = 32 * (warp & 3);       // TMEM lanes this warp may access
         Acc accQ[G], accR[G];
 #pragma unroll
@@ -664,17 +681,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreadsTC, 1) k_per
 // Column sums over CTAs and warps, fixed order: TMEM column 32 gc + lane (gc = c >> 5) is held by the four warps
 // 4 (gc / G) .. + 3 as their group gc % G, and is label column c = 32 gc + beta(lane).  raw[col] = Q, raw[512 + col] = R
 // as exact integers (or doubles when weighted) in units of the quantisation step: what a unit-range shard exchanges.
-template <bool WEIGHTED>
+template <bool WEIGHTED, class GEO>
 __global__ void k_tc_reduce(const void *partial, int ncta, void *raw)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
+    constexpr int kEpiWarps = GEO::kEpiWarps, kEpiGroups = GEO::kEpiGroups, kProducerWarps = GEO::kProducerWarps;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= kCols) return;
     constexpr int G = kEpiGroups;
     const int gc = c >> 5, lane = c & 31;
     int e = 0;  // warp row that reads column group gc in the epilogue
-    while (e + 1 < kEpiWarps && epi_first(e + 1) <= gc) ++e;
-    const int g = gc - epi_first(e);
+    while (e + 1 < kEpiWarps && GEO::epi_first(e + 1) <= gc) ++e;
+    const int g = gc - GEO::epi_first(e);
     const Acc *p = reinterpret_cast<const Acc *>(partial);
     Acc sq = 0, sr = 0;
     for (int b = 0; b < ncta; ++b)

@@ -680,14 +680,16 @@ def test_full_size_config3_weighted_tc_properties(ctx):
     assert 1e-8 < Tp.std() < 1e-4
 
 
-def test_perm_tc_accumulator_headroom_coincident_points(ctx):
+@pytest.mark.parametrize("dim", [2, 6])
+def test_perm_tc_accumulator_headroom_coincident_points(ctx, dim):
     """The largest values the int32 TMEM accumulators can see: 260 000 coincident events, psi = 1 for every pair, so
-    every work unit of the first row tiles runs the full 660 K blocks of 96 j with all digits at their maximum:
-    |Y| = 32767 x 96 x 660 = 2 076 117 120 of 2^31 = 2 147 483 648 (run_perm_tc picks Lmax = 660 from N = 2.4e5 on, which
-    is every config-2/3/4 launch).  300 permutations: both 256-column accumulators.  Pin P1 at scale: T = 1/2 + 1/2 - 1
-    = 0 for the observed and for every permutation; the raw sums are the pair counts."""
+    every work unit of the first row tiles runs the longest unit its geometry allows with all digits at their maximum --
+    dim = 2 (Geo<128, 16, 2>, et_tc.cuh): |Y| = 32767 x 128 x 512 = 2 147 418 112, dim = 6 (Geo<96, 12, 3>): 32767 x 96 x
+    660 = 2 076 117 120, of 2^31 = 2 147 483 648 (run_perm_tc caps the units there from N = 2.4e5 on, which is every
+    config-2/3/4 launch).  300 permutations: both 256-column accumulators.  Pin P1 at scale: T = 1/2 + 1/2 - 1 = 0 for the
+    observed and for every permutation; the raw sums are the pair counts."""
     n = nbar = 130000
-    x, xb = np.full((n, 2), 0.25), np.full((nbar, 2), 0.25)
+    x, xb = np.full((n, dim), 0.25), np.full((nbar, dim), 0.25)
     got = ctx.permutation_test(x, xb, 0.3, 300, 3)
     assert ctx.stats().dominant_kernel == "k_perm_tc"
     o = got.observed
