@@ -113,9 +113,9 @@ typedef struct {
 typedef enum {
     ET_OPT_PERM_KERNEL = 0, /* permutation sums: 0 (default) = tensor-core contraction (tcgen05
                                kind::i8, psi quantised to 15 bits, exact integer sums) when the
-                               padded pooled size is >= 16384 rows, else the fp32 CUDA-core
+                               padded pooled size is >= 8192 rows, else the fp32 CUDA-core
                                kernel; 1 = always CUDA cores; 2 = always tensor cores (below
-                               16384 rows the 15-bit rounding noise can exceed the 1e-6 tolerance
+                               8192 rows the 15-bit rounding noise can exceed the 1e-6 tolerance
                                of T: a test hook)                       */
     ET_OPT_PERM_OFFSET = 1, /* first permutation index p0 (default 0): the calls evaluate
                                permutations p0 .. p0+nperm-1 of the seed's stream, T_perm[k] is
@@ -133,7 +133,8 @@ typedef enum {
                                |u_j|^2 - 2 u_i.u_j (dim + 2 operations; psi then carries a relative
                                rounding error of about 8e-8 |u|^2_max, |u|^2_max the squared half
                                diagonal of the bounding box over 2 sigma^2 / log2 e); 0 (default) =
-                               Gram form when dim >= 4, n + nbar >= 4096 and |u|^2_max <= 48, else differences
+                               Gram form when dim >= 4, n + nbar >= 4096 and |u|^2_max <= 48, else differences;
+                               2 falls back to differences when |u|^2_max > 96 (et_stats.distance_form tells)
                                (DESIGN.md section 6).  T stays within the 1e-6 tolerance either way    */
 } et_option;
 

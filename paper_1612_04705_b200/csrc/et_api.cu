@@ -334,7 +334,7 @@ constexpr double kGramMaxU2 = 48.0;
 bool use_gram(const et_ctx *ctx, const Layout &L, int dim)
 {
     if (ctx->opt_distance == 1) return false;
-    if (ctx->opt_distance == 2) return true;
+    if (ctx->opt_distance == 2) return ctx->umax2 <= 96.0;  // beyond, 2^(|u_i|^2) times a 128-term sum leaves the fp32 range
     return dim >= 4 && L.N >= kGramMinN && ctx->umax2 <= kGramMaxU2;
 }
 
@@ -1243,7 +1243,10 @@ bool use_tc(const et_ctx *ctx, const Layout &L)
 {
     if (ctx->opt_perm_kernel == 1) return false;
     if (ctx->opt_perm_kernel == 2) return true;
-    return L.npad >= 16384;
+    // >= 8192 padded rows: the 15-bit rounding noise of T (0.82 / 32766 / N) is then 8 sigma < 4e-8, inside the 1e-6
+    // tolerance for every term scale >= 0.04, and the contraction beats the CUDA-core kernel (one pass per 32 columns) by
+    // 5 - 10 x at 1000 permutations (measured at N = 2000 .. 16 000, profiles/r02_README.md)
+    return L.npad >= 8192;
 }
 
 }  // namespace

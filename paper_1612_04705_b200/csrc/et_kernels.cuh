@@ -168,9 +168,11 @@ __device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int 
 // skip_mask: bit c1 * 4 + c2 (c1 <= c2) set = tile pairs of that class pair are not evaluated (their slot stays 0);
 // the guard-band escalation needs six of the ten class-pair sums only.  Units unit0 + k * unit_step (k = 0, 1, ...) are
 // this launch's share: (0, 1) on one GPU, (rank, world) when the unit range is sharded over ranks.
-// GRAM: e_ij = |u_i|^2 + |u_j|^2 + sum_k u_ik (-2 u_jk) -- one FADD2 and D FFMA2 per two pairs instead of D FADD2, one
-// FMUL2 and D - 1 FFMA2, i.e. D + 2 instead of 2 D + 1 FP32-pipe lane-ops per pair (D = 5: 7 instead of 11; the kernel is
-// then bound by the 16 MUFU.EX2 per clock and SM).  Every operation rounds a value of size <= 2 (|u_i|^2 + |u_j|^2)
+// GRAM: e_ij = |u_i|^2 + |u_j|^2 + sum_k u_ik (-2 u_jk), and the row's constant is taken out of the exponent:
+// psi_ij = 2^(-|u_i|^2) 2^(-e'_ij), e'_ij = |u_j|^2 + sum_k u_ik (-2 u_jk) -- D FFMA2 per two pairs instead of D FADD2, one
+// FMUL2 and D - 1 FFMA2, i.e. D + 1 instead of 2 D + 1 FP32-pipe lane-ops per pair with the accumulation (D = 5: 6 instead
+// of 11; the kernel is then bound by the 16 MUFU.EX2 per clock and SM); the factor 2^(-|u_i|^2) multiplies the row's fp32
+// partial sum once per 256 j, in double.  2^(-e') <= 2^(|u_i|^2) <= 2^umax2: the host keeps umax2 <= 96 for this form.  Every operation rounds a value of size <= 2 (|u_i|^2 + |u_j|^2)
 // instead of the small difference, so psi carries a relative error of about kGramErr umax2 (umax2 = the largest |u|^2: the
 // squared half diagonal of the bounding box in units of sigma sqrt(2 / log2 e)) -- zero-mean rounding noise that averages
 // over the pairs, plus a per-event part from the rounding of |u_i|^2 that acts like a weight 1 + O(1e-7 umax2) on event i.
@@ -198,8 +200,8 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
         const int slot = tile_cls[(long long)I * TI / kPad] * 4 + tile_cls[(long long)J * TI / kPad];
         if (skip_mask >> slot & 1u) continue;
         float2 ui[R][D];
-        float2 ai[GRAM ? R : 1];
-        float wi[R], self[R];   // self: w_i psi_ii as this kernel evaluates it (1 exactly with the difference form)
+        double rs[R];           // GRAM: 2^(-|u_i|^2), the factor of the row taken out of the exponent; else 1
+        float wi[R], self[R];   // self: w_i psi_ii / rs as this kernel evaluates it (w_i exactly with the difference form)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 *p = reinterpret_cast<const float4 *>(rec + ((long long)I * TI + r * kThreads + tid) * F);
@@ -214,14 +216,15 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
             for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             wi[r] = v[D];
             self[r] = v[D];
+            rs[r] = 1.0;
             if (GRAM) {
                 float na = __fmul_rn(v[0], v[0]);
 #pragma unroll
                 for (int k = 1; k < D; ++k) na = __fmaf_rn(v[k], v[k], na);
-                ai[r] = __fadd2_rn(make_float2(na, na), make_float2(0.f, 0.f));
-                // psi_ii by the instruction sequence of the loop below (each half of a packed instruction rounds like
-                // the scalar one): what the diagonal tile adds for j = i, removed again after the loop
-                float e = __fadd_rn(na, na);
+                rs[r] = exp2(-(double)na);
+                // 2^(-e'_ii) by the instruction sequence of the loop below (each half of a packed instruction rounds
+                // like the scalar one): what the diagonal tile adds for j = i, removed again after the loop
+                float e = na;
 #pragma unroll
                 for (int k = 0; k < D; ++k) e = __fmaf_rn(v[k], -2.f * v[k], e);
                 self[r] = __fmul_rn(ex2_approx(-e), v[D]);
@@ -273,7 +276,7 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
                 for (int r = 0; r < R; ++r) {
                     float2 e;
                     if (GRAM) {
-                        e = __fadd2_rn(ai[r], nu[D]);
+                        e = nu[D];
 #pragma unroll
                         for (int k = 0; k < D; ++k) e = __ffma2_rn(ui[r][k], nu[k], e);
                     } else {
@@ -294,7 +297,7 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
         double t = 0.0;
         const bool diag = I == J;
 #pragma unroll
-        for (int r = 0; r < R; ++r) t += (double)wi[r] * (diag ? racc[r] - (double)self[r] : racc[r]);
+        for (int r = 0; r < R; ++r) t += (double)wi[r] * rs[r] * (diag ? racc[r] - (double)self[r] : racc[r]);
         if (diag) t *= 0.5;
         t = warp_sum(t);
         if ((tid & 31) == 0) s_warp[tid >> 5] = t;

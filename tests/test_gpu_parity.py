@@ -575,7 +575,7 @@ def test_T_sigmas_weighted_and_errors(ctx):
 def test_perm_tc_chunk_and_size_edges(ctx, n, nbar, nperm):
     """Tensor-core path forced at its edges: the smallest samples, one permutation, and permutation counts on both
     sides of the 509-per-launch boundary (1, 2 and 3 launches of 512 label columns).  Below the default dispatch
-    threshold (16384 rows) the 15-bit quantisation noise of psi does not average out: the bound used here is 8 sigma of
+    threshold (8192 rows) the 15-bit quantisation noise of psi does not average out: the bound used here is 8 sigma of
     DESIGN.md section 6, var(T) = (1/12) q^2 [1/(2n(n-1)) + 1/(2nbar(nbar-1)) + 1/(n nbar)] with q = 1 / 32766, or the
     north-star tolerance if that is larger."""
     rng = np.random.default_rng(n * 1000 + nperm)
@@ -835,6 +835,32 @@ def test_full_size_golden(ctx, index):
         assert abs(getattr(t, k) - getattr(exp, k)) <= TOL * scale, k
     print(f"\n[golden cfg{index}] spread {spread:.3e}; |dT| tensor-core path: " + ", ".join(f"{e:.2e}" for e in errs) +
           f"; et_T {abs(t.T - exp.T):.2e}; n_near {st.n_near_before} -> {got.n_near}, escalation {st.ms_escalation:.1f} ms")
+
+
+def test_full_size_config4_p_even_golden(ctx):
+    """BASELINE configs[4] at full size (n = nbar = 10^6, 5-D), the launch bench.py times: the P-even statistic (I+II) vs
+    (III+IV) = Eq. 2 of (X, Xbar) -- column 1 of K-PERM-TC -- and et_T (k_pairs_T, Gram form at this size)
+    against the oracle's stored value (tests/golden/fullsize_T.txt, cfg4.even.*: one 2.0e12-pair fp64 pass, 97 minutes on 7
+    host cores), at the north-star tolerance and at 5 % of the permutation spread."""
+    g = _golden()
+    if "cfg4.even.T" not in g:
+        pytest.skip("cfg4.even is not in tests/golden/fullsize_T.txt yet")
+    c = dg.config(4)
+    s = dg.make_sample(c)
+    N = c.n + c.nbar
+    ev = _golden_result(g, "cfg4.even", N * (N - 1) // 2)
+    r = ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, c.nperm, c.perm_seed)
+    assert ctx.stats().dominant_kernel == "k_perm_tc"
+    assert tuple(float(v) for v in r.count) == tuple(g[f"cfg4.count.{k}"] for k in ("I", "II", "III", "IV"))
+    spread = r.p_odd.T_perm.std()
+    assert_T_close(r.p_even, ev, term_rel=TERM_REL_TC)
+    assert abs(r.p_even.T - ev.T) <= 0.05 * spread, (r.p_even.T, ev.T, spread)
+    t = ctx.T(s.x, s.xbar, c.sigma)
+    assert ctx.stats().distance_form == 2
+    assert_T_close(t, ev)
+    assert abs(t.T - ev.T) <= 0.05 * spread
+    print(f"\n[golden cfg4.even] spread {spread:.3e}; |dT| tensor-core column 1 {abs(r.p_even.T - ev.T):.2e}, et_T {abs(t.T - ev.T):.2e} "
+          f"(= {abs(t.T - ev.T) / ev.term_scale:.1e} of the term scale)")
 
 
 # ----------------------------------------------------------------------------- exact p-values (guard-band escalation)
