@@ -121,8 +121,9 @@ def ncu_traffic(kernel: str, cfg_index: int, default_nperm: bool):
 
     per_launch = {}
     with open(path) as f:
-        for r in csv.DictReader(f):
-            if r["Metric Name"] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        lines = [ln for ln in f if not ln.startswith("==")]   # ncu's own log lines precede the CSV header
+        for r in csv.DictReader(lines):
+            if r.get("Metric Name") in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
                 per_launch[r["ID"]] = per_launch.get(r["ID"], 0.0) + float(r["Metric Value"].replace(",", ""))
     if not per_launch:
         return None, None
