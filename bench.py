@@ -302,6 +302,18 @@ def run_ours(args):
             sep = sum(ms_of(lambda v=v: ctx.T(d["x"], d["xbar"], v)) for v in sg)
         sigma_scan = {"sigmas": sg, "ms_fused": fused, "ms_separate": sep, "pair_sigma_evals_per_s": len(sg) * pairs1 / (fused * 1e-3)}
 
+    # binned S_CP chi^2 of the same samples (Eq. 1; NEXT-4): the paper's O(N) comparison method on a uniform
+    # grid over the bounding box, about 10 bins per axis in 2-D ("O(10) to O(10^2)" bins), 3 per axis in 5-D
+    try:
+        nb = [10] * cfg.dim if cfg.dim <= 2 else [3] * cfg.dim
+        lo = np.minimum(s.x.min(axis=0), s.xbar.min(axis=0)).astype(np.float64)
+        hi = np.maximum(s.x.max(axis=0), s.xbar.max(axis=0)).astype(np.float64)
+        ctx.scp(d["x"], d["xbar"], lo, hi, nb)
+        sc_ = ctx.scp(d["x"], d["xbar"], lo, hi, nb)
+        scp = {"chi2": sc_.chi2, "ndf": sc_.ndf, "p_value": sc_.p_value, "bins": sc_.bins_total, "ms": ctx.stats().ms_total}
+    except (binding.EtError, ValueError) as exc:
+        scp = {"error": str(exc)}
+
     # GEV fit of this step's permutation T values: the p-value where counting gives 0 (host-only, ~ms)
     try:
         g = binding.gev_pvalue(res.T_perm, res.observed.T, np.random.default_rng(12345).standard_normal((2000, 3)))
@@ -362,6 +374,7 @@ def run_ours(args):
         "escalation": {"n_near_before": agg.get("n_near_before", 0), "n_escalated": agg.get("n_escalated", 0),
                        "n_near_after": res.n_near, "escalation_ms": agg["ms_esc"] / args.steps},
         "gev": gev,
+        "scp": scp,
         "et_T": et_T,
         "sigma_scan": sigma_scan,
         "share_pairs_kernels": agg["ms_pairs"] / ms, "share_labels": agg["ms_labels"] / ms,
