@@ -10,6 +10,8 @@
 #include <algorithm>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>  // header-only NVTX v3: ranges for Nsight tools, a no-op when no tool is attached
+
 #include "../../include/et.h"
 #include "et_kernels.cuh"
 #include "et_tc.cuh"
@@ -72,6 +74,9 @@ struct et_ctx {
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     Buf scpcnt, scpS;
     bool tc_attr_set = false;
+    // NVTX ranges: the call and its spans (labels, O(N^2) kernels, escalation); ids of the open ones
+    nvtxRangeId_t nvtx_call = 0, nvtx_span[8] = {0};
+    bool nvtx_call_open = false, nvtx_span_open[8] = {false};
 };
 
 namespace {
@@ -200,8 +205,18 @@ et_status upload_tile_classes(et_ctx *ctx, const Layout &L, Buf *dst = nullptr)
 }
 
 // ---- call bracketing / stats -----------------------------------------------------------------------------
+void nvtx_close_all(et_ctx *ctx)
+{
+    for (int k = 0; k < 8; ++k)
+        if (ctx->nvtx_span_open[k]) { nvtxRangeEnd(ctx->nvtx_span[k]); ctx->nvtx_span_open[k] = false; }
+    if (ctx->nvtx_call_open) { nvtxRangeEnd(ctx->nvtx_call); ctx->nvtx_call_open = false; }
+}
+
 et_status begin_call(et_ctx *ctx)
 {
+    nvtx_close_all(ctx);  // a call that returned an error left its ranges open
+    ctx->nvtx_call = nvtxRangeStartA("libet call");
+    ctx->nvtx_call_open = true;
     ctx->stats = et_stats{};
     ctx->acc_pairs_ms = ctx->acc_labels_ms = 0;
     for (int k = 0; k < 4; ++k) { ctx->kc_ms[k] = 0; ctx->kc_launches[k] = 0; ctx->kc_ops[k] = 0; }
@@ -225,10 +240,18 @@ et_status end_call(et_ctx *ctx)
     ctx->stats.dominant_launches = ctx->kc_launches[dom];
     ctx->stats.dominant_ops = ctx->kc_ops[dom];
     snprintf(ctx->stats.dominant_kernel, sizeof(ctx->stats.dominant_kernel), "%s", ctx->kc_launches[dom] ? kKcName[dom] : "");
+    nvtx_close_all(ctx);
     return ET_OK;
 }
 // Bracket a group of launches with events; the elapsed time is read (after a sync) by span_end.
-et_status span_begin(et_ctx *ctx, int slot) { CUDA_TRY(cudaEventRecord(ctx->ev[slot], ctx->stream)); return ET_OK; }
+et_status span_begin(et_ctx *ctx, int slot)
+{
+    if (ctx->nvtx_span_open[slot]) nvtxRangeEnd(ctx->nvtx_span[slot]);
+    ctx->nvtx_span[slot] = nvtxRangeStartA(slot == 4 ? "libet labels" : slot == 6 ? "libet escalation" : "libet pair kernels");
+    ctx->nvtx_span_open[slot] = true;
+    CUDA_TRY(cudaEventRecord(ctx->ev[slot], ctx->stream));
+    return ET_OK;
+}
 et_status span_end(et_ctx *ctx, int slot, double *acc, int kc = -1, int64_t launches = 0, int64_t ops = 0)
 {
     CUDA_TRY(cudaEventRecord(ctx->ev[slot + 1], ctx->stream));
@@ -236,6 +259,7 @@ et_status span_end(et_ctx *ctx, int slot, double *acc, int kc = -1, int64_t laun
     float ms = 0;
     CUDA_TRY(cudaEventElapsedTime(&ms, ctx->ev[slot], ctx->ev[slot + 1]));
     *acc += ms;
+    if (ctx->nvtx_span_open[slot]) { nvtxRangeEnd(ctx->nvtx_span[slot]); ctx->nvtx_span_open[slot] = false; }
     if (kc >= 0) { ctx->kc_ms[kc] += ms; ctx->kc_launches[kc] += launches; ctx->kc_ops[kc] += ops; }
     return ET_OK;
 }
@@ -1289,13 +1313,15 @@ void et_destroy(et_ctx *ctx)
                    &ctx->Q, &ctx->partRW, &ctx->RW, &ctx->mm, &ctx->flag, &ctx->counter, &ctx->src, &ctx->posx, &ctx->posb,
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
-                   &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw};
+                   &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
+                   &ctx->scpcnt, &ctx->scpS};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     for (int i = 0; i < 8; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     if (ctx->own_stream && ctx->stream) cudaStreamDestroy(ctx->stream);
+    nvtx_close_all(ctx);
     delete ctx;
 }
 
