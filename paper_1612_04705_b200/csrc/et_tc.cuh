@@ -52,6 +52,7 @@ struct Geo {
     static constexpr int kKB = KB;                  // j per K block
     static constexpr int kProducerWarps = PW;
     static constexpr int kStages = ST;
+    static constexpr bool kHoistQ2 = PW == 12;      // see the producer loop of k_perm_tc
     static constexpr int kRowsPerThread = kTM * KB / 8 / (PW * 32);  // 4
     static constexpr int kEpiWarps = PW / 4;                         // warps per TMEM lane quarter
     static constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;  // most 32-column groups a warp reads in the epilogue
@@ -520,15 +521,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
             const int dthr = row0 + mrow0 - 8 * oct;
             // this thread's label words of K block kb, prefetched one block ahead into registers.  The element index is
             // 64 bits wide: npadK * words_total passes 2^32 at 2 M pooled rows with the maximum permutation count.
-            const bool q2 = P.nq > 1;
+            const bool q2rt = P.nq > 1;
             unsigned long long im = (unsigned long long)(U.kb_begin * kKB + jj) * (unsigned)P.words_total + (unsigned)(P.word0 + 4 * (int)rank + l3);
-            uint32_t mw = __ldg(P.maskT + im), mw2 = q2 ? __ldg(P.maskT + im + 8) : 0u;
+            uint32_t mw = __ldg(P.maskT + im), mw2 = q2rt ? __ldg(P.maskT + im + 8) : 0u;
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
                 const uint32_t mcur = mw, mcur2 = mw2;
                 if (kb + 1 < U.kb_end) {
                     im += (unsigned)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
-                    if (q2) mw2 = __ldg(P.maskT + im + 8);
+                    if (q2rt) mw2 = __ldg(P.maskT + im + 8);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
                 mbar_wait_a(bar0 + 8 * kStages + 8 * st, pe ^ 1);
@@ -539,8 +540,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                 //      The four 16-byte label stores are issued between the four j pairs of the psi tile, so that the ALU-pipe
                 //      work of the expansion overlaps the FMA-pipe work of the distances (profiles/r01e).
                 const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
-                auto tile = [&](auto diag_tag) {
+                auto tile = [&](auto diag_tag, auto q2_tag) {
                     constexpr bool DIAG = decltype(diag_tag)::value;
+                    // both 256-column accumulators in use?  0 / 1: known at compile time (this copy of the tile code serves one
+                    // case), 2: the run-time flag
+                    constexpr int Q2T = decltype(q2_tag)::value;
+                    const bool q2 = Q2T == 2 ? q2rt : Q2T == 1;
                     const int x = kb * kKB - dthr;  // DIAG: element (r, t) is dropped when x <= 16 r - t
                     uint32_t pk[R][4];              // bytes 1 and 2 of (f_2tp, f_2tp+1): (lo, lo, v >> 8, v >> 8) of two j
 #pragma unroll
@@ -613,8 +618,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                         }
                     }
                 };
-                if (kb < kb_diag) tile(std::true_type{});   // K block overlaps (or lies below) the rows of this CTA: keep only j > i
-                else tile(std::false_type{});
+                // kb < kb_diag: the K block overlaps (or lies below) the rows of this CTA, keep only j > i.  GEO::kHoistQ2: four
+                // copies of the tile code and one branch per K block instead of eight uniform q2 branches inside it -- measured
+                // -5 % with the 12-warp geometry (dim = 8: 41.3 -> 39.1 ms) and +4 % with the 16-warp one (config 4: 2.69 -> 2.80 s)
+                using RT = std::integral_constant<int, 2>;
+                using Q0 = std::integral_constant<int, 0>;
+                using Q1 = std::integral_constant<int, 1>;
+                if (GEO::kHoistQ2) {
+                    if (kb < kb_diag) { if (q2rt) tile(std::true_type{}, Q1{}); else tile(std::true_type{}, Q0{}); }
+                    else { if (q2rt) tile(std::false_type{}, Q1{}); else tile(std::false_type{}, Q0{}); }
+                } else {
+                    if (kb < kb_diag) tile(std::true_type{}, RT{});
+                    else tile(std::false_type{}, RT{});
+                }
                 fence_async_smem();
                 __syncwarp();
                 if (lane == 0) {
