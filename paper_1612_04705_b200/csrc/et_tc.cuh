@@ -52,13 +52,14 @@ struct Geo {
     static constexpr int kKB = KB;                  // j per K block
     static constexpr int kProducerWarps = PW;
     static constexpr int kStages = ST;
-    static constexpr bool kHoistQ2 = PW == 12;      // see the producer loop of k_perm_tc
     static constexpr int kRowsPerThread = kTM * KB / 8 / (PW * 32);  // 4
     static constexpr int kEpiWarps = PW / 4;                         // warps per TMEM lane quarter
     static constexpr int kEpiGroups = (16 + kEpiWarps - 1) / kEpiWarps;  // most 32-column groups a warp reads in the epilogue
     __host__ __device__ static constexpr int epi_first(int e) { return 16 * e / kEpiWarps; }  // groups [epi_first(e), epi_first(e + 1)) of warp row e
     static constexpr int kProducers = PW * 32;
-    static constexpr int kThreadsTC = kProducers + 64;  // + the MMA warp + the record loader warp
+    static constexpr int kHelperWarps = 2;              // label helpers: the B tile of the second accumulator (k_perm_tc)
+    static constexpr int kThreadsTC = kProducers + 64 + 32 * kHelperWarps;  // + the MMA warp + the record loader warp + the helpers
+    static_assert(KB % (16 * kHelperWarps) == 0, "whole 8-j groups per helper warp");
     static constexpr int kABytes = 2 * kTM * KB;        // hi and lo digit tiles
     static constexpr int kBPlane = KB * 128;            // one plane of this CTA's half of B: KB j x 128 columns
     static constexpr int kBBytes = 2 * 2 * kBPlane;     // [q 2][digit 2][plane]
@@ -395,7 +396,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
     if (tid == 0) {
         // full / accempty are used in the leader only (arrivals from the producer warps of BOTH CTAs);
         // empty / accfull receive one multicast tcgen05.commit arrival in each CTA
-        for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], 2 * kProducerWarps); mbar_init(&bar_empty[s], 1); }
+        const uint32_t nfull = 2 * (kProducerWarps + (P.nq > 1 ? GEO::kHelperWarps : 0));  // the helpers fill the q = 1 planes
+        for (int s = 0; s < kStages; ++s) { mbar_init(&bar_full[s], nfull); mbar_init(&bar_empty[s], 1); }
         mbar_init(&bar_accfull, 1);
         mbar_init(&bar_accempty, 2 * kProducerWarps);
         for (int s = 0; s < kRecSlots; ++s) { mbar_init(&bar_rec[s], 1); mbar_init(&bar_recfree[s], kProducerWarps); }
@@ -462,7 +464,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                 }
             }
         }
-    } else {
+    } else if (warp < kProducerWarps) {
         // =========================================================================== producers + epilogue
         // psi task of a thread: octet oct of the K block (8 j), rows m_r = mrow0 + 16 r, r < R = 4.  A half-warp holds
         // 8 rows x 2 octets, so its 8-byte A-tile stores fall into 16 different bank pairs (no conflicts).
@@ -521,15 +523,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
             const int dthr = row0 + mrow0 - 8 * oct;
             // this thread's label words of K block kb, prefetched one block ahead into registers.  The element index is
             // 64 bits wide: npadK * words_total passes 2^32 at 2 M pooled rows with the maximum permutation count.
-            const bool q2rt = P.nq > 1;
+            // (the word of the second accumulator, q = 1, is expanded by the helper warps)
             unsigned long long im = (unsigned long long)(U.kb_begin * kKB + jj) * (unsigned)P.words_total + (unsigned)(P.word0 + 4 * (int)rank + l3);
-            uint32_t mw = __ldg(P.maskT + im), mw2 = q2rt ? __ldg(P.maskT + im + 8) : 0u;
+            uint32_t mw = __ldg(P.maskT + im);
             for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
-                const uint32_t mcur = mw, mcur2 = mw2;
+                const uint32_t mcur = mw;
                 if (kb + 1 < U.kb_end) {
                     im += (unsigned)(kKB * P.words_total);
                     mw = __ldg(P.maskT + im);
-                    if (q2rt) mw2 = __ldg(P.maskT + im + 8);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
                 mbar_wait_a(bar0 + 8 * kStages + 8 * st, pe ^ 1);
@@ -540,12 +541,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                 //      The four 16-byte label stores are issued between the four j pairs of the psi tile, so that the ALU-pipe
                 //      work of the expansion overlaps the FMA-pipe work of the distances (profiles/r01e).
                 const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
-                auto tile = [&](auto diag_tag, auto q2_tag) {
+                auto tile = [&](auto diag_tag) {
                     constexpr bool DIAG = decltype(diag_tag)::value;
-                    // both 256-column accumulators in use?  0 / 1: known at compile time (this copy of the tile code serves one
-                    // case), 2: the run-time flag
-                    constexpr int Q2T = decltype(q2_tag)::value;
-                    const bool q2 = Q2T == 2 ? q2rt : Q2T == 1;
                     const int x = kb * kKB - dthr;  // DIAG: element (r, t) is dropped when x <= 16 r - t
                     uint32_t pk[R][4];              // bytes 1 and 2 of (f_2tp, f_2tp+1): (lo, lo, v >> 8, v >> 8) of two j
 #pragma unroll
@@ -563,20 +560,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur >> (4 * tp + t)) & 0x01010101u;
                                 sts128((tp == 0 ? pbB : pbB1) + kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
-                                if (q2) {
-#pragma unroll
-                                    for (int t = 0; t < 4; ++t) q[t] = (mcur2 >> (4 * tp + t)) & 0x01010101u;
-                                    sts128((tp == 0 ? pbB : pbB1) + 3 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
-                                }
                             } else {
 #pragma unroll
                                 for (int t = 0; t < 4; ++t) q[t] = (mcur << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
                                 sts128(tp == 2 ? pbB : pbB1, make_uint4(q[0], q[1], q[2], q[3]));
-                                if (q2) {
-#pragma unroll
-                                    for (int t = 0; t < 4; ++t) q[t] = (mcur2 << (7 - (4 * (tp - 2) + t))) & 0x80808080u;
-                                    sts128((tp == 2 ? pbB : pbB1) + 2 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
-                                }
                             }
                         }
                         {
@@ -618,19 +605,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                         }
                     }
                 };
-                // kb < kb_diag: the K block overlaps (or lies below) the rows of this CTA, keep only j > i.  GEO::kHoistQ2: four
-                // copies of the tile code and one branch per K block instead of eight uniform q2 branches inside it -- measured
-                // -5 % with the 12-warp geometry (dim = 8: 41.3 -> 39.1 ms) and +4 % with the 16-warp one (config 4: 2.69 -> 2.80 s)
-                using RT = std::integral_constant<int, 2>;
-                using Q0 = std::integral_constant<int, 0>;
-                using Q1 = std::integral_constant<int, 1>;
-                if (GEO::kHoistQ2) {
-                    if (kb < kb_diag) { if (q2rt) tile(std::true_type{}, Q1{}); else tile(std::true_type{}, Q0{}); }
-                    else { if (q2rt) tile(std::false_type{}, Q1{}); else tile(std::false_type{}, Q0{}); }
-                } else {
-                    if (kb < kb_diag) tile(std::true_type{}, RT{});
-                    else tile(std::false_type{}, RT{});
-                }
+                if (kb < kb_diag) tile(std::true_type{});   // K block overlaps (or lies below) the rows of this CTA: keep only j > i
+                else tile(std::false_type{});
                 fence_async_smem();
                 __syncwarp();
                 if (lane == 0) {
@@ -686,6 +662,64 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         for (int g = 0; g < G; ++g) {
             out[(g * 32 + lane) * 2] = accQ[g];
             out[(g * 32 + lane) * 2 + 1] = accR[g];
+        }
+    } else if (P.nq > 1) {
+        // =========================================================================== label helpers (second accumulator)
+        // The two helper warps expand the label words of the column half q = 1 (word 8 + 4 rank + l3 of every j of the K
+        // block) into the q = 1 planes of the B tile, so that a producer thread expands one word per K block instead of
+        // two.  They cost no registers (18 warps are allocated as 20, 14 as 16) and take about a tenth of the producers'
+        // instructions; the "full" barrier counts their arrivals too.  Lane -> (l3 = lane & 3, j = 8 (NW h + i) + (lane >> 2)),
+        // i < NW = kKB / 16: the same (j, 16-byte chunk) -> address map as the producers' label stores.
+        constexpr int NW = kKB / (8 * GEO::kHelperWarps);
+        const int h = warp - (kProducerWarps + 2), l3 = lane & 3, jsub = lane >> 2;
+        const uint32_t bar0 = smem_u32(bars_s);
+        uint32_t pbB = smem_u32(smem) + kABytes + (NW * h) * 1024 + jsub * 128 + (((2 * l3) ^ jsub) << 4);
+        uint32_t st = 0, pe = 0;
+        const unsigned long long jstride = 8ull * (unsigned)P.words_total;
+        for (int u = cluster_id; u < P.nunits; u += nclusters) {
+            const Unit U = P.units[u];
+            unsigned long long im = (unsigned long long)(U.kb_begin * kKB + 8 * NW * h + jsub) * (unsigned)P.words_total +
+                                    (unsigned)(P.word0 + 8 + 4 * (int)rank + l3);
+            uint32_t mw[NW];
+            if (U.kb_begin < U.kb_end) {
+#pragma unroll
+                for (int i = 0; i < NW; ++i) mw[i] = __ldg(P.maskT + im + i * jstride);
+            }
+            for (int kb = U.kb_begin; kb < U.kb_end; ++kb) {
+                uint32_t cur[NW];
+#pragma unroll
+                for (int i = 0; i < NW; ++i) cur[i] = mw[i];
+                if (kb + 1 < U.kb_end) {
+                    im += (unsigned)(kKB * P.words_total);
+#pragma unroll
+                    for (int i = 0; i < NW; ++i) mw[i] = __ldg(P.maskT + im + i * jstride);
+                }
+                mbar_wait_a(bar0 + 8 * kStages + 8 * st, pe ^ 1);   // the stage is free
+#pragma unroll
+                for (int i = 0; i < NW; ++i) {
+                    const uint32_t b0 = pbB + i * 1024, b1 = b0 ^ 16u, m = cur[i];
+                    uint32_t q[4];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) q[t] = (m >> t) & 0x01010101u;
+                    sts128(b0 + 3 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) q[t] = (m >> (4 + t)) & 0x01010101u;
+                    sts128(b1 + 3 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) q[t] = (m << (7 - t)) & 0x80808080u;
+                    sts128(b0 + 2 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) q[t] = (m << (3 - t)) & 0x80808080u;
+                    sts128(b1 + 2 * kBPlane, make_uint4(q[0], q[1], q[2], q[3]));
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(mapa_rank(bar0 + 8 * st, 0));
+                const bool wrapS = st == kStages - 1;
+                st = wrapS ? 0 : st + 1;
+                pe ^= wrapS ? 1u : 0u;
+                pbB += wrapS ? (uint32_t)(kStageBytes - kStages * kStageBytes) : (uint32_t)kStageBytes;
+            }
         }
     }
     tc_fence_before();
