@@ -43,8 +43,8 @@ __host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
 
 // Geometry of the kernel: K blocks of KB j (KB / 32 UMMA K steps), PW producer warps (a thread evaluates 4 rows x 8 j of
 // the 128 x KB psi tile of its CTA: PW = KB / 8), ST shared-memory stages.  Two are built:
-//   Geo<96, 12, 3>:  14 warps x 128 registers, three 72 KB stages.  No register spills for any dim.
-//   Geo<128, 16, 2>: 18 warps x 96 registers, two 96 KB stages: a fourth producer warp per scheduler hides more of the
+//   Geo<96, 12, 3>:  16 warps (12 producers, MMA, loader, two label helpers) x 128 registers, three 72 KB stages.
+//   Geo<128, 16, 2>: 20 warps x 96 registers, two 96 KB stages: a fourth producer warp per scheduler hides more of the
 //                    producers' latency (profiles/r02_README.md: -4.6 % at config 4, same at dim = 2), but the i rows of
 //                    dim >= 6 no longer fit the registers (dim = 8: +75 %).  run_perm_tc takes it for dim <= 5.
 template <int KB, int PW, int ST>
@@ -539,7 +539,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                 //      8 q + 4 rank + l3 -> 32 columns, byte p of a word is label bit beta(p): register t of the lo plane is
                 //      (m >> t) & 0x01010101 (bytes a), of the hi plane (m << (7 - t)) & 0x80808080 (bytes 128 a).
                 //      The four 16-byte label stores are issued between the four j pairs of the psi tile, so that the ALU-pipe
-                //      work of the expansion overlaps the FMA-pipe work of the distances (profiles/r01e).
+                //      work of the expansion overlaps the FMA-pipe work of the distances (round 1, profiles/r01g_README.md history).
                 const uint32_t pbB1 = pbB ^ 16u;  // stage bases are 1024-byte aligned
                 auto tile = [&](auto diag_tag) {
                     constexpr bool DIAG = decltype(diag_tag)::value;
