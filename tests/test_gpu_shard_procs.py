@@ -15,13 +15,12 @@ pytestmark = pytest.mark.gpu
 def _worker(rank, world, port, q):
     import torch.distributed as dist
 
-    from paper_1612_04705_b200 import binding, build
+    from paper_1612_04705_b200 import binding
     from paper_1612_04705_b200 import datagen as dg
 
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        build.build()
         c = dg.config(1, scale=0.2)
         s = dg.make_sample(c)
         c4 = dg.config(4, scale=0.02)
@@ -47,6 +46,10 @@ def _worker(rank, world, port, q):
 
 def test_unit_shard_two_processes_over_gloo():
     import torch.multiprocessing as mp
+
+    from paper_1612_04705_b200 import build
+
+    build.build()   # once, here: the two ranks must not both decide to rebuild libet.so
 
     with socket.socket() as sk:
         sk.bind(("127.0.0.1", 0))
