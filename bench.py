@@ -158,7 +158,10 @@ def run_ours(args):
         os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
-    build.build()
+    if rank == 0:
+        build.build()      # one rank (re)builds libet.so if it is stale; the others wait
+    if world > 1:
+        dist.barrier()
     peaks = load_peaks()
 
     cfg = dg.config(args.config)
