@@ -24,6 +24,9 @@
  *   - The context owns a stream (or borrows the caller's), all scratch and the
  *     label buffers; it is not thread-safe (one context per host thread).
  *   - Every call is complete (stream-synchronised) on return.
+ *   - ET_DEVICE inputs must be complete before the call as seen from the context's stream: produced on
+ *     that stream (pass it to et_create), or synchronised by the caller (a library-owned stream is
+ *     non-blocking and does not wait for the legacy default stream).  They must live on the context's device.
  *   - On any status != ET_OK the outputs are untouched and et_last_error()
  *     explains.  There is no CPU fallback: without a CUDA device et_create
  *     fails with ET_ERR_CUDA.
