@@ -14,6 +14,9 @@ can be interrupted and restarted):
                                                        (config 4: the P-odd grouping (I+IV) vs (II+III))
   cfgC.perm.K                                          T of permutation K (from scratch, labels of reading R4, the
                                                        config's permutation seed), K < 2 (config 4: K = 0)
+  cfgC.perm.K (K >= the count above, --extra-perm)     the same quantity for one more permutation, evaluated as
+                                                       oracle.T on the split that oracle.labels gives (one pass instead
+                                                       of re-running the whole block)
   cfg4.even.{...}                                      P-even grouping (I+II) vs (III+IV) = Eq. 2 of (X, Xbar)
   cfg4.count.{I,II,III,IV}                             class sizes of the Sect. 5 split
 Each block is preceded by a comment line with the host cores used and the wall time.
@@ -84,11 +87,28 @@ def run_two_sample(out: Out, tag: str, a, b, sigma, wa, wb, nperm, seed):
         out.put(f"{tag}.perm.{k}", r.T_perm[k])
 
 
+def run_extra_perm(out: Out, tag: str, a, b, sigma, wa, wb, k, seed):
+    """T of permutation k alone: the pooled events split by oracle.labels (reading R4), Eq. 2 by oracle.T."""
+    key = f"{tag}.perm.{k}"
+    if key in out.have:
+        return
+    pooled = np.vstack([a, b])
+    w = None if wa is None else np.concatenate([wa, wb])
+    N, n = len(pooled), len(a)
+    lab = (oracle.labels(N, n, k + 1, seed)[:, k >> 5] >> (k & 31)) & 1
+    t0 = time.time()
+    r = oracle.T(pooled[lab == 1], pooled[lab == 0], sigma, None if w is None else w[lab == 1], None if w is None else w[lab == 0])
+    out.comment(f"{key}: oracle.labels + oracle.T on the permuted split ({int(lab.sum())} + {N - int(lab.sum())} events), "
+                f"{oracle.num_threads()} host cores, {time.time() - t0:.0f} s wall")
+    out.put(key, r.T)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="3,2,4")
     ap.add_argument("--out", default=os.path.join(ROOT, "tests", "golden", "fullsize_T.txt"))
     ap.add_argument("--scale", type=float, default=1.0, help="shrink n, nbar (dry runs only; the committed file is scale 1)")
+    ap.add_argument("--extra-perm", type=int, default=-1, help="also store T of this permutation index (one oracle.T pass)")
     args = ap.parse_args()
     out = Out(args.out)
     if not out.have:
@@ -99,6 +119,8 @@ def main():
         s = dg.make_sample(cfg)
         if not cfg.podd:
             run_two_sample(out, tag, s.x, s.xbar, cfg.sigma, s.wx, s.wxbar, 2, cfg.perm_seed)
+            if args.extra_perm >= 0:
+                run_extra_perm(out, tag, s.x, s.xbar, cfg.sigma, s.wx, s.wxbar, args.extra_perm, cfg.perm_seed)
             continue
         posx, _ = oracle.podd_split(s.mom_x[:, 0], s.mom_x[:, 1], s.mom_x[:, 2], False)
         posb, _ = oracle.podd_split(s.mom_xbar[:, 0], s.mom_xbar[:, 1], s.mom_xbar[:, 2], True)
@@ -112,6 +134,8 @@ def main():
             out.comment(f"{tag}.even: oracle.T n={cfg.n} nbar={cfg.nbar}; {oracle.num_threads()} host cores, {time.time() - t0:.0f} s wall")
             out.put_result(f"{tag}.even", r)
         run_two_sample(out, tag, np.vstack([I, IV]), np.vstack([II, III]), cfg.sigma, None, None, 1, cfg.perm_seed)
+        if args.extra_perm >= 0:
+            run_extra_perm(out, tag, np.vstack([I, IV]), np.vstack([II, III]), cfg.sigma, None, None, args.extra_perm, cfg.perm_seed)
 
 
 if __name__ == "__main__":
