@@ -7,18 +7,19 @@
 //   R_c = sum_{i<j} w_i w_j psi_ij (a_ic + a_jc)       = sum_i real_i w_i Y_ic + sum_i a_ic w_i Y_i,ones
 //   S   = sum_{i<j} w_i w_j psi_ij                     = Q of the all-ones column
 // and S_xx = Q, S_bb = S - R + Q, S_xb = R - 2Q.  Y = Psi A is a GEMM whose left operand is
-// never stored.  A cluster of two CTAs (one SM pair) works on a 256-row tile; per K block of 96 j each CTA evaluates its
-// 128 x 96 tile of psi in fp32 (packed FFMA2 + MUFU.EX2, 12 producer warps, 4 rows x 8 j per thread; the j side comes
-// as pre-formatted pair records that a loader warp bulk-copies into a shared-memory ring), quantises
-// Psi_ij = w_j psi_ij to a 15-bit fixed-point integer v = 128 hi + lo, writes the two digit tiles (hi 8 bits, lo 7) into
-// its shared memory as K chunks of 32 bytes in the UMMA K-major SWIZZLE_32B layout, and expands ITS HALF of the label
-// columns from the bit masks into the B tile (bytes 128 a and a, MN-major SWIZZLE_128B).  One thread of the leader CTA
-// issues tcgen05.mma.cta_group::2.kind::i8 (M = 256, N = 256, K = 32): the pair's tensor cores read A from their own
-// SM and each half of B from one SM of the pair, so a label byte is written and read once per 256 rows instead of
-// once per 128.  The kernel is bound by the CUDA-core tile generation, not by the tensor pipe
-// (profiles/r01g_README.md).  Accumulation is ONE int32 per column in TMEM (all 512 columns of each SM).  Integer
-// accumulation is exact, so S, R and Q are sums of the SAME quantised Psi whatever the schedule (hard part 3
-// "consistency"), and the unweighted result is bit-reproducible.
+// never stored.  A cluster of two CTAs (one SM pair) works on a 256-row tile; per K block of KB j (Geo below: 128 or 96)
+// each CTA evaluates its 128 x KB tile of psi in fp32 (packed FFMA2 + MUFU.EX2, KB / 8 producer warps, 4 rows x 8 j per
+// thread; the j side comes as pre-formatted pair records that a loader warp bulk-copies into a shared-memory ring),
+// quantises Psi_ij = w_j psi_ij to a 15-bit fixed-point integer v = lo + 128 hi (lo = v & 255, hi = 2 (v >> 8); see
+// kMagicUnsigned below), writes the two digit tiles into its shared memory as K chunks of 32 bytes in the UMMA K-major
+// SWIZZLE_32B layout, and expands ITS HALF of the label columns from the bit masks into the B tile (bytes a and 128 a,
+// MN-major SWIZZLE_128B).  One thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M = 256, N = 256,
+// K = 32): the pair's tensor cores read A from their own SM and each half of B from one SM of the pair, so a label byte
+// is written and read once per 256 rows instead of once per 128.  At config 4 the tensor pipe is 74 % busy, the producers
+// are latency-bound and the board sits at its power cap (profiles/r02_README.md).  Accumulation is
+// ONE int32 per column in TMEM (all 512 columns of each SM).  Integer accumulation is exact, so S, R and Q are sums of the
+// SAME quantised Psi whatever the schedule (hard part 3 "consistency"), and the unweighted result is
+// bit-reproducible.
 //
 // Columns of one launch (512): 0 = observed labelling, 1 = second labelling (P-even grouping of Sect. 5, else a copy
 // of column 0), 2 = all ones, 3.. = 509 permutations.  Inside a 32-column mask word the B tile / TMEM column p holds
@@ -107,7 +108,7 @@ __host__ __device__ constexpr int beta(int p) { return (p >> 2) + 8 * (p & 3); }
 
 struct Unit {
     int I;         // 256-row tile
-    int kb_begin;  // first K block (96 j each), >= the block that holds the tile's first row
+    int kb_begin;  // first K block (Geo::kKB j each), >= the block that holds the tile's first row
     int kb_end;
     int pad;
 };
@@ -355,7 +356,7 @@ struct TCParams {
     int word0;
     const Unit *units;
     int nunits;
-    float sc256;             // 256 sc: Psi_ij = w_j psi_ij is quantised to v = floor(sc Psi + dither) (15 bits); applied in recP
+    float sc256;             // 256 sc: Psi_ij = w_j psi_ij is quantised to v = floor(sc Psi + 1/2) (15 bits); applied in recP
     float magic;             // kMagicUnsigned, or kMagicSigned when weights can be negative
     uint32_t hixor;          // 0, or 0x80808080 with kMagicSigned: hi digit = 2 byte2 - 128
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
@@ -480,7 +481,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         for (int g = 0; g < G; ++g) { accQ[g] = 0; accR[g] = 0; }
         // Thread constants of the main loop.  They are made opaque to the compiler (keep()), which otherwise
         // rematerialises them from the lane index in every K block to save registers (~45 instructions, profiles/r01c).
-        // dither levels of this thread (two j per packed instruction); kept opaque like the other loop constants
         const uint32_t fmask = __float_as_uint(P.magic);  // a masked element: v = 0
         const float magic1 = keep(P.magic + 128.f);        // + half a step: round to nearest
         const float2 magicA = make_float2(magic1, magic1);
@@ -518,7 +518,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                 for (int k = 0; k < D; ++k) ui2[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
             }
             // K blocks below kb_diag overlap (or lie below) the rows of this CTA: there only j > i is kept, i.e. element
-            // (r, t) of this thread's tile is dropped when kb * 64 + t <= dthr + 16 r
+            // (r, t) of this thread's tile is dropped when kb * kKB + t <= dthr + 16 r
             const int kb_diag = (row0 + kTM + kKB - 1) / kKB;
             const int dthr = row0 + mrow0 - 8 * oct;
             // this thread's label words of K block kb, prefetched one block ahead into registers.  The element index is
