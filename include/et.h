@@ -331,6 +331,37 @@ et_status et_row_sums(et_ctx *ctx, const void *x, const double *wx, int64_t n,
                       int dim, et_dtype dtype, et_memspace mem, double sigma,
                       const int64_t *rows, int64_t nrows, double *r_x, double *r_xbar);
 
+/* ---- The entry point that allocates nothing (csrc/et_static.cu) --------------------------------------
+ * For callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid allocation.  et_T_static evaluates Eq. 2 like et_T, but all of its scratch (the
+ * bounding box, the pooled fp32 records, the per-CTA partial sums) is ONE file-scope static __device__
+ * array of ET_STATIC_SCRATCH_BYTES that every GPU loading libet.so holds until exit.  It needs no context.
+ *
+ *   et_static_setup(device): once per device, BEFORE any capture: resolves the device address of the array
+ *     (cudaGetSymbolAddress with that device current; the caller's current device is restored).  Idempotent.
+ *   et_T_static(device, cuda_stream, x, n, xbar, nbar, dim, dtype, sigma, out_device):
+ *     x[n][dim], xbar[nbar][dim] are DEVICE pointers on `device`, complete as seen from `cuda_stream` (NULL =
+ *     the legacy default stream); out_device is a DEVICE et_result owned by the caller (8-byte aligned).  The call
+ *     enqueues five kernels on the stream and returns WITHOUT synchronising: it calls no cudaMalloc, cudaFree,
+ *     cudaMallocHost, creates no stream or event, and copies nothing to the host; the caller synchronises the
+ *     stream (or launches the captured graph) before reading *out_device.  Makes `device` current.
+ *     Limit: 65536 + npad * 4 * ceil((dim + 1) / 4) * 4 bytes <= ET_STATIC_SCRATCH_BYTES, npad = n and nbar
+ *     each rounded up to 1024 -- about 5.2e5 pooled events at dim <= 3, 2.6e5 at dim 4..7, 1.7e5 at dim 8
+ *     (BASELINE configs 0, 1 and 3 fit, configs 2 and 4 do not); a larger call returns ET_ERR_INVALID and
+ *     enqueues nothing.  Other errors: ET_ERR_INVALID (null pointer, n < 2, nbar < 2, dim, dtype, set-up
+ *     missing), ET_ERR_SIGMA, ET_ERR_CUDA (a launch failed).  Non-finite coordinates cannot be reported
+ *     without a synchronisation: T, the three terms and the three sums of *out_device are then NaN.
+ *     Every call shares the array and finds the last call's contents in it; the kernels reset or overwrite
+ *     what they use.  Calls that overlap on the GPU (two streams, two host threads, two graphs in flight) RACE
+ *     on the array: the caller serialises them.  Arithmetic: that of et_T's difference form (fp32 per pair,
+ *     fp64 sums, fixed order): the result agrees with et_T to rounding order.
+ *   et_static_last_error(): message of the calling thread's last failed et_static_setup / et_T_static. */
+#define ET_STATIC_SCRATCH_BYTES (8u << 20)
+et_status et_static_setup(int device);
+et_status et_T_static(int device, void *cuda_stream, const void *x, int64_t n, const void *xbar, int64_t nbar,
+                      int dim, et_dtype dtype, double sigma, et_result *out_device);
+const char *et_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,7 +29,8 @@ STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ER
 
 # every symbol include/et.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ["et_create", "et_destroy", "et_last_error", "et_set_option", "et_set_shard", "et_get_stats", "et_version", "et_T",
-           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_permutation_test_sigmas", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums", "et_scp"]
+           "et_T_weighted", "et_T_sigmas", "et_T_bkg", "et_bkg_permutation_test", "et_gev_pvalue", "et_permutation_test", "et_permutation_test_sigmas", "et_podd_split", "et_podd_test", "et_perm_labels", "et_row_sums", "et_scp",
+           "et_static_setup", "et_T_static", "et_static_last_error"]
 
 
 class EtError(RuntimeError):
@@ -222,6 +223,7 @@ def lib():
         vp, i64, u64, dbl, ci = C.c_void_p, C.c_int64, C.c_uint64, C.c_double, C.c_int
         L.et_last_error.restype = C.c_char_p
         L.et_version.restype = C.c_char_p
+        L.et_static_last_error.restype = C.c_char_p
         L.et_destroy.restype = None
         # the argument types of EVERY entry point of include/et.h, in its order (a missing one would let ctypes pass a
         # Python int as a 32-bit C int and truncate an int64 silently)
@@ -245,6 +247,7 @@ def lib():
             "et_perm_labels": [vp, i64, i64, i64, u64, ci, vp],
             "et_row_sums": [vp] + wsample + tail + [vp, i64, vp, vp],
             "et_scp": [vp] + sample + [ci, ci, ci, vp, vp, vp, vp, vp, vp, vp],
+            "et_static_setup": [ci], "et_T_static": [ci, vp] + sample + [ci, ci, dbl, vp], "et_static_last_error": [],
         }.items():
             getattr(L, name).argtypes = args
         assert all(getattr(L, n).argtypes is not None for n in SYMBOLS)
@@ -356,6 +359,43 @@ def make_allgather(rank: int, world: int, group=None):
             traceback.print_exc()
             return 1
     return fn
+
+
+# ---- the entry point that allocates nothing (include/et.h, csrc/et_static.cu) -------------------------------------
+STATIC_SCRATCH_BYTES = 8 << 20
+RESULT_DOUBLES = C.sizeof(_Result) // 8   # a device et_result is this many 8-byte words (the last one an int64)
+
+
+def static_setup(device: int = 0) -> None:
+    """Once per device, outside any graph capture: resolves the device address of the library's static scratch."""
+    st = lib().et_static_setup(C.c_int(device))
+    if st != ET_OK:
+        raise EtError(st, lib().et_static_last_error().decode())
+
+
+def T_static(x, xbar, sigma: float, out, stream=None) -> None:
+    """et_T_static: x, xbar are CUDA tensors [n, dim] (float32 or float64, same device), `out` a CUDA float64 tensor of
+    RESULT_DOUBLES elements on that device (the device et_result).  Enqueues on `stream` (None: the legacy default
+    stream) and returns without synchronising; decode a host copy of `out` with result_from_words."""
+    ax, ab = _coords(x, xbar)
+    if ax.mem != ET_DEVICE:
+        raise ValueError("T_static takes device tensors (there is no staging: the call allocates nothing)")
+    import torch
+
+    if not (_is_torch(out) and out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= RESULT_DOUBLES
+            and out.device.index == ax.keep.device.index):
+        raise ValueError(f"out must be a contiguous CUDA float64 tensor of >= {RESULT_DOUBLES} elements on the inputs' device")
+    sp = None if stream is None else C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+    st = lib().et_T_static(C.c_int(ax.keep.device.index), sp, ax.ptr, C.c_int64(ax.shape[0]), ab.ptr, C.c_int64(ab.shape[0]),
+                           C.c_int(ax.shape[1]), C.c_int(ax.dtype), C.c_double(sigma), C.c_void_p(out.data_ptr()))
+    if st != ET_OK:
+        raise EtError(st, lib().et_static_last_error().decode())
+
+
+def result_from_words(words) -> Result:
+    """A host copy (numpy float64[RESULT_DOUBLES]) of a device et_result -> Result."""
+    w = np.ascontiguousarray(np.asarray(words, dtype=np.float64)[:RESULT_DOUBLES])
+    return _res(_Result.from_buffer_copy(w.tobytes()))
 
 
 class Context:
