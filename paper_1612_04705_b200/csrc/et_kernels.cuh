@@ -160,7 +160,7 @@ __device__ __forceinline__ JRec<D> load_jrec(const float4 *__restrict__ sj, int 
 // fp32 per pair and per 128-j partial row sum, fp64 from there on; per-unit block reduction in a fixed order, so the
 // result depends only on the grid size.
 // Packed FP32 pipe, two j per instruction: the j records are staged in shared memory as PAIRS, float2 k of pair p =
-// (-u_{2p,k}, -u_{2p+1,k}), float2 D = (w_2p, w_2p+1), and every thread keeps its R i rows duplicated, (u_ik, u_ik), so that one FADD2 / FFMA2 does the
+// (-u_{2p,k}, -u_{2p+1,k}), float2 D = (w_2p, w_2p+1), and every thread's R i rows enter as (u_ik, u_ik) -- ONE register: ptxas encodes the pair as the scalar-broadcast operand form R.F32 of FADD2 / FFMA2 (round 2: a materialised register pair per coordinate cost 20 registers at D = 5: Gram form 128 -> 80 registers, 3 CTAs per SM instead of 2, config 4 578 -> 561 ms) -- so that one FADD2 / FFMA2 does the
 // subtraction / square-accumulate of (i, 2p) and (i, 2p+1) at once.  Each half of a packed instruction rounds like the
 // scalar one (u_i + (-u_j) == u_i - u_j exactly), so psi is bit-identical to psi_pair<D>.  The packed instructions
 // halve the issue slots per pair (2D+1 FP32 lane-ops and one MUFU.EX2 per pair stay): measured 2.3 -> 2.8e12 pairs/s
@@ -211,9 +211,9 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T(const float *__restrict__ 
                 const float4 t = __ldg(p + q);
                 v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
             }
-            // "+ 0" materialises the duplicated pair in an aligned register pair once per unit
+            // (u_ik, u_ik) from one register: the packed instructions take it as a scalar-broadcast operand (R.F32)
 #pragma unroll
-            for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
+            for (int k = 0; k < D; ++k) ui[r][k] = make_float2(v[k], v[k]);
             wi[r] = v[D];
             self[r] = v[D];
             rs[r] = 1.0;
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kThreads) k_pairs_T_multi(const float *__restr
                 v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
             }
 #pragma unroll
-            for (int k = 0; k < D; ++k) ui[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
+            for (int k = 0; k < D; ++k) ui[r][k] = make_float2(v[k], v[k]);
             wi[r] = v[D];
         }
         double racc[NS][R];

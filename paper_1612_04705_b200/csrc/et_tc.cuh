@@ -324,7 +324,7 @@ __device__ __forceinline__ T lane_transpose_sum(T (&x)[32], int lane)
 
 // Pair records of the j side: recP[pair][entry] float2, entry k < D = (-u_{2 pair, k}, -u_{2 pair + 1, k}), entry D =
 // (s, s') with s = 256 sc w_j (the quantisation scale times the weight), zero padded to pair_rec_f4(D) float4.  With the
-// i rows duplicated in registers, d = u_i + (-u_j) and Psi = 2^(-e) s + magic are packed FADD2 / FFMA2 over two j.
+// i rows as scalar-broadcast operands (u_ik, u_ik) of the packed instructions, d = u_i + (-u_j) and Psi = 2^(-e) s + magic are packed FADD2 / FFMA2 over two j.
 template <int D>
 __global__ void __launch_bounds__(kThreads) k_pair_records(const float *__restrict__ rec, long long npairs, float sc, float4 *__restrict__ recP)
 {
@@ -502,7 +502,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
             const Unit U = P.units[u];
             const int row0 = U.I * kTM2 + (int)rank * kTM;   // npad < 2^31
-            // this thread's i rows, duplicated for the packed FP32 pipe
+            // this thread's i rows; the packed FP32 instructions take (u_ik, u_ik) as a scalar-broadcast operand (R.F32 in SASS)
             float2 ui2[R][D];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
@@ -513,9 +513,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                     const float4 t = __ldg(p + qq);
                     v[4 * qq] = t.x; v[4 * qq + 1] = t.y; v[4 * qq + 2] = t.z; v[4 * qq + 3] = t.w;
                 }
-                // "+ 0" materialises each pair in an aligned register pair once per unit
+                // one register per coordinate (a materialised pair cost 20 registers at D = 5: config 4 -0.9 %, dim 6-8 -8..10 %)
 #pragma unroll
-                for (int k = 0; k < D; ++k) ui2[r][k] = __fadd2_rn(make_float2(v[k], v[k]), make_float2(0.f, 0.f));
+                for (int k = 0; k < D; ++k) ui2[r][k] = make_float2(v[k], v[k]);
             }
             // K blocks below kb_diag overlap (or lie below) the rows of this CTA: there only j > i is kept, i.e. element
             // (r, t) of this thread's tile is dropped when kb * kKB + t <= dthr + 16 r
