@@ -110,3 +110,24 @@ def test_c_caller_runs_et_T_on_the_gpu(lib, tmp_path):
     r = subprocess.run([build_c_caller(tmp_path)], capture_output=True, text=True)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "T = 0.125" in r.stdout and "permutation test ok" in r.stdout, r.stdout
+
+
+def test_static_entry_point_fails_loudly_without_setup_or_device(lib):
+    """et_T_static (the entry point that allocates nothing) never computes without its set-up: without a CUDA device
+    et_static_setup reports ET_ERR_CUDA, and a call on a device that was not set up is ET_ERR_INVALID with a message."""
+    try:
+        import torch
+
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    if not has_gpu:
+        assert lib.et_static_setup(0) == -6
+        assert b"CUDA" in lib.et_static_last_error()
+    buf = (ctypes.c_double * 16)()
+    out = (ctypes.c_double * 10)()
+    p = ctypes.cast(buf, ctypes.c_void_p)
+    st = lib.et_T_static(63, None, p, 4, p, 4, 2, 1, 0.3, ctypes.cast(out, ctypes.c_void_p))  # device 63 is never set up
+    assert st == -1 and b"et_static_setup" in lib.et_static_last_error()
+    assert lib.et_T_static(63, None, None, 4, p, 4, 2, 1, 0.3, ctypes.cast(out, ctypes.c_void_p)) == -1
+    assert lib.et_T_static(63, None, p, 4, p, 4, 2, 1, -1.0, ctypes.cast(out, ctypes.c_void_p)) == -2
