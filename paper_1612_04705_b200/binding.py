@@ -287,7 +287,7 @@ def _marshal(a, want=None) -> _Arr:
         return _Arr(C.c_void_p(a.data_ptr()), dt, mem, tuple(a.shape), a)
     a = np.asarray(a)
     if want == "f64" or a.dtype not in (np.float32, np.float64):
-        a = a.astype(np.float64)
+        a = a.astype(np.float64, copy=False)   # no copy when it already is float64: a pinned buffer stays the caller's pinned buffer
     a = np.ascontiguousarray(a)
     dt = ET_F32 if a.dtype == np.float32 else ET_F64
     return _Arr(C.c_void_p(a.ctypes.data), dt, ET_HOST, a.shape, a)
