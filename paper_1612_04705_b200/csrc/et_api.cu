@@ -73,6 +73,7 @@ struct et_ctx {
     int64_t opt_distance = 0;       // ET_OPT_DISTANCE
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     Buf scpcnt, scpS;
+    Buf selcand, selsave;  // radix select: candidate lists of the index half, state after the key32 half
     bool tc_attr_set = false;
     // NVTX ranges: the call and its spans (labels, O(N^2) kernels, escalation); ids of the open ones
     nvtxRangeId_t nvtx_call = 0, nvtx_span[8] = {0};
@@ -472,7 +473,7 @@ et_status run_label_select(et_ctx *ctx, long long N, long long n_x, int nperm, u
     const long long p0 = ctx->opt_perm_offset;
     const unsigned ngroups = (unsigned)(((p0 + nperm - 1) >> 2) - (p0 >> 2) + 1);
     const dim3 grid((unsigned)((N + (long long)kThreads * ev - 1) / ((long long)kThreads * ev)), ngroups);
-    for (int pass = 0; pass < 8; ++pass) {
+    auto hist_pass = [&](int pass) -> et_status {
         k_sel_hist<<<grid, kThreads, 0, ctx->stream>>>(N, nperm, p0, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), pass,
                                                       static_cast<const SelState *>(ctx->sel.p),
                                                       static_cast<unsigned int *>(ctx->hist.p), ev);
@@ -480,6 +481,30 @@ et_status run_label_select(et_ctx *ctx, long long N, long long n_x, int nperm, u
         k_sel_pick<<<(nperm + 7) / 8, 256, 0, ctx->stream>>>(static_cast<SelState *>(ctx->sel.p),
                                                              static_cast<unsigned int *>(ctx->hist.p), nperm);
         LAUNCH_CHECK();
+        return ET_OK;
+    };
+    for (int pass = 0; pass < 4; ++pass) ET_TRY(hist_pass(pass));   // the key32 half of the composites
+    // the index half: one sweep lists the events of the wanted key32 bucket (about one), k_sel_finish takes the rank-th index
+    ET_TRY(ensure(ctx, ctx->selcand, (size_t)nperm * (kSelCand + 1) * sizeof(uint32_t) + 16));
+    unsigned int *cand_cnt = static_cast<unsigned int *>(ctx->selcand.p);
+    int *overflow = reinterpret_cast<int *>(cand_cnt + nperm);
+    uint32_t *cand = reinterpret_cast<uint32_t *>(cand_cnt + nperm + 4);
+    CUDA_TRY(cudaMemsetAsync(cand_cnt, 0, ((size_t)nperm + 4) * sizeof(uint32_t), ctx->stream));
+    ET_TRY(ensure(ctx, ctx->selsave, (size_t)nperm * sizeof(SelState)));
+    CUDA_TRY(cudaMemcpyAsync(ctx->selsave.p, ctx->sel.p, (size_t)nperm * sizeof(SelState), cudaMemcpyDeviceToDevice, ctx->stream));
+    k_sel_collect<<<grid, kThreads, 0, ctx->stream>>>(N, nperm, p0, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+                                                     static_cast<const SelState *>(ctx->sel.p), cand_cnt, cand, ev);
+    LAUNCH_CHECK();
+    k_sel_finish<<<(nperm + 255) / 256, 256, 0, ctx->stream>>>(static_cast<SelState *>(ctx->sel.p), cand_cnt, cand, nperm, overflow);
+    LAUNCH_CHECK();
+    int ovf = 0;
+    ET_TRY(ensure_pinned(ctx, 4096));
+    CUDA_TRY(cudaMemcpyAsync(ctx->pinned, overflow, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+    memcpy(&ovf, ctx->pinned, sizeof(int));
+    if (ovf != 0) {  // a bucket beyond kSelCand events: the four sweeps over the index half, from the saved state
+        CUDA_TRY(cudaMemcpyAsync(ctx->sel.p, ctx->selsave.p, (size_t)nperm * sizeof(SelState), cudaMemcpyDeviceToDevice, ctx->stream));
+        for (int pass = 4; pass < 8; ++pass) ET_TRY(hist_pass(pass));
     }
     return ET_OK;
 }
@@ -879,6 +904,19 @@ et_status finish_perm(et_ctx *ctx, int nwords, int64_t nperm, long long npairs, 
 
 
 // ---- tensor-core permutation sums (K-PERM-TC) -------------------------------------------------------------
+// W_c of the TC layout for unit weights (chunk ch, column c at ch * 512 + c): see run_perm_tc_g
+__global__ void k_fill_W_tc(int nchunks, int nperm, double nA, double n_second, double Ntot, double *__restrict__ W)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nchunks * tc::kCols) return;
+    const int ch = k / tc::kCols, c = k % tc::kCols;
+    double w;
+    if (c == 0) w = nA;
+    else if (c == 1) w = n_second;
+    else if (c == 2) w = Ntot;
+    else w = ch * tc::kPermsPerChunk + c - tc::kSpecial < nperm ? nA : 0.0;
+    W[k] = w;
+}
 // T for every label column of the TC layout (et_tc.cuh): chunk ch, column c at index ch * 512 + c.
 __global__ void __launch_bounds__(256) k_perm_stat_tc(const double *__restrict__ Q, const double *__restrict__ R, const double *__restrict__ W,
                                                      int nperm, long long npairs_obs, long long npairs_second, double qstep, double egram, double wabs,
@@ -1210,7 +1248,17 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     const int nchunkW = 64;
     ET_TRY(ensure(ctx, ctx->tcWpart, (size_t)words_total * nchunkW * 32 * sizeof(double)));
     ET_TRY(ensure(ctx, ctx->tcW, (size_t)words_total * 32 * sizeof(double)));
-    {
+    if (!weighted) {
+        // unit weights: W_c is the number of ones of the column, known without a pass over the 256 MB of labels -- n_a for the
+        // observed labelling and for every permutation (reading R4 preserves the sizes; pin P10), the size of the second
+        // labelling's sample, N for the all-ones column: the same doubles k_perm_W_tc sums up
+        long long n_second = 0;
+        for (int c = 0; c < L.ncls; ++c)
+            if (lab2_classes >> c & 1u) n_second += L.seg_count[c];
+        k_fill_W_tc<<<(nchunks * tc::kCols + 255) / 256, 256, 0, ctx->stream>>>(nchunks, nperm, (double)L.n_a, (double)n_second, (double)L.N,
+                                                                                 static_cast<double *>(ctx->tcW.p));
+        LAUNCH_CHECK();
+    } else {
         const dim3 gridW((unsigned)nchunkW, (unsigned)words_total);
         tc::k_perm_W_tc<<<gridW, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
                                                             static_cast<const uint32_t *>(ctx->maskT.p), words_total, L.npad, nchunkW,
@@ -1314,7 +1362,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
                    &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
-                   &ctx->scpcnt, &ctx->scpS};
+                   &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);

@@ -791,6 +791,61 @@ __global__ void k_sel_pick(SelState *st, unsigned int *hist, int nperm)
     for (int k = 0; k < 8; ++k) h[lane * 8 + k] = 0u;
 }
 
+// After the four passes over the key32 half of the composites the wanted one lies in the bucket of the events whose key32
+// equals the prefix: one event plus N / 2^32 expected others.  Instead of four more sweeps over the index half (each
+// a Philox evaluation per event and four permutations), ONE sweep lists the bucket's events and k_sel_finish takes the
+// rank-th smallest index among them -- the same K*_p.  cand[p][kSelCand]; a bucket that does not fit (cnt > kSelCand:
+// not reachable for N < 2^31, expected bucket size <= 1.5) sets *overflow and the host falls back to the four sweeps.
+constexpr int kSelCand = 64;
+__global__ void __launch_bounds__(kThreads) k_sel_collect(long long N, int nperm, long long p0, uint32_t seed_lo, uint32_t seed_hi,
+                                                         const SelState *__restrict__ st, unsigned int *__restrict__ cand_cnt,
+                                                         uint32_t *__restrict__ cand, int ev_per_thread)
+{
+    const long long p4 = (p0 >> 2) + blockIdx.y;
+    unsigned long long pre[4];
+    long long pl[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        pl[q] = 4 * p4 + q - p0;
+        if (pl[q] < 0 || pl[q] >= nperm) pl[q] = -1;
+        pre[q] = pl[q] >= 0 ? st[pl[q]].prefix : 0ull;
+    }
+    const long long base = (long long)blockIdx.x * kThreads * ev_per_thread;
+    for (int e = 0; e < ev_per_thread; ++e) {
+        const long long i = base + (long long)e * kThreads + threadIdx.x;
+        if (i >= N) break;
+        uint64_t K[4];
+        label_keys4((uint32_t)i, (uint32_t)p4, seed_lo, seed_hi, K);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (pl[q] < 0 || (K[q] >> 32) != pre[q]) continue;
+            const unsigned int slot = atomicAdd(&cand_cnt[pl[q]], 1u);
+            if (slot < (unsigned)kSelCand) cand[pl[q] * kSelCand + slot] = (uint32_t)i;
+        }
+    }
+}
+// one thread per permutation; *overflow != 0 afterwards: some bucket did not fit and NO state may be used
+__global__ void k_sel_finish(SelState *st, unsigned int *__restrict__ cand_cnt, const uint32_t *__restrict__ cand, int nperm, int *overflow)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= nperm) return;
+    const unsigned int cnt = cand_cnt[p];
+    cand_cnt[p] = 0u;  // clean for the next call
+    if (cnt > (unsigned)kSelCand) { atomicOr(overflow, 1); return; }
+    const uint32_t *c = cand + (long long)p * kSelCand;
+    const long long rank = st[p].rank;
+    for (unsigned int a = 0; a < cnt; ++a) {
+        long long below = 0;
+        for (unsigned int b = 0; b < cnt; ++b) below += c[b] < c[a] ? 1 : 0;   // indices are distinct
+        if (below == rank) {
+            st[p].prefix = (st[p].prefix << 32) | (unsigned long long)c[a];
+            st[p].rank = 0;
+            return;
+        }
+    }
+    atomicOr(overflow, 2);  // rank outside the bucket: cannot happen (the histogram passes counted these events)
+}
+
 // Writes label words.  After the eight passes st[p].prefix is the n-th smallest composite K*_p; a_ip = (K_ip <= K*_p).
 // Column c of the output: c < col_off is the observed labelling (i < n_x), else permutation c - col_off.
 // Output word for pooled event i and word index g: out[g * stride_g + pos(i) * stride_i].
