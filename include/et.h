@@ -130,7 +130,7 @@ typedef enum {
                                many permutations (default 16, at most 64; 0 = off) whose T_p lies
                                inside the guard band of T_obs, one 5/8 all-pairs pass each on the
                                CUDA cores (a full pass when weighted); skipped when more are inside  */
-    ET_OPT_DISTANCE = 3     /* distance arithmetic of the all-pairs kernel of et_T / et_T_weighted /
+    ET_OPT_DISTANCE = 3,    /* distance arithmetic of the all-pairs kernel of et_T / et_T_weighted /
                                et_T_bkg and of the escalation: 1 = differences, e = sum_k (u_ik - u_jk)^2
                                (2 dim + 1 FP32 operations per pair); 2 = Gram form, e = |u_i|^2 +
                                |u_j|^2 - 2 u_i.u_j (dim + 2 operations; psi then carries a relative
@@ -139,6 +139,11 @@ typedef enum {
                                Gram form when dim >= 4, n + nbar >= 4096 and |u|^2_max <= 48, else differences;
                                2 falls back to differences when |u|^2_max > 96 (et_stats.distance_form tells)
                                (DESIGN.md section 6).  T stays within the 1e-6 tolerance either way    */
+    ET_OPT_LABEL_SELECT = 4 /* radix select of the n-th smallest composite key of every permutation
+                               (reading R4): 0 (default) = four histogram sweeps over the key32 half, then
+                               one sweep that lists the wanted bucket's events; 1 = eight histogram sweeps
+                               (the fallback of 0 for a bucket of more than 64 events, selectable so that it
+                               can be tested).  The labels are the same bits either way                    */
 } et_option;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t to

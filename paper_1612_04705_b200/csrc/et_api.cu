@@ -71,6 +71,7 @@ struct et_ctx {
     double wmin = 1.0, wmax = 1.0;  // range of the fp32-rounded weights of the last prep (1, 1 when unweighted)
     double umax2 = 0.0;             // bound of |u|^2 over the records of the last prep: squared half diagonal of the bounding box, scaled
     int64_t opt_distance = 0;       // ET_OPT_DISTANCE
+    int64_t opt_label_select = 0;   // ET_OPT_LABEL_SELECT
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     Buf scpcnt, scpS;
     Buf selcand, selsave;  // radix select: candidate lists of the index half, state after the key32 half
@@ -484,6 +485,10 @@ et_status run_label_select(et_ctx *ctx, long long N, long long n_x, int nperm, u
         return ET_OK;
     };
     for (int pass = 0; pass < 4; ++pass) ET_TRY(hist_pass(pass));   // the key32 half of the composites
+    if (ctx->opt_label_select == 1) {
+        for (int pass = 4; pass < 8; ++pass) ET_TRY(hist_pass(pass));
+        return ET_OK;
+    }
     // the index half: one sweep lists the events of the wanted key32 bucket (about one), k_sel_finish takes the rank-th index
     ET_TRY(ensure(ctx, ctx->selcand, (size_t)nperm * (kSelCand + 1) * sizeof(uint32_t) + 16));
     unsigned int *cand_cnt = static_cast<unsigned int *>(ctx->selcand.p);
@@ -1392,6 +1397,11 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
     if (opt == ET_OPT_DISTANCE) {
         if (value < 0 || value > 2) return fail(ctx, ET_ERR_INVALID, "ET_OPT_DISTANCE must be 0, 1 or 2");
         ctx->opt_distance = value;
+        return ET_OK;
+    }
+    if (opt == ET_OPT_LABEL_SELECT) {
+        if (value < 0 || value > 1) return fail(ctx, ET_ERR_INVALID, "ET_OPT_LABEL_SELECT must be 0 or 1");
+        ctx->opt_label_select = value;
         return ET_OK;
     }
     if (opt == ET_OPT_EXACT_P) {

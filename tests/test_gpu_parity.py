@@ -183,6 +183,19 @@ def test_labels_bit_exact(ctx, N, n, nperm, seed):
     assert (bits.sum(0) == n).all()  # P10
 
 
+@pytest.mark.parametrize("N,n,nperm,seed", [(37, 11, 9, 0xE7E57), (5003, 1, 33, 7), (2049, 2048, 64, 2**63 + 5), (70001, 35000, 40, 99)])
+def test_labels_select_fallback_gives_the_same_bits(ctx, N, n, nperm, seed):
+    """ET_OPT_LABEL_SELECT = 1: the eight histogram sweeps (the fallback of the candidate-list finish for a key32 bucket of
+    more than 64 events, which no input reaches) give the oracle's labels bit for bit too."""
+    ctx.set_option(binding.ET_OPT_LABEL_SELECT, 1)
+    try:
+        got = ctx.perm_labels(N, n, nperm, seed)
+    finally:
+        ctx.set_option(binding.ET_OPT_LABEL_SELECT, 0)
+    assert (got == oracle.labels(N, n, nperm, seed)).all()
+    assert (got == ctx.perm_labels(N, n, nperm, seed)).all()
+
+
 def test_labels_large_sampled(ctx):
     """Config-4 sized label problem: every permutation has exactly n ones; a few permutations against the oracle."""
     N, n, nperm, seed = 2_000_000, 1_000_000, 96, 0xE7E57 + 4
