@@ -73,6 +73,20 @@ def test_static_matches_existing_path_on_two_calls_in_a_row(torch_dev):
         assert_close(g, oracle.T(np.asarray(hx, dtype=np.float64), np.asarray(hxb, dtype=np.float64), sg))
 
 
+@pytest.mark.parametrize("dim", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_static_all_dims_against_the_oracle(torch_dev, dim, dtype):
+    """Every instantiation of the variant kernel (dim 1..8, both input dtypes), ragged sizes around the 1024-row padding."""
+    torch = torch_dev
+    rng = np.random.default_rng(100 + dim)
+    n, nbar = 1024 + 3 * dim, 2049 - dim
+    x = rng.normal(size=(n, dim)).astype(dtype)
+    xb = (rng.normal(size=(nbar, dim)) * 1.1 + 0.1).astype(dtype)
+    sigma = 0.4 * np.sqrt(dim)
+    got = call_static(torch, torch.from_numpy(x).to("cuda:0"), torch.from_numpy(xb).to("cuda:0"), sigma)
+    assert_close(got, oracle.T(x.astype(np.float64), xb.astype(np.float64), sigma))
+
+
 def test_static_allocates_no_device_memory(torch_dev):
     torch = torch_dev
     cases = samples(torch)
