@@ -139,6 +139,12 @@ typedef enum {
                                Gram form when dim >= 4, n + nbar >= 4096 and |u|^2_max <= 48, else differences;
                                2 falls back to differences when |u|^2_max > 96 (et_stats.distance_form tells)
                                (DESIGN.md section 6).  T stays within the 1e-6 tolerance either way    */
+    ET_OPT_TC_ORDER = 5,    /* row order of the tensor-core contraction: 1 (default) = the records of every class
+                               segment in Morton order of their coordinates (a sorted copy; labels written
+                               through the inverse map; unit weights only), 0 = the layout order.  The
+                               integer sums of the unweighted contraction do not depend on it bit for bit, the
+                               time does: the board runs at its power cap and similar neighbouring rows
+                               cost the tensor pipe less energy (-2.3 % per launch at BASELINE config 4)  */
     ET_OPT_LABEL_SELECT = 4 /* radix select of the n-th smallest composite key of every permutation
                                (reading R4): 0 (default) = four histogram sweeps over the key32 half, then
                                one sweep that lists the wanted bucket's events; 1 = eight histogram sweeps

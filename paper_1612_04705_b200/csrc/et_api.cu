@@ -17,6 +17,8 @@
 #include "et_tc.cuh"
 #include "et_scp.cuh"
 
+#include <cub/device/device_radix_sort.cuh>  // library sort of (key, row) for the row order of the contraction (et_tc.cuh)
+
 using namespace et;
 
 namespace {
@@ -75,6 +77,11 @@ struct et_ctx {
     Buf maskT, units, tcpart, tcQ, tcR, tcWpart, tcW, recP, tcraw;
     Buf scpcnt, scpS;
     Buf selcand, selsave;  // radix select: candidate lists of the index half, state after the key32 half
+    // row order of the tensor-core contraction (et_tc.cuh, k_morton_keys): keys, order[new] = old, inv[old] = new, sorted records
+    Buf tckey, tckey2, tcidx, tcorder, tcinv, recS, cubtmp;
+    bool tc_sorted = false;         // maskT of the last label write is in the sorted order (tcorder / tcinv hold it)
+    int64_t opt_tc_order = 1;       // ET_OPT_TC_ORDER
+    double uhalf[ET_MAX_DIM] = {0};  // half range of the records' coordinate k over the bounding box (last prep)
     bool tc_attr_set = false;
     // NVTX ranges: the call and its spans (labels, O(N^2) kernels, escalation); ids of the open ones
     nvtxRangeId_t nvtx_call = 0, nvtx_span[8] = {0};
@@ -303,6 +310,7 @@ et_status run_prep_t(et_ctx *ctx, const TIn *x, const TIn *xbar, const double *w
     for (int k = 0; k < dim; ++k) {
         const double half = 0.5 * ((double)key2f(h[32 + 2 * k + 1]) - (double)key2f(h[32 + 2 * k])) * P.scale;
         ctx->umax2 += half * half;
+        ctx->uhalf[k] = half;
     }
     P.n = L.n; P.nbar = L.nbar; P.npad = L.npad; P.dim = dim; P.ncls = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) P.seg_pos[c] = L.seg_pos[c];
@@ -1135,6 +1143,44 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     lo.nseg = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) lo.seg_first[c] = L.seg_first[c];
     for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
+    // row order of the contraction (et_tc.cuh): Morton order inside every class segment.  With reuse_labels the order that
+    // the labels were written in is kept (the keys of another sigma could round differently).
+    // Unit weights only: there every pair enters once with a symmetric quantised psi, so the integer sums do not depend on
+    // the row order at all; with weights Psi_ij = w_j psi_ij is rounded per ordered pair and the order would show in the last
+    // bits (and the weighted 2-D configs gain nothing: 44.23 vs 44.24 ms per launch at config 3).
+    if (!reuse_labels) ctx->tc_sorted = ctx->opt_tc_order != 0 && !weighted;
+    const float *recT = static_cast<const float *>(ctx->rec.p);
+    if (ctx->tc_sorted) {
+        const int F4 = rec_floats(dim) / 4;
+        ET_TRY(ensure(ctx, ctx->tcorder, (size_t)L.npad * sizeof(int)));
+        ET_TRY(ensure(ctx, ctx->tcinv, (size_t)L.npad * sizeof(int)));
+        ET_TRY(ensure(ctx, ctx->recS, (size_t)L.npad * rec_floats(dim) * sizeof(float)));
+        if (!reuse_labels) {
+            tc::MortonParams M{};
+            M.ncls = L.ncls; M.dim = dim;
+            M.bits = std::min(28 / dim, 10);
+            for (int c = 0; c <= L.ncls; ++c) M.seg_pos[c] = L.seg_pos[c];
+            for (int c = 0; c < L.ncls; ++c) M.seg_count[c] = L.seg_count[c];
+            for (int k = 0; k < dim; ++k) M.half[k] = (float)ctx->uhalf[k];
+            ET_TRY(ensure(ctx, ctx->tckey, (size_t)L.npad * sizeof(uint32_t)));
+            ET_TRY(ensure(ctx, ctx->tckey2, (size_t)L.npad * sizeof(uint32_t)));
+            ET_TRY(ensure(ctx, ctx->tcidx, (size_t)L.npad * sizeof(int)));
+            tc::k_morton_keys<<<(unsigned)((L.npad + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
+                recT, rec_floats(dim), L.npad, M, static_cast<uint32_t *>(ctx->tckey.p), static_cast<int *>(ctx->tcidx.p));
+            LAUNCH_CHECK();
+            size_t tmp_bytes = 0;
+            CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, static_cast<const uint32_t *>(ctx->tckey.p), static_cast<uint32_t *>(ctx->tckey2.p),
+                                                     static_cast<const int *>(ctx->tcidx.p), static_cast<int *>(ctx->tcorder.p), (int)L.npad, 0, 30, ctx->stream));
+            ET_TRY(ensure(ctx, ctx->cubtmp, tmp_bytes));
+            CUDA_TRY(cub::DeviceRadixSort::SortPairs(ctx->cubtmp.p, tmp_bytes, static_cast<const uint32_t *>(ctx->tckey.p), static_cast<uint32_t *>(ctx->tckey2.p),
+                                                     static_cast<const int *>(ctx->tcidx.p), static_cast<int *>(ctx->tcorder.p), (int)L.npad, 0, 30, ctx->stream));
+            ctx->stats.launches += 3;
+        }
+        tc::k_order_gather<<<ctx->num_sms * 8, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->rec.p), static_cast<const int *>(ctx->tcorder.p), L.npad, F4,
+                                                                    static_cast<int *>(ctx->tcinv.p), static_cast<float4 *>(ctx->recS.p));
+        LAUNCH_CHECK();
+        recT = static_cast<const float *>(ctx->recS.p);
+    }
     if (!reuse_labels) {
         ET_TRY(run_label_select(ctx, L.N, L.n_a, nperm, seed));
         ET_TRY(ensure(ctx, ctx->maskT, (size_t)npadK * words_total * sizeof(uint32_t)));
@@ -1142,7 +1188,8 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         const dim3 grid((unsigned)((L.N + kThreads - 1) / kThreads), (unsigned)words_total);
         tc::k_label_write_tc<<<grid, kThreads, 0, ctx->stream>>>(L.N, L.n_a, nperm, ctx->opt_perm_offset, (uint32_t)(seed & 0xffffffffu),
                                                                 (uint32_t)(seed >> 32), static_cast<const SelState *>(ctx->sel.p), lo,
-                                                                lab2_classes, words_total, static_cast<uint32_t *>(ctx->maskT.p));
+                                                                lab2_classes, words_total, ctx->tc_sorted ? static_cast<const int *>(ctx->tcinv.p) : nullptr,
+                                                                static_cast<uint32_t *>(ctx->maskT.p));
         LAUNCH_CHECK();
     }
     ET_TRY(span_end(ctx, 4, &ctx->acc_labels_ms));
@@ -1202,12 +1249,12 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     ET_TRY(ensure(ctx, ctx->recP, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4)));
     CUDA_TRY(cudaMemsetAsync(ctx->recP.p, 0, (size_t)(npadK / 2) * tc::pair_rec_f4(dim) * sizeof(float4), ctx->stream));
     DISPATCH_DIM(dim, (tc::k_pair_records<D><<<(unsigned)((L.npad / 2 + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
-                          static_cast<const float *>(ctx->rec.p), L.npad / 2, scf, static_cast<float4 *>(ctx->recP.p))));
+                          recT, L.npad / 2, scf, static_cast<float4 *>(ctx->recP.p))));
     LAUNCH_CHECK();
     long long cols_algo = 0, cols_exec = 0;
     for (int ch = 0; ch < nchunks; ++ch) {
         tc::TCParams P{};
-        P.rec = static_cast<const float *>(ctx->rec.p);
+        P.rec = recT;
         P.maskT = static_cast<const uint32_t *>(ctx->maskT.p);
         P.words_total = words_total;
         P.word0 = ch * tc::kWordsPerChunk;
@@ -1265,7 +1312,7 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         LAUNCH_CHECK();
     } else {
         const dim3 gridW((unsigned)nchunkW, (unsigned)words_total);
-        tc::k_perm_W_tc<<<gridW, kThreads, 0, ctx->stream>>>(static_cast<const float *>(ctx->rec.p), rec_floats(dim), dim,
+        tc::k_perm_W_tc<<<gridW, kThreads, 0, ctx->stream>>>(recT, rec_floats(dim), dim,
                                                             static_cast<const uint32_t *>(ctx->maskT.p), words_total, L.npad, nchunkW,
                                                             static_cast<double *>(ctx->tcWpart.p));
         LAUNCH_CHECK();
@@ -1367,7 +1414,8 @@ void et_destroy(et_ctx *ctx)
                    &ctx->blkcnt, &ctx->totals, &ctx->clsw, &ctx->clssum, &ctx->result, &ctx->tperm, &ctx->rows, &ctx->rowsout,
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
                    &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
-                   &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave};
+                   &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave, &ctx->tckey, &ctx->tckey2, &ctx->tcidx, &ctx->tcorder,
+                   &ctx->tcinv, &ctx->recS, &ctx->cubtmp};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
@@ -1397,6 +1445,11 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
     if (opt == ET_OPT_DISTANCE) {
         if (value < 0 || value > 2) return fail(ctx, ET_ERR_INVALID, "ET_OPT_DISTANCE must be 0, 1 or 2");
         ctx->opt_distance = value;
+        return ET_OK;
+    }
+    if (opt == ET_OPT_TC_ORDER) {
+        if (value < 0 || value > 1) return fail(ctx, ET_ERR_INVALID, "ET_OPT_TC_ORDER must be 0 or 1");
+        ctx->opt_tc_order = value;
         return ET_OK;
     }
     if (opt == ET_OPT_LABEL_SELECT) {

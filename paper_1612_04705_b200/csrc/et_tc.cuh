@@ -39,6 +39,7 @@ constexpr int kSpecial = 3;              // observed, second labelling, ones
 constexpr int kPermsPerChunk = kCols - kSpecial;
 constexpr int kWordsPerChunk = kCols / 32;
 constexpr int kMaxRecSlots = 4;
+constexpr int kMaxDimTC = 8;          // = ET_MAX_DIM (include/et.h)
 // float4 per pair record: dim + 1 float2 entries, padded to an even count
 __host__ __device__ constexpr int pair_rec_f4(int dim) { return (dim + 2) / 2; }
 
@@ -771,7 +772,8 @@ __global__ void k_tc_scale(const void *raw, double inv_sc, double *__restrict__ 
 // c >= 3 permutation p = ch * 509 + c - 3 (local index; global p0 + p) if p < nperm.  grid = (events, chunks * 16).
 __global__ void __launch_bounds__(kThreads) k_label_write_tc(long long N, long long n_x, int nperm, long long p0, uint32_t seed_lo,
                                                             uint32_t seed_hi, const SelState *__restrict__ st, LabelOut L,
-                                                            unsigned lab2_classes, int words_total, uint32_t *__restrict__ maskT)
+                                                            unsigned lab2_classes, int words_total, const int *__restrict__ inv,
+                                                            uint32_t *__restrict__ maskT)
 {
     const long long i = blockIdx.x * (long long)kThreads + threadIdx.x;
     const int ch = blockIdx.y / kWordsPerChunk, W = blockIdx.y % kWordsPerChunk;
@@ -794,7 +796,58 @@ __global__ void __launch_bounds__(kThreads) k_label_write_tc(long long N, long l
         if ((pg >> 2) != have_p4) { have_p4 = pg >> 2; label_keys4((uint32_t)i, (uint32_t)have_p4, seed_lo, seed_hi, K); }
         if (K[pg & 3] <= st[p].prefix) word |= 1u << b;
     }
+    if (inv) pos = inv[pos];  // row of the contraction's own order (k_morton_keys)
     maskT[pos * words_total + blockIdx.y] = word;
+}
+
+// ---- row order of the contraction -----------------------------------------------------------------------------------
+// The sums of k_perm_tc do not depend on the order of the rows inside a class segment (unit weights: bit for bit, every
+// pair enters once with a symmetric quantised psi), but its TIME does: the board runs at its power cap and the energy of
+// an MMA follows the operand bits -- with neighbouring rows close in phase space the digit tiles of neighbouring j are
+// alike and far tiles are mostly zero: -2.3 % per launch at config 4 (profiles/r02_README.md).  So the contraction
+// runs on a copy of the records in Morton order: key = class << 28 | interleaved bits of the coordinates quantised over the
+// bounding box (padding rows: the largest key of their class, so every class keeps its row range), a stable sort of
+// (key, row), then order[new] = old, inv[old] = new and recS[new] = rec[old].  The labels are written through inv; the
+// escalation and every other kernel keep the layout order.
+struct MortonParams {
+    int ncls, dim, bits;
+    long long seg_pos[kMaxCls + 1], seg_count[kMaxCls];
+    float half[kMaxDimTC];  // half range of u_k over the bounding box (0: a degenerate axis)
+};
+__global__ void __launch_bounds__(kThreads) k_morton_keys(const float *__restrict__ rec, int F, long long npad, MortonParams M,
+                                                         uint32_t *__restrict__ key, int *__restrict__ idx)
+{
+    const long long row = blockIdx.x * (long long)kThreads + threadIdx.x;
+    if (row >= npad) return;
+    int cls = 0;
+    for (int c = 0; c < M.ncls; ++c)
+        if (row >= M.seg_pos[c]) cls = c;
+    uint32_t m = 0x0fffffffu;
+    if (row - M.seg_pos[cls] < M.seg_count[cls]) {
+        uint32_t q[kMaxDimTC];
+        const int top = (1 << M.bits) - 1;
+        for (int k = 0; k < M.dim; ++k) {
+            const float h = M.half[k];
+            const float t = h > 0.f ? (rec[row * F + k] + h) / (2.f * h) * (float)(1 << M.bits) : 0.f;
+            q[k] = (uint32_t)min(max((int)t, 0), top);
+        }
+        m = 0u;
+        for (int b = M.bits - 1; b >= 0; --b)
+            for (int k = 0; k < M.dim; ++k) m = (m << 1) | ((q[k] >> b) & 1u);
+    }
+    key[row] = ((uint32_t)cls << 28) | m;
+    idx[row] = (int)row;
+}
+// inv[order[r]] = r, recS[r] = rec[order[r]] (F4 float4 per row); one thread per float4
+__global__ void k_order_gather(const float4 *__restrict__ rec, const int *__restrict__ order, long long npad, int F4, int *__restrict__ inv,
+                               float4 *__restrict__ recS)
+{
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < npad * F4; k += (long long)gridDim.x * blockDim.x) {
+        const long long r = k / F4;
+        const int q = (int)(k % F4), old = order[r];
+        if (q == 0) inv[old] = (int)r;
+        recS[k] = rec[(long long)old * F4 + q];
+    }
 }
 
 // W_c = sum_i a_ic w_i for every column of the TC layout.  grid = (row chunks, words_total); lane = bit.

@@ -344,6 +344,31 @@ def test_perm_tc_is_bit_reproducible(ctx):
     assert (a.T_perm == b.T_perm).all() and a.observed.T == b.observed.T
 
 
+def test_perm_tc_row_order_does_not_change_the_sums(ctx):
+    """ET_OPT_TC_ORDER: the contraction runs on a Morton-ordered copy of the records (labels written through the inverse
+    map); the unweighted integer sums, hence every T_p, T_obs and the P-even T of the Sect. 5 test, are the same bits in
+    the layout order.  5-D four-body sample (both geometries' dims: 5 and 6 by zero-padding a coordinate), P-odd split."""
+    c = dg.config(4, scale=0.012)
+    s = dg.make_sample(c)
+    res = {}
+    for order in (1, 0):
+        ctx.set_option(binding.ET_OPT_TC_ORDER, order)
+        try:
+            with force_kernel(ctx, 2):
+                res[order] = (ctx.podd_test(s.x, s.mom_x, s.xbar, s.mom_xbar, c.sigma, 40, c.perm_seed),
+                              ctx.permutation_test(np.c_[s.x, 0.3 * s.x[:, :1]], np.c_[s.xbar, 0.3 * s.xbar[:, :1]], c.sigma, 520, 7))
+                assert ctx.stats().dominant_kernel == "k_perm_tc"
+        finally:
+            ctx.set_option(binding.ET_OPT_TC_ORDER, 1)
+    (pa, ta), (pb, tb) = res[1], res[0]
+    assert (pa.p_odd.T_perm == pb.p_odd.T_perm).all() and pa.p_odd.observed == pb.p_odd.observed and pa.p_even == pb.p_even
+    assert (ta.T_perm == tb.T_perm).all() and ta.observed == tb.observed and ta.count_gt == tb.count_gt
+    # and the sorted run is the oracle's answer (the 6-D sample: 8 permutations from scratch)
+    exp = oracle.perm_test(np.c_[s.x, 0.3 * s.x[:, :1]], np.c_[s.xbar, 0.3 * s.xbar[:, :1]], c.sigma, 8, 7)
+    assert abs(ta.observed.T - exp.observed.T) <= TOL * exp.observed.term_scale
+    assert np.abs(ta.T_perm[:8] - exp.T_perm).max() <= TOL * exp.observed.term_scale
+
+
 def test_perm_tc_weighted(ctx):
     c = dg.config(3, scale=0.012)  # 2400 + 2400 events, weights U[-0.5, 1.5]: signed hi digit
     s = dg.make_sample(c)
