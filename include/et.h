@@ -100,7 +100,8 @@ typedef struct {
     int64_t dominant_launches;
     int64_t dominant_ops;      /* ALGORITHMIC work of those launches: FP32-pipe thread instructions
                                   (CUDA-core kernels: unique pairs x (2 dim + 1), per mask word
-                                  unique pairs x (2 dim + 32)) or 2 x MACs (tensor-core kernel)     */
+                                  unique pairs x (2 dim + 32)) or 2 x MACs (tensor-core kernel; with
+                                  ET_OPT_TC_SKIP in force: of the K blocks that were evaluated)       */
     char dominant_kernel[32];  /* "k_pairs_T", "k_pairs_rows", "k_perm32", "k_perm_tc" or ""       */
     int64_t dominant_ops_executed; /* k_perm_tc: the same count over the label columns the launches
                                   carried (256 or 512 per launch, the three special columns in every
@@ -145,6 +146,10 @@ typedef enum {
                                integer sums of the unweighted contraction do not depend on it bit for bit, the
                                time does: the board runs at its power cap and similar neighbouring rows
                                cost the tensor pipe less energy (-2.3 % per launch at BASELINE config 4)  */
+    ET_OPT_TC_SKIP = 6,     /* exact skipping of far K blocks in the tensor-core contraction (needs ET_OPT_TC_ORDER):
+                               1 (default) = (row tile, K block) pairs whose bounding boxes are farther apart than
+                               the distance at which the 15-bit psi rounds to 0 (4.7 sigma) are not evaluated,
+                               when that is at least 5 % of the blocks; 0 = every block.  Same sums bit for bit   */
     ET_OPT_LABEL_SELECT = 4 /* radix select of the n-th smallest composite key of every permutation
                                (reading R4): 0 (default) = four histogram sweeps over the key32 half, then
                                one sweep that lists the wanted bucket's events; 1 = eight histogram sweeps

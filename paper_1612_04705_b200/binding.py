@@ -26,6 +26,7 @@ ET_OPT_EXACT_P = 2
 ET_OPT_DISTANCE = 3
 ET_OPT_LABEL_SELECT = 4
 ET_OPT_TC_ORDER = 5
+ET_OPT_TC_SKIP = 6
 STATUS_NAMES = {0: "ET_OK", -1: "ET_ERR_INVALID", -2: "ET_ERR_SIGMA", -3: "ET_ERR_NONFINITE", -4: "ET_ERR_DEGENERATE",
                 -5: "ET_ERR_NOMEM", -6: "ET_ERR_CUDA"}
 

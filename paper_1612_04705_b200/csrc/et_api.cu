@@ -79,6 +79,8 @@ struct et_ctx {
     Buf selcand, selsave;  // radix select: candidate lists of the index half, state after the key32 half
     // row order of the tensor-core contraction (et_tc.cuh, k_morton_keys): keys, order[new] = old, inv[old] = new, sorted records
     Buf tckey, tckey2, tcidx, tcorder, tcinv, recS, cubtmp;
+    Buf tcboxes, tcbitmap;          // exact skipping of far K blocks: bounding boxes, bitmap[row tile][K block]
+    int64_t opt_tc_skip = 1;        // ET_OPT_TC_SKIP
     bool tc_sorted = false;         // maskT of the last label write is in the sorted order (tcorder / tcinv hold it)
     int64_t opt_tc_order = 1;       // ET_OPT_TC_ORDER
     double uhalf[ET_MAX_DIM] = {0};  // half range of the records' coordinate k over the bounding box (last prep)
@@ -1042,9 +1044,12 @@ __global__ void __launch_bounds__(256) k_esc_apply(const DevNear *__restrict__ n
 }
 
 template <int D, class G>
-et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted)
+et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted, bool skip)
 {
-    if (weighted) {
+    if (!weighted && skip) {  // far K blocks are not evaluated (et_tc.cuh, SKIP)
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
+        tc::k_perm_tc<D, false, G, true><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
+    } else if (weighted) {
         CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
         tc::k_perm_tc<D, true, G><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
     } else {
@@ -1204,6 +1209,34 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     auto first_kb = [](int I) { return (long long)I * tc::kTM2 / G::kKB; };  // K block that holds the tile's first row
     long long total_kb = 0;
     for (int I = 0; I < nT; ++I) total_kb += NK - first_kb(I);
+    // Exact skipping of far K blocks (et_tc.cuh): with the rows in Morton order, mark for every row tile the K blocks whose
+    // bounding box is within the distance at which a quantised Psi can be non-zero; the SKIP kernel walks the marked ones
+    // only.  Taken when at least 5 % of the blocks are unmarked (BASELINE config 4: < 1 %, the plain kernel runs).
+    bool use_skip = false;
+    const int bm_words = (NK + 31) / 32;
+    long long marked_kb = total_kb;
+    if (ctx->tc_sorted && ctx->opt_tc_skip != 0) {
+        const int F = rec_floats(dim);
+        ET_TRY(ensure(ctx, ctx->tcboxes, ((size_t)nT + (size_t)NK) * 2 * tc::kMaxDimTC * sizeof(float)));
+        ET_TRY(ensure(ctx, ctx->tcbitmap, (size_t)nT * bm_words * sizeof(uint32_t) + 16));
+        float *tlo = static_cast<float *>(ctx->tcboxes.p), *thi = tlo + (size_t)nT * tc::kMaxDimTC;
+        float *klo = thi + (size_t)nT * tc::kMaxDimTC, *khi = klo + (size_t)NK * tc::kMaxDimTC;
+        unsigned long long *marked = reinterpret_cast<unsigned long long *>(static_cast<uint32_t *>(ctx->tcbitmap.p) + (size_t)nT * bm_words + ((size_t)nT * bm_words & 1));
+        tc::k_row_boxes<<<(unsigned)((nT + 7) / 8), kThreads, 0, ctx->stream>>>(recT, F, dim, L.npad, tc::kTM2, nT, tlo, thi);
+        LAUNCH_CHECK();
+        tc::k_row_boxes<<<(unsigned)((NK + 7) / 8), kThreads, 0, ctx->stream>>>(recT, F, dim, L.npad, G::kKB, NK, klo, khi);
+        LAUNCH_CHECK();
+        CUDA_TRY(cudaMemsetAsync(marked, 0, sizeof(unsigned long long), ctx->stream));
+        tc::k_tile_bitmap<<<(unsigned)nT, kThreads, 0, ctx->stream>>>(tlo, thi, klo, khi, dim, NK, G::kKB, bm_words,
+                                                                    static_cast<uint32_t *>(ctx->tcbitmap.p), marked);
+        LAUNCH_CHECK();
+        unsigned long long m = 0;
+        ET_TRY(ensure_pinned(ctx, 4096));
+        CUDA_TRY(cudaMemcpyAsync(ctx->pinned, marked, sizeof(m), cudaMemcpyDeviceToHost, ctx->stream));
+        CUDA_TRY(cudaStreamSynchronize(ctx->stream));
+        memcpy(&m, ctx->pinned, sizeof(m));
+        if ((double)m < 0.95 * (double)total_kb) { use_skip = true; marked_kb = (long long)m; }
+    }
     // about 24 units per cluster and rank (ranks of a unit-range shard take every world-th unit of the same table)
     const long long nshare = (long long)nclusters_max * 24 * ctx->shard_world;
     long long Lmax = (total_kb + nshare - 1) / nshare;
@@ -1271,7 +1304,9 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         cols_algo += ch == 0 ? cols_used : cols_used - tc::kSpecial;  // the special columns are algorithmic work once
         cols_exec += 256 * P.nq;
         P.partial = ctx->tcpart.p;
-        DISPATCH_DIM(dim, ET_TRY((launch_perm_tc<D, G>(ctx, P, grid, weighted))));
+        P.bitmap = use_skip ? static_cast<const uint32_t *>(ctx->tcbitmap.p) : nullptr;
+        P.bm_words = bm_words;
+        DISPATCH_DIM(dim, ET_TRY((launch_perm_tc<D, G>(ctx, P, grid, weighted, use_skip))));
         // the scale actually applied is the fp32 value of 256 sc
         const double inv_sc = 256.0 / (double)P.sc256;
         if (weighted) tc::k_tc_reduce<true, G><<<2, 256, 0, ctx->stream>>>(ctx->tcpart.p, grid, ctx->tcraw.p);
@@ -1291,9 +1326,11 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         // algorithmic work (et.h): 2 digits x 2 ops per (pair, label column) over the columns the test needs -- the
         // permutations plus observed / second labelling / ones once; the executed count (padded accumulators, the
         // special columns repeated in every chunk) is kept beside it
-        ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, 2ll * 2 * pairs * cols_algo));
-        ctx->stats.dominant_ops_executed = 2ll * 2 * pairs * cols_exec;
-        ctx->stats.pair_evals += (long long)nchunks * total_kb * tc::kTM2 * G::kKB;
+        // with far K blocks skipped the work is that of the evaluated blocks (the rest is known to be exactly zero)
+        const double evaluated = use_skip ? (double)marked_kb / (double)total_kb : 1.0;
+        ET_TRY(span_end(ctx, 2, &ctx->acc_pairs_ms, KC_PERMTC, nchunks, (int64_t)(2.0 * 2 * (double)pairs * (double)cols_algo * evaluated)));
+        ctx->stats.dominant_ops_executed = (int64_t)(2.0 * 2 * (double)pairs * (double)cols_exec * evaluated);
+        ctx->stats.pair_evals += (long long)nchunks * (use_skip && ctx->shard_world == 1 ? marked_kb : total_kb) * tc::kTM2 * G::kKB;
     }
 
     // W_c
@@ -1415,7 +1452,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
                    &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
                    &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave, &ctx->tckey, &ctx->tckey2, &ctx->tcidx, &ctx->tcorder,
-                   &ctx->tcinv, &ctx->recS, &ctx->cubtmp};
+                   &ctx->tcinv, &ctx->recS, &ctx->cubtmp, &ctx->tcboxes, &ctx->tcbitmap};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
@@ -1445,6 +1482,11 @@ et_status et_set_option(et_ctx *ctx, et_option opt, int64_t value)
     if (opt == ET_OPT_DISTANCE) {
         if (value < 0 || value > 2) return fail(ctx, ET_ERR_INVALID, "ET_OPT_DISTANCE must be 0, 1 or 2");
         ctx->opt_distance = value;
+        return ET_OK;
+    }
+    if (opt == ET_OPT_TC_SKIP) {
+        if (value < 0 || value > 1) return fail(ctx, ET_ERR_INVALID, "ET_OPT_TC_SKIP must be 0 or 1");
+        ctx->opt_tc_skip = value;
         return ET_OK;
     }
     if (opt == ET_OPT_TC_ORDER) {

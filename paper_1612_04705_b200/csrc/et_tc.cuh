@@ -363,13 +363,30 @@ struct TCParams {
     uint32_t idesc_hi;       // hi digit: s8 when weights can be negative, else u8
     int nq;                  // 256-column accumulators in use: 2, or 1 when this launch has <= 256 label columns
     void *partial;           // [gridDim.x][GEO::kProducerWarps][GEO::kEpiGroups][32 lanes][2] of Acc
+    const uint32_t *bitmap;  // SKIP: bit kb of word row I = K block kb can hold a non-zero quantised Psi for row tile I (k_tile_bitmap)
+    int bm_words;            // words per row tile
 };
+
+// SKIP: the K blocks of a unit that the bitmap marks, in ascending order -- every role of k_perm_tc walks the same list
+// (a unit without a marked block is skipped by every role, barriers and phases untouched).
+__device__ __forceinline__ int next_kb(const uint32_t *__restrict__ bmI, int kb, int end)
+{
+    while (kb < end) {
+        const uint32_t w = __ldg(bmI + (kb >> 5)) >> (kb & 31);
+        if (w) {
+            kb += __ffs((int)w) - 1;
+            return kb < end ? kb : end;
+        }
+        kb = (kb | 31) + 1;
+    }
+    return end;
+}
 
 // One launch = 512 label columns.  Grid: persistent, one CTA per SM, clusters of 2 (an SM pair); unit u is processed
 // by cluster u % (gridDim.x / 2).  CTA rank r of the pair owns rows 256 I + 128 r .. + 127 (its psi tile, its half of
 // the accumulator rows in its own TMEM) and the label columns [256 q + 128 r, 256 q + 128 r + 128), q = 0, 1.
 // WEIGHTED: accumulate w_i Y in double; else exact int64.
-template <int D, bool WEIGHTED, class GEO>
+template <int D, bool WEIGHTED, class GEO, bool SKIP = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) k_perm_tc(TCParams P)
 {
     using Acc = typename std::conditional<WEIGHTED, double, long long>::type;
@@ -420,11 +437,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         if (rank == 0 && lane == 0) {
             const uint32_t idesc_lo = umma_idesc_i8(false), idesc_hi = P.idesc_hi;
             uint32_t it = 0, un = 0;
-            for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
+            for (int u = cluster_id; u < P.nunits; u += nclusters) {
                 const Unit U = P.units[u];
+                const uint32_t *bmI = SKIP ? P.bitmap + (long long)U.I * P.bm_words : nullptr;
+                const int kb_first = SKIP ? next_kb(bmI, U.kb_begin, U.kb_end) : U.kb_begin;
+                if (SKIP && kb_first >= U.kb_end) continue;      // nothing marked: no role touches this unit
                 mbar_wait_cluster(&bar_accempty, (un & 1) ^ 1);  // both epilogues of the previous unit have drained TMEM
                 tc_fence_after();
-                for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+                for (int kb = kb_first; kb < U.kb_end; kb = SKIP ? next_kb(bmI, kb + 1, U.kb_end) : kb + 1, ++it) {
                     const int s = it % kStages;
                     mbar_wait_cluster(&bar_full[s], (it / kStages) & 1);
                     tc_fence_after();
@@ -440,13 +460,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
                                 // A digit tile: K chunks of 32 bytes, each a [128 rows x 32 B] SWIZZLE_32B sub-tile
                                 const uint64_t da = umma_desc(a_base + d * (kTM * kKB) + ks * (kTM * 32), 16, 256, 6);
                                 const uint64_t db = umma_desc(b_base + (q * 2 + d) * kBPlane + ks * 4 * 1024, kBPlane, 1024, 2);
-                                const uint32_t acc = (kb > U.kb_begin || d > 0 || ks > 0) ? 1u : 0u;
+                                const uint32_t acc = (kb > kb_first || d > 0 || ks > 0) ? 1u : 0u;
                                 umma_i8_pair(tmem + q * 256, da, db, d == 0 ? idesc_hi : idesc_lo, acc);
                             }
                     }
                     umma_commit_pair(&bar_empty[s]);  // frees the stage in both CTAs when these MMAs have read it
                 }
                 umma_commit_pair(&bar_accfull);
+                ++un;
             }
         }
     } else if (warp == kProducerWarps + 1) {
@@ -459,7 +480,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
             uint32_t it = 0;
             for (int u = cluster_id; u < P.nunits; u += nclusters) {
                 const Unit U = P.units[u];
-                for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+                const uint32_t *bmI = SKIP ? P.bitmap + (long long)U.I * P.bm_words : nullptr;
+                for (int kb = SKIP ? next_kb(bmI, U.kb_begin, U.kb_end) : U.kb_begin; kb < U.kb_end;
+                     kb = SKIP ? next_kb(bmI, kb + 1, U.kb_end) : kb + 1, ++it) {
                     const uint32_t slot = it & (kRecSlots - 1);
                     if (it >= kRecSlots) mbar_wait(&bar_recfree[slot], ((it / kRecSlots) - 1) & 1);
                     bulk_g2s(smem_u32(recs + slot * kRecSlotBytes), P.recP + (long long)kb * (kKB / 2) * NLD, kRecSlotBytes, &bar_rec[slot]);
@@ -500,8 +523,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         const uint32_t bar0 = smem_u32(bars_s);
         uint32_t paA = smem_u32(smem) + offA, pbB = smem_u32(smem) + offB, pjJ = smem_u32(smem) + offJ;
         uint32_t it = 0, un = 0, st = 0, pe = 0;   // K blocks done, units done, stage index it % kStages, its phase (it / kStages) & 1
-        for (int u = cluster_id; u < P.nunits; u += nclusters, ++un) {
+        for (int u = cluster_id; u < P.nunits; u += nclusters) {
             const Unit U = P.units[u];
+            const uint32_t *bmI = SKIP ? P.bitmap + (long long)U.I * P.bm_words : nullptr;
+            const int kb_first = SKIP ? next_kb(bmI, U.kb_begin, U.kb_end) : U.kb_begin;
+            if (SKIP && kb_first >= U.kb_end) continue;      // nothing marked: no role touches this unit
             const int row0 = U.I * kTM2 + (int)rank * kTM;   // npad < 2^31
             // this thread's i rows; the packed FP32 instructions take (u_ik, u_ik) as a scalar-broadcast operand (R.F32 in SASS)
             float2 ui2[R][D];
@@ -525,12 +551,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
             // this thread's label words of K block kb, prefetched one block ahead into registers.  The element index is
             // 64 bits wide: npadK * words_total passes 2^32 at 2 M pooled rows with the maximum permutation count.
             // (the word of the second accumulator, q = 1, is expanded by the helper warps)
-            unsigned long long im = (unsigned long long)(U.kb_begin * kKB + jj) * (unsigned)P.words_total + (unsigned)(P.word0 + 4 * (int)rank + l3);
+            unsigned long long im = (unsigned long long)(kb_first * kKB + jj) * (unsigned)P.words_total + (unsigned)(P.word0 + 4 * (int)rank + l3);
             uint32_t mw = __ldg(P.maskT + im);
-            for (int kb = U.kb_begin; kb < U.kb_end; ++kb, ++it) {
+            int kb_next = 0;
+            for (int kb = kb_first; kb < U.kb_end; kb = kb_next, ++it) {
                 const uint32_t mcur = mw;
-                if (kb + 1 < U.kb_end) {
-                    im += (unsigned)(kKB * P.words_total);
+                kb_next = SKIP ? next_kb(bmI, kb + 1, U.kb_end) : kb + 1;
+                if (kb_next < U.kb_end) {
+                    im += (unsigned long long)(unsigned)((kb_next - kb) * kKB) * (unsigned)P.words_total;
                     mw = __ldg(P.maskT + im);
                 }
                 mbar_wait_a(bar0 + 8 * (2 * kStages + 2) + 8 * (it & (kRecSlots - 1)), (it / kRecSlots) & 1);
@@ -656,6 +684,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(mapa_rank(smem_u32(&bar_accempty), 0));
+            ++un;
         }
         // per-warp partial column sums: partial[cta][warp][g][lane][2]; lane L of group g = TMEM column 32 (grp0 + g) + L
         Acc *out = reinterpret_cast<Acc *>(P.partial) + ((long long)blockIdx.x * kProducerWarps + warp) * G * 32 * 2;
@@ -679,19 +708,23 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEO::kThreadsTC, 1) 
         const unsigned long long jstride = 8ull * (unsigned)P.words_total;
         for (int u = cluster_id; u < P.nunits; u += nclusters) {
             const Unit U = P.units[u];
-            unsigned long long im = (unsigned long long)(U.kb_begin * kKB + 8 * NW * h + jsub) * (unsigned)P.words_total +
+            const uint32_t *bmI = SKIP ? P.bitmap + (long long)U.I * P.bm_words : nullptr;
+            const int kb_first = SKIP ? next_kb(bmI, U.kb_begin, U.kb_end) : U.kb_begin;
+            unsigned long long im = (unsigned long long)(kb_first * kKB + 8 * NW * h + jsub) * (unsigned)P.words_total +
                                     (unsigned)(P.word0 + 8 + 4 * (int)rank + l3);
             uint32_t mw[NW];
-            if (U.kb_begin < U.kb_end) {
+            if (kb_first < U.kb_end) {
 #pragma unroll
                 for (int i = 0; i < NW; ++i) mw[i] = __ldg(P.maskT + im + i * jstride);
             }
-            for (int kb = U.kb_begin; kb < U.kb_end; ++kb) {
+            int kb_next = 0;
+            for (int kb = kb_first; kb < U.kb_end; kb = kb_next) {
                 uint32_t cur[NW];
 #pragma unroll
                 for (int i = 0; i < NW; ++i) cur[i] = mw[i];
-                if (kb + 1 < U.kb_end) {
-                    im += (unsigned)(kKB * P.words_total);
+                kb_next = SKIP ? next_kb(bmI, kb + 1, U.kb_end) : kb + 1;
+                if (kb_next < U.kb_end) {
+                    im += (unsigned long long)(unsigned)((kb_next - kb) * kKB) * (unsigned)P.words_total;
 #pragma unroll
                     for (int i = 0; i < NW; ++i) mw[i] = __ldg(P.maskT + im + i * jstride);
                 }
@@ -848,6 +881,70 @@ __global__ void k_order_gather(const float4 *__restrict__ rec, const int *__rest
         if (q == 0) inv[old] = (int)r;
         recS[k] = rec[(long long)old * F4 + q];
     }
+}
+
+// ---- exact skipping of far K blocks (SKIP) -------------------------------------------------------------------------
+// v = floor(sc Psi + 1/2) is 0 for every pair with |u_i - u_j|^2 > log2(2 sc) = 16.0 (unit weights), i.e. farther apart than
+// 4.7 sigma: a (row tile, K block) pair whose bounding boxes are farther apart than that contributes exactly nothing to
+// any integer sum and is not evaluated at all -- no psi, no labels, no MMAs; the sums stay the same bits.  It pays where
+// the sample is wide in units of sigma and the rows are in Morton order (the Dalitz plot at sigma = 0.1: 59 % of the K
+// blocks); run_perm_tc_g takes the SKIP kernel only when the bitmap marks less than 95 % of the blocks.
+// Bounding boxes of consecutive groups of `rows_per_box` rows (real rows only: weight != 0); one warp per box.
+constexpr float kSkipDist2 = 16.1f;  // > log2(65532) = 15.99998 with room for the fp32 rounding of the distance and of ex2.approx
+__global__ void __launch_bounds__(kThreads) k_row_boxes(const float *__restrict__ rec, int F, int dim, long long nrows, int rows_per_box,
+                                                       long long nboxes, float *__restrict__ lo, float *__restrict__ hi)
+{
+    const long long box = blockIdx.x * (long long)(kThreads / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (box >= nboxes) return;
+    float a[kMaxDimTC], b[kMaxDimTC];
+#pragma unroll
+    for (int k = 0; k < kMaxDimTC; ++k) { a[k] = 3.0e38f; b[k] = -3.0e38f; }
+    for (int r = lane; r < rows_per_box; r += 32) {
+        const long long row = box * rows_per_box + r;
+        if (row >= nrows || rec[row * F + dim] == 0.f) continue;
+#pragma unroll
+        for (int k = 0; k < kMaxDimTC; ++k)
+            if (k < dim) { const float v = rec[row * F + k]; a[k] = fminf(a[k], v); b[k] = fmaxf(b[k], v); }
+    }
+#pragma unroll
+    for (int k = 0; k < kMaxDimTC; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a[k] = fminf(a[k], __shfl_xor_sync(0xffffffffu, a[k], o));
+            b[k] = fmaxf(b[k], __shfl_xor_sync(0xffffffffu, b[k], o));
+        }
+        if (lane == 0) { lo[box * kMaxDimTC + k] = a[k]; hi[box * kMaxDimTC + k] = b[k]; }
+    }
+}
+// bitmap[I][kb >> 5] bit kb & 31 = the boxes of row tile I and K block kb are within kSkipDist2 (and kb is not below the
+// tile's first block); marked += the number of marked blocks.  grid = row tiles, block = kThreads.
+__global__ void __launch_bounds__(kThreads) k_tile_bitmap(const float *__restrict__ tlo, const float *__restrict__ thi, const float *__restrict__ klo,
+                                                         const float *__restrict__ khi, int dim, int NK, int kKB, int bm_words,
+                                                         uint32_t *__restrict__ bitmap, unsigned long long *__restrict__ marked)
+{
+    const int I = blockIdx.x, lane = threadIdx.x & 31;
+    const int kb0 = (int)((long long)I * kTM2 / kKB);
+    float a[kMaxDimTC], b[kMaxDimTC];
+#pragma unroll
+    for (int k = 0; k < kMaxDimTC; ++k) { a[k] = tlo[(long long)I * kMaxDimTC + k]; b[k] = thi[(long long)I * kMaxDimTC + k]; }
+    unsigned int cnt = 0;
+    for (int kb = threadIdx.x; kb < bm_words * 32; kb += kThreads) {
+        bool need = false;
+        if (kb >= kb0 && kb < NK) {
+            float d2 = 0.f;
+#pragma unroll
+            for (int k = 0; k < kMaxDimTC; ++k)
+                if (k < dim) {
+                    const float g = fmaxf(0.f, fmaxf(klo[(long long)kb * kMaxDimTC + k] - b[k], a[k] - khi[(long long)kb * kMaxDimTC + k]));
+                    d2 = fmaf(g, g, d2);
+                }
+            need = d2 <= kSkipDist2;   // an empty box (3e38 / -3e38) gives inf: not needed
+        }
+        const unsigned int w = __ballot_sync(0xffffffffu, need);
+        if (lane == 0) { bitmap[(long long)I * bm_words + (kb >> 5)] = w; cnt += __popc(w); }
+    }
+    if (lane == 0 && cnt) atomicAdd(marked, (unsigned long long)cnt);
 }
 
 // W_c = sum_i a_ic w_i for every column of the TC layout.  grid = (row chunks, words_total); lane = bit.

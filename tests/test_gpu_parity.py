@@ -369,6 +369,32 @@ def test_perm_tc_row_order_does_not_change_the_sums(ctx):
     assert np.abs(ta.T_perm[:8] - exp.T_perm).max() <= TOL * exp.observed.term_scale
 
 
+@pytest.mark.parametrize("sigma,nperm", [(0.1, 40), (0.05, 520)])
+def test_perm_tc_skipping_far_blocks_does_not_change_the_sums(ctx, sigma, nperm):
+    """ET_OPT_TC_SKIP: (row tile, K block) pairs beyond the distance at which the 15-bit psi rounds to 0 are not evaluated.
+    Dalitz sample at a small sigma (the plot is many sigma wide): most blocks are skipped, and T_obs and every T_p are the
+    same bits as with every block evaluated; the oracle agrees within the tolerance."""
+    c = dg.config(1, scale=0.2)
+    s = dg.make_sample(c)
+    res, evals = {}, {}
+    for skip in (1, 0):
+        ctx.set_option(binding.ET_OPT_TC_SKIP, skip)
+        try:
+            with force_kernel(ctx, 2):
+                res[skip] = ctx.permutation_test(s.x, s.xbar, sigma, nperm, c.perm_seed)
+                st = ctx.stats()
+                assert st.dominant_kernel == "k_perm_tc"
+                evals[skip] = st.pair_evals
+        finally:
+            ctx.set_option(binding.ET_OPT_TC_SKIP, 1)
+    assert evals[1] < 0.6 * evals[0], evals                       # the skip is in force
+    assert (res[1].T_perm == res[0].T_perm).all() and res[1].observed == res[0].observed
+    assert (res[1].count_gt, res[1].n_near) == (res[0].count_gt, res[0].n_near)
+    exp = oracle.perm_test(s.x, s.xbar, sigma, 4, c.perm_seed)
+    assert abs(res[1].observed.T - exp.observed.T) <= TOL * exp.observed.term_scale
+    assert np.abs(res[1].T_perm[:4] - exp.T_perm).max() <= TOL * exp.observed.term_scale
+
+
 def test_perm_tc_weighted(ctx):
     c = dg.config(3, scale=0.012)  # 2400 + 2400 events, weights U[-0.5, 1.5]: signed hi digit
     s = dg.make_sample(c)
