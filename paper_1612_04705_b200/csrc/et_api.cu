@@ -17,8 +17,6 @@
 #include "et_tc.cuh"
 #include "et_scp.cuh"
 
-#include <cub/device/device_radix_sort.cuh>  // library sort of (key, row) for the row order of the contraction (et_tc.cuh)
-
 using namespace et;
 
 namespace {
@@ -78,7 +76,7 @@ struct et_ctx {
     Buf scpcnt, scpS;
     Buf selcand, selsave;  // radix select: candidate lists of the index half, state after the key32 half
     // row order of the tensor-core contraction (et_tc.cuh, k_morton_keys): keys, order[new] = old, inv[old] = new, sorted records
-    Buf tckey, tckey2, tcidx, tcorder, tcinv, recS, cubtmp;
+    Buf tckey, tckey2, tcidx, tcorder, tcinv, recS, rshist;  // rshist: the radix sort's histogram
     Buf tcboxes, tcbitmap;          // exact skipping of far K blocks: bounding boxes, bitmap[row tile][K block]
     int64_t opt_tc_skip = 1;        // ET_OPT_TC_SKIP
     bool tc_sorted = false;         // maskT of the last label write is in the sorted order (tcorder / tcinv hold it)
@@ -1163,23 +1161,36 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         if (!reuse_labels) {
             tc::MortonParams M{};
             M.ncls = L.ncls; M.dim = dim;
-            M.bits = std::min(28 / dim, 10);
+            M.bits = std::min(20 / dim, 10);
             for (int c = 0; c <= L.ncls; ++c) M.seg_pos[c] = L.seg_pos[c];
             for (int c = 0; c < L.ncls; ++c) M.seg_count[c] = L.seg_count[c];
             for (int k = 0; k < dim; ++k) M.half[k] = (float)ctx->uhalf[k];
             ET_TRY(ensure(ctx, ctx->tckey, (size_t)L.npad * sizeof(uint32_t)));
             ET_TRY(ensure(ctx, ctx->tckey2, (size_t)L.npad * sizeof(uint32_t)));
             ET_TRY(ensure(ctx, ctx->tcidx, (size_t)L.npad * sizeof(int)));
+            // keys into (tckey2, tcorder); pass 1 -> (tckey, tcidx); pass 2 -> (tckey2, tcorder): the order ends in tcorder
             tc::k_morton_keys<<<(unsigned)((L.npad + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
-                recT, rec_floats(dim), L.npad, M, static_cast<uint32_t *>(ctx->tckey.p), static_cast<int *>(ctx->tcidx.p));
+                recT, rec_floats(dim), L.npad, M, static_cast<uint32_t *>(ctx->tckey2.p), static_cast<int *>(ctx->tcorder.p));
             LAUNCH_CHECK();
-            size_t tmp_bytes = 0;
-            CUDA_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, static_cast<const uint32_t *>(ctx->tckey.p), static_cast<uint32_t *>(ctx->tckey2.p),
-                                                     static_cast<const int *>(ctx->tcidx.p), static_cast<int *>(ctx->tcorder.p), (int)L.npad, 0, 30, ctx->stream));
-            ET_TRY(ensure(ctx, ctx->cubtmp, tmp_bytes));
-            CUDA_TRY(cub::DeviceRadixSort::SortPairs(ctx->cubtmp.p, tmp_bytes, static_cast<const uint32_t *>(ctx->tckey.p), static_cast<uint32_t *>(ctx->tckey2.p),
-                                                     static_cast<const int *>(ctx->tcidx.p), static_cast<int *>(ctx->tcorder.p), (int)L.npad, 0, 30, ctx->stream));
-            ctx->stats.launches += 3;
+            // at most 4096 tiles (one warp each) of at least 4096 elements
+            long long tile = std::max<long long>(4096, (L.npad + 4095) / 4096);
+            tile = (tile + 31) / 32 * 32;
+            const long long ntiles = (L.npad + tile - 1) / tile, nhist = (long long)tc::kRsBins * ntiles;
+            ET_TRY(ensure(ctx, ctx->rshist, (size_t)nhist * sizeof(uint32_t)));
+            uint32_t *ka = static_cast<uint32_t *>(ctx->tckey2.p), *kb2 = static_cast<uint32_t *>(ctx->tckey.p);
+            int *va = static_cast<int *>(ctx->tcorder.p), *vb = static_cast<int *>(ctx->tcidx.p);
+            const unsigned rs_grid = (unsigned)((ntiles + tc::kRsWarps - 1) / tc::kRsWarps);
+            for (int pass = 0; pass < 2; ++pass) {
+                tc::k_rs_hist<<<rs_grid, 32 * tc::kRsWarps, 0, ctx->stream>>>(ka, L.npad, pass * tc::kRsBits, tile, ntiles, static_cast<uint32_t *>(ctx->rshist.p));
+                LAUNCH_CHECK();
+                tc::k_rs_scan<<<1, 1024, 0, ctx->stream>>>(static_cast<uint32_t *>(ctx->rshist.p), nhist);
+                LAUNCH_CHECK();
+                tc::k_rs_scatter<<<rs_grid, 32 * tc::kRsWarps, 0, ctx->stream>>>(ka, va, L.npad, pass * tc::kRsBits, tile, ntiles,
+                                                                             static_cast<const uint32_t *>(ctx->rshist.p), kb2, vb);
+                LAUNCH_CHECK();
+                std::swap(ka, kb2);
+                std::swap(va, vb);
+            }
         }
         tc::k_order_gather<<<ctx->num_sms * 8, 256, 0, ctx->stream>>>(static_cast<const float4 *>(ctx->rec.p), static_cast<const int *>(ctx->tcorder.p), L.npad, F4,
                                                                     static_cast<int *>(ctx->tcinv.p), static_cast<float4 *>(ctx->recS.p));
@@ -1452,7 +1463,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
                    &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
                    &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave, &ctx->tckey, &ctx->tckey2, &ctx->tcidx, &ctx->tcorder,
-                   &ctx->tcinv, &ctx->recS, &ctx->cubtmp, &ctx->tcboxes, &ctx->tcbitmap};
+                   &ctx->tcinv, &ctx->recS, &ctx->rshist, &ctx->tcboxes, &ctx->tcbitmap};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);

@@ -838,9 +838,9 @@ __global__ void __launch_bounds__(kThreads) k_label_write_tc(long long N, long l
 // pair enters once with a symmetric quantised psi), but its TIME does: the board runs at its power cap and the energy of
 // an MMA follows the operand bits -- with neighbouring rows close in phase space the digit tiles of neighbouring j are
 // alike and far tiles are mostly zero: -2.3 % per launch at config 4 (profiles/r02_README.md).  So the contraction
-// runs on a copy of the records in Morton order: key = class << 28 | interleaved bits of the coordinates quantised over the
-// bounding box (padding rows: the largest key of their class, so every class keeps its row range), a stable sort of
-// (key, row), then order[new] = old, inv[old] = new and recS[new] = rec[old].  The labels are written through inv; the
+// runs on a copy of the records in Morton order: key = class << 20 | interleaved bits of the coordinates quantised over the
+// bounding box (padding rows: the largest key of their class, so every class keeps its row range), a stable radix sort of
+// (key, row) (k_rs_*: two passes of 11 bits over the 22-bit key), then order[new] = old, inv[old] = new and recS[new] = rec[old].  The labels are written through inv; the
 // escalation and every other kernel keep the layout order.
 struct MortonParams {
     int ncls, dim, bits;
@@ -855,7 +855,7 @@ __global__ void __launch_bounds__(kThreads) k_morton_keys(const float *__restric
     int cls = 0;
     for (int c = 0; c < M.ncls; ++c)
         if (row >= M.seg_pos[c]) cls = c;
-    uint32_t m = 0x0fffffffu;
+    uint32_t m = 0x000fffffu;
     if (row - M.seg_pos[cls] < M.seg_count[cls]) {
         uint32_t q[kMaxDimTC];
         const int top = (1 << M.bits) - 1;
@@ -868,9 +868,75 @@ __global__ void __launch_bounds__(kThreads) k_morton_keys(const float *__restric
         for (int b = M.bits - 1; b >= 0; --b)
             for (int k = 0; k < M.dim; ++k) m = (m << 1) | ((q[k] >> b) & 1u);
     }
-    key[row] = ((uint32_t)cls << 28) | m;
+    key[row] = ((uint32_t)cls << 20) | m;
     idx[row] = (int)row;
 }
+// Stable LSD radix sort of (key, value) pairs, kRsBits bits per pass: one warp per tile of `tile` consecutive elements
+// (a multiple of 32).  k_rs_hist: hist[bin * ntiles + t] = elements of tile t in bin; k_rs_scan: exclusive prefix in place
+// (bin-major, so equal digits keep their tile order); k_rs_scatter: the rank of an element inside its tile is the count of
+// earlier elements with the same digit -- earlier steps from the warp's shared-memory counter, the same step from
+// __match_any_sync -- so the pass is stable.
+constexpr int kRsBits = 11, kRsBins = 1 << kRsBits, kRsWarps = 4;
+__global__ void __launch_bounds__(32 * kRsWarps) k_rs_hist(const uint32_t *__restrict__ key, long long n, int shift, long long tile, long long ntiles,
+                                                          uint32_t *__restrict__ hist)
+{
+    __shared__ uint32_t cnt[kRsWarps][kRsBins];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long t = blockIdx.x * (long long)kRsWarps + w;
+    for (int b = lane; b < kRsBins; b += 32) cnt[w][b] = 0u;
+    __syncwarp();
+    if (t < ntiles) {
+        for (long long i = t * tile + lane; i < min(n, (t + 1) * tile); i += 32) atomicAdd(&cnt[w][(key[i] >> shift) & (kRsBins - 1)], 1u);
+        __syncwarp();
+        for (int b = lane; b < kRsBins; b += 32) hist[(long long)b * ntiles + t] = cnt[w][b];
+    }
+}
+// exclusive prefix sum of `total` counters in place; one block of 1024 threads, a contiguous chunk per thread
+__global__ void __launch_bounds__(1024) k_rs_scan(uint32_t *__restrict__ hist, long long total)
+{
+    __shared__ uint32_t part[1024];
+    const long long chunk = (total + 1023) / 1024, a = threadIdx.x * chunk, b = min(total, a + chunk);
+    uint32_t sum = 0u;
+    for (long long i = a; i < b; ++i) sum += hist[i];
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0u;
+        for (int k = 0; k < 1024; ++k) { const uint32_t v = part[k]; part[k] = run; run += v; }
+    }
+    __syncthreads();
+    uint32_t run = part[threadIdx.x];
+    for (long long i = a; i < b; ++i) { const uint32_t v = hist[i]; hist[i] = run; run += v; }
+}
+__global__ void __launch_bounds__(32 * kRsWarps) k_rs_scatter(const uint32_t *__restrict__ key_in, const int *__restrict__ val_in, long long n, int shift,
+                                                             long long tile, long long ntiles, const uint32_t *__restrict__ off,
+                                                             uint32_t *__restrict__ key_out, int *__restrict__ val_out)
+{
+    __shared__ uint32_t cnt[kRsWarps][kRsBins];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long t = blockIdx.x * (long long)kRsWarps + w;
+    for (int b = lane; b < kRsBins; b += 32) cnt[w][b] = 0u;
+    __syncwarp();
+    if (t >= ntiles) return;
+    const long long end = min(n, (t + 1) * tile);
+    for (long long i0 = t * tile; i0 < end; i0 += 32) {   // tile is a multiple of 32: the trip count is the warp's
+        const long long i = i0 + lane;
+        const bool valid = i < end;
+        const uint32_t k = valid ? key_in[i] : 0u;
+        const uint32_t d = valid ? (k >> shift) & (kRsBins - 1) : (uint32_t)kRsBins;   // invalid lanes: a group of their own
+        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t base = valid ? cnt[w][d] : 0u;
+        __syncwarp();
+        if (valid && lane == __ffs((int)peers) - 1) cnt[w][d] = base + (uint32_t)__popc(peers);
+        __syncwarp();
+        if (valid) {
+            const long long pos = (long long)off[(long long)d * ntiles + t] + base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+            key_out[pos] = k;
+            val_out[pos] = val_in[i];
+        }
+    }
+}
+
 // inv[order[r]] = r, recS[r] = rec[order[r]] (F4 float4 per row); one thread per float4
 __global__ void k_order_gather(const float4 *__restrict__ rec, const int *__restrict__ order, long long npad, int F4, int *__restrict__ inv,
                                float4 *__restrict__ recS)
