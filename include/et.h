@@ -142,8 +142,10 @@ typedef enum {
                                (DESIGN.md section 6).  T stays within the 1e-6 tolerance either way    */
     ET_OPT_TC_ORDER = 5,    /* row order of the tensor-core contraction: 1 (default) = the records of every class
                                segment in Morton order of their coordinates (a sorted copy; labels written
-                               through the inverse map; unit weights only), 0 = the layout order.  The
-                               integer sums of the unweighted contraction do not depend on it bit for bit, the
+                               through the inverse map), 0 = the layout order.  The integer sums of the
+                               unweighted contraction do not depend on it bit for bit (weighted sums: in
+                               the last bits, far inside the guard band; the keys come from the input
+                               coordinates, so a sigma scan and its single calls still agree exactly), the
                                time does: the board runs at its power cap and similar neighbouring rows
                                cost the tensor pipe less energy (-2.3 % per launch at BASELINE config 4)  */
     ET_OPT_TC_SKIP = 6,     /* exact skipping of far K blocks in the tensor-core contraction (needs ET_OPT_TC_ORDER):

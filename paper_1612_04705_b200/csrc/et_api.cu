@@ -81,7 +81,7 @@ struct et_ctx {
     int64_t opt_tc_skip = 1;        // ET_OPT_TC_SKIP
     bool tc_sorted = false;         // maskT of the last label write is in the sorted order (tcorder / tcinv hold it)
     int64_t opt_tc_order = 1;       // ET_OPT_TC_ORDER
-    double uhalf[ET_MAX_DIM] = {0};  // half range of the records' coordinate k over the bounding box (last prep)
+    Buf prepkey;                    // Morton key of every record row (k_prep)
     bool tc_attr_set = false;
     // NVTX ranges: the call and its spans (labels, O(N^2) kernels, escalation); ids of the open ones
     nvtxRangeId_t nvtx_call = 0, nvtx_span[8] = {0};
@@ -310,12 +310,16 @@ et_status run_prep_t(et_ctx *ctx, const TIn *x, const TIn *xbar, const double *w
     for (int k = 0; k < dim; ++k) {
         const double half = 0.5 * ((double)key2f(h[32 + 2 * k + 1]) - (double)key2f(h[32 + 2 * k])) * P.scale;
         ctx->umax2 += half * half;
-        ctx->uhalf[k] = half;
+        const double half_x = 0.5 * ((double)key2f(h[32 + 2 * k + 1]) - (double)key2f(h[32 + 2 * k]));
+        P.inv_half[k] = half_x > 0.0 ? 1.0 / half_x : 0.0;
     }
     P.n = L.n; P.nbar = L.nbar; P.npad = L.npad; P.dim = dim; P.ncls = L.ncls;
     for (int c = 0; c <= L.ncls; ++c) P.seg_pos[c] = L.seg_pos[c];
     for (int c = 0; c < L.ncls; ++c) P.seg_count[c] = L.seg_count[c];
     ET_TRY(ensure(ctx, ctx->rec, (size_t)L.npad * rec_floats(dim) * sizeof(float)));
+    ET_TRY(ensure(ctx, ctx->prepkey, (size_t)L.npad * sizeof(uint32_t)));
+    P.key_bits = std::min(20 / dim, 10);
+    P.key = static_cast<uint32_t *>(ctx->prepkey.p);
     k_prep<TIn><<<grid, 256, 0, ctx->stream>>>(x, xbar, wx, wxbar, src, P, static_cast<float *>(ctx->rec.p));
     LAUNCH_CHECK();
     return ET_OK;
@@ -1044,7 +1048,10 @@ __global__ void __launch_bounds__(256) k_esc_apply(const DevNear *__restrict__ n
 template <int D, class G>
 et_status launch_perm_tc(et_ctx *ctx, const tc::TCParams &P, int grid, bool weighted, bool skip)
 {
-    if (!weighted && skip) {  // far K blocks are not evaluated (et_tc.cuh, SKIP)
+    if (skip && weighted) {  // far K blocks are not evaluated (et_tc.cuh, SKIP)
+        CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, true, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
+        tc::k_perm_tc<D, true, G, true><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
+    } else if (skip) {
         CUDA_TRY(cudaFuncSetAttribute(tc::k_perm_tc<D, false, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::smem_tc(D)));
         tc::k_perm_tc<D, false, G, true><<<grid, G::kThreadsTC, G::smem_tc(D), ctx->stream>>>(P);
     } else if (weighted) {
@@ -1148,10 +1155,11 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     for (int c = 0; c < L.ncls; ++c) lo.seg_pos[c] = L.seg_pos[c];
     // row order of the contraction (et_tc.cuh): Morton order inside every class segment.  With reuse_labels the order that
     // the labels were written in is kept (the keys of another sigma could round differently).
-    // Unit weights only: there every pair enters once with a symmetric quantised psi, so the integer sums do not depend on
-    // the row order at all; with weights Psi_ij = w_j psi_ij is rounded per ordered pair and the order would show in the last
-    // bits (and the weighted 2-D configs gain nothing: 44.23 vs 44.24 ms per launch at config 3).
-    if (!reuse_labels) ctx->tc_sorted = ctx->opt_tc_order != 0 && !weighted;
+    // Unit weights: every pair enters once with a symmetric quantised psi, so the integer sums do not depend on the row
+    // order at all.  With weights Psi_ij = w_j psi_ij is rounded per ordered pair, so the order shows in the last bits of the
+    // sums (far inside the guard band); the keys come from the input coordinates and do not depend on sigma, so a sigma
+    // scan and its single calls still agree bit for bit.
+    if (!reuse_labels) ctx->tc_sorted = ctx->opt_tc_order != 0;
     const float *recT = static_cast<const float *>(ctx->rec.p);
     if (ctx->tc_sorted) {
         const int F4 = rec_floats(dim) / 4;
@@ -1159,18 +1167,12 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
         ET_TRY(ensure(ctx, ctx->tcinv, (size_t)L.npad * sizeof(int)));
         ET_TRY(ensure(ctx, ctx->recS, (size_t)L.npad * rec_floats(dim) * sizeof(float)));
         if (!reuse_labels) {
-            tc::MortonParams M{};
-            M.ncls = L.ncls; M.dim = dim;
-            M.bits = std::min(20 / dim, 10);
-            for (int c = 0; c <= L.ncls; ++c) M.seg_pos[c] = L.seg_pos[c];
-            for (int c = 0; c < L.ncls; ++c) M.seg_count[c] = L.seg_count[c];
-            for (int k = 0; k < dim; ++k) M.half[k] = (float)ctx->uhalf[k];
             ET_TRY(ensure(ctx, ctx->tckey, (size_t)L.npad * sizeof(uint32_t)));
             ET_TRY(ensure(ctx, ctx->tckey2, (size_t)L.npad * sizeof(uint32_t)));
             ET_TRY(ensure(ctx, ctx->tcidx, (size_t)L.npad * sizeof(int)));
-            // keys into (tckey2, tcorder); pass 1 -> (tckey, tcidx); pass 2 -> (tckey2, tcorder): the order ends in tcorder
-            tc::k_morton_keys<<<(unsigned)((L.npad + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
-                recT, rec_floats(dim), L.npad, M, static_cast<uint32_t *>(ctx->tckey2.p), static_cast<int *>(ctx->tcorder.p));
+            // keys (k_prep) into (tckey2, tcorder); pass 1 -> (tckey, tcidx); pass 2 -> (tckey2, tcorder): the order ends in tcorder
+            tc::k_key_iota<<<(unsigned)((L.npad + kThreads - 1) / kThreads), kThreads, 0, ctx->stream>>>(
+                static_cast<const uint32_t *>(ctx->prepkey.p), L.npad, static_cast<uint32_t *>(ctx->tckey2.p), static_cast<int *>(ctx->tcorder.p));
             LAUNCH_CHECK();
             // at most 4096 tiles (one warp each) of at least 4096 elements
             long long tile = std::max<long long>(4096, (L.npad + 4095) / 4096);
@@ -1463,7 +1465,7 @@ void et_destroy(et_ctx *ctx)
                    &ctx->count64, &ctx->maskT, &ctx->units, &ctx->tcpart, &ctx->tcQ, &ctx->tcR, &ctx->tcWpart, &ctx->tcW, &ctx->recP,
                    &ctx->shardbuf, &ctx->tcraw, &ctx->rec2, &ctx->tilecls2, &ctx->esccls, &ctx->escD, &ctx->nearbuf, &ctx->escw,
                    &ctx->scpcnt, &ctx->scpS, &ctx->selcand, &ctx->selsave, &ctx->tckey, &ctx->tckey2, &ctx->tcidx, &ctx->tcorder,
-                   &ctx->tcinv, &ctx->recS, &ctx->rshist, &ctx->tcboxes, &ctx->tcbitmap};
+                   &ctx->tcinv, &ctx->recS, &ctx->rshist, &ctx->tcboxes, &ctx->tcbitmap, &ctx->prepkey};
     for (Buf *b : bufs)
         if (b->p) cudaFree(b->p);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);

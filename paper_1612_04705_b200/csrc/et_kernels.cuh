@@ -93,6 +93,12 @@ struct PrepParams {
     int ncls;
     long long seg_pos[kMaxCls + 1];    // first padded row of each class segment (seg_pos[ncls] = npad)
     long long seg_count[kMaxCls];      // real rows in each class segment
+    // Morton key of every row for the row order of the tensor-core contraction (et_tc.cuh): class << 20 | the interleaved top
+    // key_bits bits per axis of (x - centre) / half range, in fp64 from the INPUT coordinates, so the key does not depend on
+    // sigma (a sigma scan and its single calls order the rows alike); padding rows get the largest key of their class
+    double inv_half[8];                // 1 / half range of coordinate k over the bounding box (0: a degenerate axis)
+    int key_bits;
+    uint32_t *key;                     // [npad], or nullptr
 };
 
 // Writes the pooled records.  src == nullptr: two classes, class 0 = x in input order, class 1 = xbar.
@@ -113,12 +119,27 @@ __global__ void k_prep(const TIn *__restrict__ x, const TIn *__restrict__ xbar, 
             else if (row - P.seg_pos[1] < P.nbar) s = P.n + (row - P.seg_pos[1]);
         }
         float *o = rec + row * F;
+        int cls = 0;
+        for (int c = 1; c < P.ncls; ++c)
+            if (row >= P.seg_pos[c]) cls = c;
         if (s < 0) {
             for (int k = 0; k < F; ++k) o[k] = 0.0f;
+            if (P.key) P.key[row] = ((uint32_t)cls << 20) | 0x000fffffu;
             continue;
         }
         const TIn *p = s < P.n ? x + s * P.dim : xbar + (s - P.n) * P.dim;
         for (int k = 0; k < P.dim; ++k) o[k] = (float)(((double)p[k] - P.centre[k]) * P.scale);
+        if (P.key) {
+            const int top = (1 << P.key_bits) - 1;
+            uint32_t q[8], m = 0u;
+            for (int k = 0; k < P.dim; ++k) {
+                const double t = (((double)p[k] - P.centre[k]) * P.inv_half[k] + 1.0) * 0.5 * (double)(1 << P.key_bits);
+                q[k] = (uint32_t)min(max((int)t, 0), top);
+            }
+            for (int b = P.key_bits - 1; b >= 0; --b)
+                for (int k = 0; k < P.dim; ++k) m = (m << 1) | ((q[k] >> b) & 1u);
+            P.key[row] = ((uint32_t)cls << 20) | m;
+        }
         double w = 1.0;
         if (wx) w = s < P.n ? wx[s] : wxbar[s - P.n];
         o[P.dim] = (float)w;

@@ -839,36 +839,16 @@ __global__ void __launch_bounds__(kThreads) k_label_write_tc(long long N, long l
 // an MMA follows the operand bits -- with neighbouring rows close in phase space the digit tiles of neighbouring j are
 // alike and far tiles are mostly zero: -2.3 % per launch at config 4 (profiles/r02_README.md).  So the contraction
 // runs on a copy of the records in Morton order: key = class << 20 | interleaved bits of the coordinates quantised over the
-// bounding box (padding rows: the largest key of their class, so every class keeps its row range), a stable radix sort of
+// bounding box (written by k_prep from the input coordinates; padding rows: the largest key of their class, so every class
+// keeps its row range), a stable radix sort of
 // (key, row) (k_rs_*: two passes of 11 bits over the 22-bit key), then order[new] = old, inv[old] = new and recS[new] = rec[old].  The labels are written through inv; the
 // escalation and every other kernel keep the layout order.
-struct MortonParams {
-    int ncls, dim, bits;
-    long long seg_pos[kMaxCls + 1], seg_count[kMaxCls];
-    float half[kMaxDimTC];  // half range of u_k over the bounding box (0: a degenerate axis)
-};
-__global__ void __launch_bounds__(kThreads) k_morton_keys(const float *__restrict__ rec, int F, long long npad, MortonParams M,
-                                                         uint32_t *__restrict__ key, int *__restrict__ idx)
+// the keys come from k_prep (PrepParams::key); the sort works on a copy and starts from the identity order
+__global__ void __launch_bounds__(kThreads) k_key_iota(const uint32_t *__restrict__ key_in, long long npad, uint32_t *__restrict__ key, int *__restrict__ idx)
 {
     const long long row = blockIdx.x * (long long)kThreads + threadIdx.x;
     if (row >= npad) return;
-    int cls = 0;
-    for (int c = 0; c < M.ncls; ++c)
-        if (row >= M.seg_pos[c]) cls = c;
-    uint32_t m = 0x000fffffu;
-    if (row - M.seg_pos[cls] < M.seg_count[cls]) {
-        uint32_t q[kMaxDimTC];
-        const int top = (1 << M.bits) - 1;
-        for (int k = 0; k < M.dim; ++k) {
-            const float h = M.half[k];
-            const float t = h > 0.f ? (rec[row * F + k] + h) / (2.f * h) * (float)(1 << M.bits) : 0.f;
-            q[k] = (uint32_t)min(max((int)t, 0), top);
-        }
-        m = 0u;
-        for (int b = M.bits - 1; b >= 0; --b)
-            for (int k = 0; k < M.dim; ++k) m = (m << 1) | ((q[k] >> b) & 1u);
-    }
-    key[row] = ((uint32_t)cls << 20) | m;
+    key[row] = key_in[row];
     idx[row] = (int)row;
 }
 // Stable LSD radix sort of (key, value) pairs, kRsBits bits per pass: one warp per tile of `tile` consecutive elements
