@@ -1228,7 +1228,8 @@ et_status run_perm_tc_g(et_ctx *ctx, const Layout &L, int dim, int nperm, uint64
     bool use_skip = false;
     const int bm_words = (NK + 31) / 32;
     long long marked_kb = total_kb;
-    if (ctx->tc_sorted && ctx->opt_tc_skip != 0) {
+    // (the bitmap is nT x NK bits: 15 MB at 2e6 rows, O(N^2); beyond 256 MB -- about 8e6 rows -- every block is evaluated)
+    if (ctx->tc_sorted && ctx->opt_tc_skip != 0 && (size_t)nT * (size_t)bm_words * sizeof(uint32_t) <= ((size_t)256 << 20)) {
         const int F = rec_floats(dim);
         ET_TRY(ensure(ctx, ctx->tcboxes, ((size_t)nT + (size_t)NK) * 2 * tc::kMaxDimTC * sizeof(float)));
         ET_TRY(ensure(ctx, ctx->tcbitmap, (size_t)nT * bm_words * sizeof(uint32_t) + 16));
